@@ -1,0 +1,148 @@
+/*
+ * fe_mf.h -- C-ABI of the B200-native matrix-free finite-element Helmholtz multivector apply
+ * and Chebyshev filter (hot path of arXiv 2208.07129).
+ *
+ * The library computes, entirely in hand-written sm_100a CUDA kernels and in IEEE FP64,
+ *
+ *     Y = A X,   A = K + sigma*M                        (Eq. 3, Eq. 6)
+ *
+ * for a degree-p (1..8) hexahedral GLL Lagrange discretisation with (p+1)^3 Gauss-Legendre
+ * quadrature points per cell, by sum factorisation (Alg. 1
+ * Alg. 2, Eq. 15): gather -> N1D x3 -> D~1D x3 -> quadrature-point scaling -> D~1D^T x3 ->
+ * N1D^T x3 -> scatter-add, fused in one kernel per (cell, vector-batch) as in PAPER.md:690-740
+ * (Alg. 4), plus the scaled Chebyshev three-term recurrence of PAPER.md:931-975 (Alg. 6 l.2-17)
+ * with the axpby folded into the apply as in PAPER.md:1169-1174 (Eq. B.1).
+ *
+ * Multivector layout (all entry points): X[J*nvec + beta], J = ix + nd_x*(iy + nd_y*iz) the
+ * lexicographic global node index (x fastest), beta the vector index, INNERMOST -- the paper's
+ * BCV layout with one batch b = nvec (Fig. 1).  nd_d = ncells_d*p (periodic) or
+ * ncells_d*p + 1 (Dirichlet; boundary nodes are counted, PAPER.md:542/820/899 DoF counts).
+ *
+ * Dirichlet convention (C^T A C of Eq. 6 literally): boundary entries of X are
+ * ignored (read as 0), boundary entries of Y are written as 0.
+ *
+ * Pointers named *_dev are DEVICE pointers on the context's CUDA device; *_host are HOST
+ * pointers.  The caller owns X, Y and the stream; the context owns tables, geometry and
+ * workspace.  Nothing is thrown or aborted across this boundary: every call returns a code and
+ * leaves a message retrievable with fe_mf_last_error().  There is no CPU fallback.
+ */
+#ifndef FE_MF_H
+#define FE_MF_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fe_mf_ctx fe_mf_ctx; /* opaque, library-owned */
+
+enum { FE_MF_OK = 0, FE_MF_EINVAL = 1, FE_MF_ENOMEM = 2, FE_MF_ECUDA = 3, FE_MF_EUNSUPPORTED = 4 };
+enum { FE_BC_PERIODIC = 0, FE_BC_DIRICHLET = 1 };
+enum { FE_GEOM_AFFINE = 0, FE_GEOM_QPOINT = 1 };
+
+/*
+ * fe_mf_create -- build a context: 1D tables N1D[q][i] = l_i(xq_q), D~1D[q][r] = l~_r'(xq_q)
+ * and Gauss weights in extended precision on the host, the geometric factors
+ * G^(s,d) = (J^-1 J^-T)_sd det J w_Q and G = sigma det J w_Q (mu = 1, kappa =
+ * sigma), and upload them.
+ *   out            receives the context (NULL on failure).
+ *   ncx,ncy,ncz    cells per direction (>= 1; >= 2 in every direction if periodic).
+ *   p              FE degree, 1..8; n_q = n_p = p+1.
+ *   sigma          A = K + sigma*M.
+ *   bc             FE_BC_PERIODIC | FE_BC_DIRICHLET (homogeneous).
+ *   geom           FE_GEOM_AFFINE: one symmetric 3x3 factor per cell, J taken at the cell centre
+ *                  (exact for parallelepipeds; "a linear map exists", Eq. 23);
+ *                  FE_GEOM_QPOINT: 6 metric entries + 1 mass factor stored per quadrature point
+ *                  from the trilinear map of the 8 cell vertices (Eq. 7c evaluated "at xi_Q").
+ *   box_lo,box_hi  HOST, 3 doubles each: the box of the uniform Cartesian mesh (used when
+ *                  vertices_host == NULL; must satisfy hi > lo).
+ *   vertices_host  HOST, NULL or [(ncz+1)][(ncy+1)][(ncx+1)][3] doubles; copied.  For periodic
+ *                  meshes the vertices on opposite box faces must match up to the box period.
+ *   cuda_device    device ordinal.
+ * Errors: EINVAL (null out, bad sizes/p/bc/geom, hi <= lo, non-positive det J at a quadrature
+ * point), ENOMEM, ECUDA, EUNSUPPORTED (device is not sm_100).
+ */
+int fe_mf_create(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
+                 const double box_lo[3], const double box_hi[3], const double *vertices_host,
+                 int cuda_device);
+
+/* nd_x*nd_y*nd_z including Dirichlet boundary nodes; -1 if ctx is NULL. */
+long long fe_mf_ndofs(const fe_mf_ctx *ctx);
+
+/*
+ * fe_mf_apply -- Y = (K + sigma M) X for nvec vectors (Eq. 6, Eq. 17).
+ *   X_dev  DEVICE, read-only, ndofs*nvec doubles, layout above.
+ *   Y_dev  DEVICE, overwritten, same shape; must not alias X_dev.
+ *   nvec   >= 1.
+ *   cuda_stream  a cudaStream_t (NULL = default stream).  All work is enqueued on it; the call
+ *                does not synchronise the host.
+ * Errors: EINVAL (null pointers, nvec < 1, aliasing), ECUDA.
+ */
+int fe_mf_apply(fe_mf_ctx *ctx, const double *X_dev, double *Y_dev, int nvec, void *cuda_stream);
+
+/*
+ * fe_mf_apply_axpby -- the fused form of Eq. (B.1) without mass scaling:
+ *     Z <- alpha * A * W  +  beta * Z  +  gamma * W
+ * W_dev read-only, Z_dev updated in place, no aliasing.  This is the one step the Chebyshev
+ * recurrence is built from (Alg. 6 l.10 and l.15).  Dirichlet: boundary rows get beta*Z + gamma*W.
+ */
+int fe_mf_apply_axpby(fe_mf_ctx *ctx, double alpha, const double *W_dev, double beta, double gamma,
+                      double *Z_dev, int nvec, void *cuda_stream);
+
+/*
+ * fe_cheb_filter -- scaled Chebyshev filter of degree m (Alg. 6 lines 2-17, garbled
+ * lines reconstructed as in SURVEY.md §8(c) step 6 / DESIGN.md reading 10):
+ *     e=(b-a)/2; c=(b+a)/2; s=e/(a0-c); s1=s; g=2/s1; a1=s1/e; a2=-c;  Y = a1 A X + a1 a2 X;
+ *     for d=2..m: s2=1/(g-s); a1=2 s2/e; a2=-s s2;  X <- a1 A Y + a2 X - c a1 Y; swap(X,Y); s=s2;
+ *   X_dev  DEVICE, input AND scratch: on return it holds iterate m-1 (for m == 1: unchanged).
+ *   Y_dev  DEVICE, output: the filtered block (always delivered here).
+ *   a,b    the damped interval [a, b] (a = upper bound of the wanted spectrum, b >= lambda_max);
+ *   a0     lower bound of the spectrum.  Requires m >= 1, b > a, a0 < a.
+ * The scalar recurrence runs on the host in double; the m fused applies are stream-ordered.
+ * Errors: EINVAL, ECUDA.
+ */
+int fe_cheb_filter(fe_mf_ctx *ctx, double *X_dev, double *Y_dev, int nvec, int m, double a, double b,
+                   double a0, void *cuda_stream);
+
+/*
+ * fe_mf_apply_host -- end-to-end convenience: same as fe_mf_apply but X_host / Y_host are HOST
+ * buffers (pinned memory recommended).  The library stages column blocks through an internal
+ * device workspace (H2D copy, kernels, D2H copy, overlapped on internal streams) and returns
+ * after Y_host is complete.  Errors as fe_mf_apply plus ENOMEM.
+ */
+int fe_mf_apply_host(fe_mf_ctx *ctx, const double *X_host, double *Y_host, int nvec);
+
+/*
+ * fe_fill_uniform -- synthetic-input generator (NOT part of the operator): fills
+ * out_dev[k] = 2*((splitmix64(seed + (offset+k)*0x9E3779B97F4A7C15) >> 11) * 2^-53) - 1 for
+ * k < count, bit-identical to the Python generator in paper_2208_07129_b200/inputs.py
+ * (SURVEY.md §8(d)).  DEVICE pointer on the current device; stream-ordered.
+ */
+int fe_fill_uniform(double *out_dev, long long count, unsigned long long seed, long long offset,
+                    void *cuda_stream);
+
+/*
+ * fe_probe_peaks -- box peaks for the roofline (BASELINE.json north_star: "peaks measured on the box
+ * by a stream/DGEMM microbenchmark"): FP64 FMA-chain rate in TFLOP/s (2 flops per DFMA) and FP64
+ * stream-copy bandwidth in GB/s (read + write bytes), best of 5 after one warm-up, on cuda_device's
+ * default stream.  Synchronises the host.  HOST output pointers.
+ */
+int fe_probe_peaks(double *fp64_tflops, double *hbm_gbs, int cuda_device);
+
+/* Introspection used by bench.py / tests: vectors per thread block chosen for this nvec, the
+ * number of kernel launches the last call enqueued, and the dominant kernel's name. */
+int fe_mf_batch_width(const fe_mf_ctx *ctx, int nvec);
+int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
+
+/* Select a kernel variant (0 = default).  For profiling/ablation only; returns EINVAL if unknown. */
+int fe_mf_set_variant(fe_mf_ctx *ctx, int variant);
+
+/* Message of the last failing call on ctx; with ctx == NULL, of the last failing fe_mf_create on
+ * this thread.  Never NULL. */
+const char *fe_mf_last_error(const fe_mf_ctx *ctx);
+
+void fe_mf_destroy(fe_mf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FE_MF_H */

@@ -1,0 +1,226 @@
+// Included by fe_mf.cu: kernel selection and the stream-ordered entry points.
+
+namespace {
+
+constexpr size_t kMaxSmem = 232448;  // 227 KB opt-in per block on sm_100
+
+// General kernel: 4 tiles of n^3*bv doubles.  Keep >= 2 blocks per SM resident.
+int general_bv(int p, int nvec) {
+  const int nn = (p + 1) * (p + 1) * (p + 1);
+  int bv = 32;
+  while (bv > 1 && ((size_t)4 * nn * bv * 8 > kMaxSmem / 2 - 1024 || bv > nvec)) bv >>= 1;
+  return bv;
+}
+
+template <int PDEG>
+cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
+  constexpr int NN = (PDEG + 1) * (PDEG + 1) * (PDEG + 1);
+  const size_t smem = (size_t)4 * NN * prm.bv * sizeof(double);
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(fe::fe_apply_general<PDEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  const long long grid = ncells * prm.nvb;
+  fe::fe_apply_general<PDEG><<<(unsigned)grid, 256, smem, st>>>(prm);
+  return cudaGetLastError();
+}
+
+fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
+  fe::ApplyParams P;
+  P.W = W; P.Z = Z; P.geom = c->geom_dev;
+  for (int k = 0; k < 7; ++k) P.ug[k] = c->ug[k];
+  P.alpha = alpha;
+  P.ncx = c->ncx; P.ncy = c->ncy; P.ncz = c->ncz;
+  P.ndx = c->ndx; P.ndy = c->ndy; P.ndz = c->ndz;
+  P.nvec = nvec; P.bv = bv; P.nvb = (nvec + bv - 1) / bv;
+  P.dirichlet = (c->bc == FE_BC_DIRICHLET) ? 1 : 0;
+  P.geom_mode = c->geom_mode;
+  return P;
+}
+
+// Z += alpha * A * W  (Z already initialised).  Counts launches into c->last_launches.
+int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st) {
+  const int bv = general_bv(c->p, nvec);
+  const fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
+  if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
+  cudaError_t e = cudaErrorInvalidValue;
+  switch (c->p) {
+    case 1: e = launch_general<1>(P, c->ncells, st); break;
+    case 2: e = launch_general<2>(P, c->ncells, st); break;
+    case 3: e = launch_general<3>(P, c->ncells, st); break;
+    case 4: e = launch_general<4>(P, c->ncells, st); break;
+    case 5: e = launch_general<5>(P, c->ncells, st); break;
+    case 6: e = launch_general<6>(P, c->ncells, st); break;
+    case 7: e = launch_general<7>(P, c->ncells, st); break;
+    case 8: e = launch_general<8>(P, c->ncells, st); break;
+  }
+  if (e != cudaSuccess) return fail(c, FE_MF_ECUDA, std::string("apply kernel launch: ") + cudaGetErrorString(e));
+  c->last_launches += 1;
+  return FE_MF_OK;
+}
+
+int stream_grid(size_t count) {
+  size_t b = (count + 255) / 256;
+  if (b > 148 * 16) b = 148 * 16;
+  if (b < 1) b = 1;
+  return (int)b;
+}
+
+// Z <- beta*Z + gamma*W, stream-ordered (S1 / the axpby half of S9).
+int launch_init(fe_mf_ctx* c, double* Z, const double* W, double beta, double gamma, size_t count, cudaStream_t st) {
+  if (beta == 0.0 && gamma == 0.0) {
+    FE_CUDA(c, cudaMemsetAsync(Z, 0, count * sizeof(double), st));
+  } else if (beta == 0.0) {
+    fe::fe_scale_copy_kernel<<<stream_grid(count), 256, 0, st>>>(Z, W, gamma, count);
+    FE_CUDA(c, cudaGetLastError());
+  } else {
+    fe::fe_axpby_kernel<<<stream_grid(count / 2 + 1), 256, 0, st>>>(Z, W, beta, gamma, count);
+    FE_CUDA(c, cudaGetLastError());
+  }
+  c->last_launches += 1;
+  return FE_MF_OK;
+}
+
+int check_io(fe_mf_ctx* c, const double* W, const double* Z, int nvec) {
+  if (!c) return FE_MF_EINVAL;
+  if (!W || !Z) return fail(c, FE_MF_EINVAL, "null device pointer");
+  if (nvec < 1) return fail(c, FE_MF_EINVAL, "nvec must be >= 1");
+  const size_t bytes = (size_t)c->ndof * nvec * sizeof(double);
+  const char* a = (const char*)W; const char* b = (const char*)Z;
+  if (a < b + bytes && b < a + bytes) return fail(c, FE_MF_EINVAL, "input and output alias");
+  return FE_MF_OK;
+}
+
+}  // namespace
+
+extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_dev, double beta, double gamma,
+                                 double* Z_dev, int nvec, void* cuda_stream) {
+  int rc = check_io(ctx, W_dev, Z_dev, nvec);
+  if (rc) return rc;
+  DeviceGuard guard(ctx->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  ctx->last_launches = 0;
+  const size_t count = (size_t)ctx->ndof * nvec;
+  rc = launch_init(ctx, Z_dev, W_dev, beta, gamma, count, st);
+  if (rc) return rc;
+  return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st);
+}
+
+extern "C" int fe_mf_apply(fe_mf_ctx* ctx, const double* X_dev, double* Y_dev, int nvec, void* cuda_stream) {
+  return fe_mf_apply_axpby(ctx, 1.0, X_dev, 0.0, 0.0, Y_dev, nvec, cuda_stream);
+}
+
+extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int nvec, int m, double a, double b,
+                              double a0, void* cuda_stream) {
+  int rc = check_io(ctx, X_dev, Y_dev, nvec);
+  if (rc) return rc;
+  if (m < 1) return fail(ctx, FE_MF_EINVAL, "m must be >= 1");
+  if (!(b > a)) return fail(ctx, FE_MF_EINVAL, "need b > a (inverted or empty damping interval)");
+  if (!(a0 < a)) return fail(ctx, FE_MF_EINVAL, "need a0 < a");
+  DeviceGuard guard(ctx->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t count = (size_t)ctx->ndof * nvec;
+  int launches = 0;
+  // Alg. 6 lines 2-9 (garbled lines per DESIGN.md reading 10)
+  const double e = (b - a) / 2.0;
+  const double c = (b + a) / 2.0;
+  double sigma = e / (a0 - c);
+  const double sigma1 = sigma;
+  const double gamma = 2.0 / sigma1;
+  double alpha1 = sigma1 / e;
+  double alpha2 = -c;
+  double* X = X_dev; double* Y = Y_dev;
+  // line 10: Y <- alpha1 A X + alpha1 alpha2 X
+  rc = fe_mf_apply_axpby(ctx, alpha1, X, 0.0, alpha1 * alpha2, Y, nvec, cuda_stream);
+  if (rc) return rc;
+  launches += ctx->last_launches;
+  for (int d = 2; d <= m; ++d) {
+    const double sigma2 = 1.0 / (gamma - sigma);
+    alpha1 = 2.0 * sigma2 / e;
+    alpha2 = -sigma * sigma2;
+    // line 15: X <- alpha1 A Y + alpha2 X - c alpha1 Y ; line 16: swap
+    rc = fe_mf_apply_axpby(ctx, alpha1, Y, alpha2, -(c * alpha1), X, nvec, cuda_stream);
+    if (rc) return rc;
+    launches += ctx->last_launches;
+    double* t = X; X = Y; Y = t;
+    sigma = sigma2;
+  }
+  if (Y != Y_dev) {  // m even: the result sits in the caller's X buffer; exchange contents
+    fe::fe_swap_kernel<<<stream_grid(count), 256, 0, st>>>(X_dev, Y_dev, count);
+    FE_CUDA(ctx, cudaGetLastError());
+    launches += 1;
+  }
+  ctx->last_launches = launches;
+  return FE_MF_OK;
+}
+
+extern "C" int fe_mf_apply_host(fe_mf_ctx* ctx, const double* X_host, double* Y_host, int nvec) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (!X_host || !Y_host) return fail(ctx, FE_MF_EINVAL, "null host pointer");
+  if (nvec < 1) return fail(ctx, FE_MF_EINVAL, "nvec must be >= 1");
+  DeviceGuard guard(ctx->device);
+  // column chunks: copies of chunk k+1 / k-1 overlap the kernels of chunk k on two streams
+  int nchunks = (nvec >= 16) ? 4 : 1;
+  int cw = (nvec + nchunks - 1) / nchunks;
+  cw = (cw + 3) / 4 * 4;
+  if (cw > nvec) cw = nvec;
+  nchunks = (nvec + cw - 1) / cw;
+  const size_t per = (size_t)ctx->ndof * cw;
+  const int nbuf = nchunks > 1 ? 2 : 1;
+  if (ctx->ws_elems < per * nbuf) {
+    if (ctx->ws_x) cudaFree(ctx->ws_x);
+    if (ctx->ws_y) cudaFree(ctx->ws_y);
+    ctx->ws_x = ctx->ws_y = nullptr; ctx->ws_elems = 0;
+    if (cudaMalloc(&ctx->ws_x, per * nbuf * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&ctx->ws_y, per * nbuf * sizeof(double)) != cudaSuccess) {
+      if (ctx->ws_x) cudaFree(ctx->ws_x);
+      ctx->ws_x = nullptr; (void)cudaGetLastError();
+      return fail(ctx, FE_MF_ENOMEM, "device workspace allocation failed");
+    }
+    ctx->ws_elems = per * nbuf;
+  }
+  for (int i = 0; i < 2; ++i)
+    if (!ctx->hs[i]) FE_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->hs[i], cudaStreamNonBlocking));
+  int launches = 0;
+  for (int k = 0; k < nchunks; ++k) {
+    const int c0 = k * cw, w = (c0 + cw <= nvec) ? cw : (nvec - c0);
+    cudaStream_t st = ctx->hs[k & 1];
+    double* dx = ctx->ws_x + (size_t)(k % nbuf) * per;
+    double* dy = ctx->ws_y + (size_t)(k % nbuf) * per;
+    FE_CUDA(ctx, cudaMemcpy2DAsync(dx, (size_t)w * 8, X_host + c0, (size_t)nvec * 8, (size_t)w * 8, (size_t)ctx->ndof,
+                                   cudaMemcpyHostToDevice, st));
+    int rc = fe_mf_apply(ctx, dx, dy, w, st);
+    if (rc) return rc;
+    launches += ctx->last_launches;
+    FE_CUDA(ctx, cudaMemcpy2DAsync(Y_host + c0, (size_t)nvec * 8, dy, (size_t)w * 8, (size_t)w * 8, (size_t)ctx->ndof,
+                                   cudaMemcpyDeviceToHost, st));
+  }
+  FE_CUDA(ctx, cudaStreamSynchronize(ctx->hs[0]));
+  FE_CUDA(ctx, cudaStreamSynchronize(ctx->hs[1]));
+  ctx->last_launches = launches;
+  return FE_MF_OK;
+}
+
+extern "C" int fe_fill_uniform(double* out_dev, long long count, unsigned long long seed, long long offset,
+                               void* cuda_stream) {
+  if (!out_dev || count < 0) return FE_MF_EINVAL;
+  if (count == 0) return FE_MF_OK;
+  fe::fe_fill_uniform_kernel<<<stream_grid((size_t)count), 256, 0, (cudaStream_t)cuda_stream>>>(out_dev, count, seed, offset);
+  return cudaGetLastError() == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
+}
+
+extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
+  if (!ctx || nvec < 1) return -1;
+  return general_bv(ctx->p, nvec);
+}
+
+extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx->last_launches : -1; }
+
+extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (variant != 0) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  ctx->variant = variant;
+  return FE_MF_OK;
+}

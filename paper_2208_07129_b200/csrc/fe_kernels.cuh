@@ -1,0 +1,206 @@
+// Device code, part 1: shared declarations, constant tables, the general ("v1") fused kernel.
+// One thread block = one FE cell x BV vectors; the whole of Alg. 2 / Alg. 4 (PAPER.md:209-247,
+// 690-740) runs between one gather and one scatter with all intermediates in shared memory.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fe {
+
+constexpr int KMAXN = 9;
+
+// 1D tables per degree p (functions of p only, so contexts can share them).
+// c_N[p][q*n+i] = N1D, c_D[p][q*n+r] = D~1D, c_w[p][q] = Gauss weights.
+__constant__ double c_N[KMAXN][KMAXN * KMAXN];
+__constant__ double c_D[KMAXN][KMAXN * KMAXN];
+__constant__ double c_w[KMAXN][KMAXN];
+
+struct ApplyParams {
+  const double* __restrict__ W;   // input multivector  [ndof][nvec]
+  double* __restrict__ Z;         // output multivector [ndof][nvec], pre-initialised; Z += alpha*A*W
+  const double* __restrict__ geom;  // per-q-point: [cell][7][n^3]; per-cell: [cell][7]; or nullptr (uniform)
+  double ug[7];                   // uniform Cartesian: G00,G01,G02,G11,G12,G22 (x det J), sigma*det J
+  double alpha;
+  int ncx, ncy, ncz;
+  int ndx, ndy, ndz;
+  int nvec;
+  int bv;                         // vectors per block
+  int nvb;                        // ceil(nvec / bv)
+  int dirichlet;                  // 1: boundary nodes read as 0 / not written
+  int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
+};
+
+// y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.
+template <int N, bool TRANS, bool ADD>
+__device__ __forceinline__ void line_contract(const double* __restrict__ M, const double* src, int sstride,
+                                              double* dst, int dstride) {
+  double x[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) x[i] = src[i * sstride];
+#pragma unroll
+  for (int q = 0; q < N; ++q) {
+    double acc = ADD ? dst[q * dstride] : 0.0;
+#pragma unroll
+    for (int i = 0; i < N; ++i) acc = fma(TRANS ? M[i * N + q] : M[q * N + i], x[i], acc);
+    dst[q * dstride] = acc;
+  }
+}
+
+// All n^2 lines along direction DIR of a [n][n][n][bv] tile.
+template <int N, int DIR, bool TRANS, bool ADD>
+__device__ __forceinline__ void pass(const double* __restrict__ M, const double* src, double* dst, int bv,
+                                     int tid, int nthreads) {
+  const int nlines = N * N * bv;
+  for (int t = tid; t < nlines; t += nthreads) {
+    const int beta = t % bv, l = t / bv;
+    const int a = l % N, b = l / N;
+    int base, stride;
+    if (DIR == 0) { base = (N * a + N * N * b) * bv; stride = bv; }
+    else if (DIR == 1) { base = (a + N * N * b) * bv; stride = N * bv; }
+    else { base = (a + N * b) * bv; stride = N * N * bv; }
+    line_contract<N, TRANS, ADD>(M, src + base + beta, stride, dst + base + beta, stride);
+  }
+}
+
+__device__ __forceinline__ long long global_node(const ApplyParams& P, int ix, int iy, int iz) {
+  return (long long)ix + (long long)P.ndx * ((long long)iy + (long long)P.ndy * iz);
+}
+
+template <int PDEG>
+__global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
+  constexpr int N = PDEG + 1, NN = N * N * N;
+  extern __shared__ double smem[];
+  const int bv = P.bv;
+  double* T = smem;
+  double* T0 = T + NN * bv;
+  double* T1 = T0 + NN * bv;
+  double* T2 = T1 + NN * bv;
+  const int tid = threadIdx.x, nth = blockDim.x;
+  const int vb = blockIdx.x % P.nvb;
+  const int cell = blockIdx.x / P.nvb;
+  const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
+  const int v0 = vb * bv;
+  const double* Nm = c_N[PDEG];
+  const double* Dm = c_D[PDEG];
+
+  // S2 gather (Q^(e), C): tile[i3][i2][i1][beta]  (Eq. 18)
+  for (int t = tid; t < NN * bv; t += nth) {
+    const int beta = t % bv, I = t / bv;
+    const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+    int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+    bool live = (v0 + beta) < P.nvec;
+    if (P.dirichlet) {
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+    } else {
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+    }
+    T0[t] = live ? P.W[global_node(P, ix, iy, iz) * P.nvec + v0 + beta] : 0.0;
+  }
+  __syncthreads();
+  // S3 interpolate (Alg. 1)
+  pass<N, 0, false, false>(Nm, T0, T1, bv, tid, nth); __syncthreads();
+  pass<N, 1, false, false>(Nm, T1, T0, bv, tid, nth); __syncthreads();
+  pass<N, 2, false, false>(Nm, T0, T, bv, tid, nth); __syncthreads();
+  // S4 gradients (Alg. 2 l.2-4)
+  pass<N, 0, false, false>(Dm, T, T0, bv, tid, nth);
+  pass<N, 1, false, false>(Dm, T, T1, bv, tid, nth);
+  pass<N, 2, false, false>(Dm, T, T2, bv, tid, nth);
+  __syncthreads();
+  // S5 quadrature-point scaling (Alg. 2 l.5-6; Eq. 22-23)
+  for (int t = tid; t < NN * bv; t += nth) {
+    const int Q = t / bv;
+    const int q1 = Q % N, q2 = (Q / N) % N, q3 = Q / (N * N);
+    double g[7];
+    if (P.geom_mode == 2) {
+      const double* gp = P.geom + (size_t)cell * 7 * NN + Q;
+#pragma unroll
+      for (int k = 0; k < 7; ++k) g[k] = __ldg(gp + k * NN);
+    } else {
+      const double wq = c_w[PDEG][q1] * c_w[PDEG][q2] * c_w[PDEG][q3];
+      if (P.geom_mode == 1) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) g[k] = __ldg(P.geom + (size_t)cell * 7 + k) * wq;
+      } else {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) g[k] = P.ug[k] * wq;
+      }
+    }
+    const double a = T0[t], b = T1[t], c = T2[t];
+    T0[t] = g[0] * a + g[1] * b + g[2] * c;
+    T1[t] = g[1] * a + g[3] * b + g[4] * c;
+    T2[t] = g[2] * a + g[4] * b + g[5] * c;
+    T[t] = g[6] * T[t];
+  }
+  __syncthreads();
+  // S6 transposed gradients (Alg. 2 l.7-9)
+  pass<N, 0, true, true>(Dm, T0, T, bv, tid, nth); __syncthreads();
+  pass<N, 1, true, true>(Dm, T1, T, bv, tid, nth); __syncthreads();
+  pass<N, 2, true, true>(Dm, T2, T, bv, tid, nth); __syncthreads();
+  // S7 integrate (N^T)
+  pass<N, 0, true, false>(Nm, T, T0, bv, tid, nth); __syncthreads();
+  pass<N, 1, true, false>(Nm, T0, T1, bv, tid, nth); __syncthreads();
+  pass<N, 2, true, false>(Nm, T1, T0, bv, tid, nth); __syncthreads();
+  // S8 scatter-add (Q^(e)T, C^T)
+  for (int t = tid; t < NN * bv; t += nth) {
+    const int beta = t % bv, I = t / bv;
+    const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+    int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+    bool live = (v0 + beta) < P.nvec;
+    if (P.dirichlet) {
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+    } else {
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+    }
+    if (live) atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], P.alpha * T0[t]);
+  }
+}
+
+// S1 / S9 pre-pass: Z <- beta*Z + gamma*W  (Eq. B.1's bX + cY part)
+__global__ void fe_axpby_kernel(double* __restrict__ Z, const double* __restrict__ W, double beta, double gamma,
+                                size_t count) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  const size_t n2 = count / 2;
+  double2* Z2 = reinterpret_cast<double2*>(Z);
+  const double2* W2 = reinterpret_cast<const double2*>(W);
+  for (size_t k = i; k < n2; k += stride) {
+    double2 z = Z2[k], w = W2[k];
+    z.x = beta * z.x + gamma * w.x;
+    z.y = beta * z.y + gamma * w.y;
+    Z2[k] = z;
+  }
+  if (i == 0 && (count & 1)) Z[count - 1] = beta * Z[count - 1] + gamma * W[count - 1];
+}
+
+// Z <- gamma*W (beta == 0: Z is not read, so it may hold anything, e.g. NaN from a fresh allocation)
+__global__ void fe_scale_copy_kernel(double* __restrict__ Z, const double* __restrict__ W, double gamma, size_t count) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t k = i; k < count; k += stride) Z[k] = gamma * W[k];
+}
+
+__global__ void fe_swap_kernel(double* __restrict__ A, double* __restrict__ B, size_t count) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t k = i; k < count; k += stride) { double a = A[k]; A[k] = B[k]; B[k] = a; }
+}
+
+// Input generator; not part of the operator.
+__global__ void fe_fill_uniform_kernel(double* __restrict__ out, long long count, unsigned long long seed,
+                                       long long offset) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long k = i; k < count; k += stride) {
+    unsigned long long z = seed + (unsigned long long)(offset + k) * 0x9E3779B97F4A7C15ULL;
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    out[k] = 2.0 * ((double)(z >> 11) * 0x1.0p-53) - 1.0;
+  }
+}
+
+}  // namespace fe

@@ -1,0 +1,182 @@
+// C-ABI of include/fe_mf.h: context, host-side setup, kernel dispatch.  sm_100a only.
+#include "../../include/fe_mf.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "fe_kernels.cuh"
+#include "fe_tables.h"
+
+struct fe_mf_ctx {
+  int ncx, ncy, ncz, p, n, bc, geom;
+  int ndx, ndy, ndz;
+  long long ndof, ncells;
+  double sigma;
+  int device;
+  int geom_mode;            // 0 uniform, 1 per-cell, 2 per-q-point
+  double ug[7];
+  double* geom_dev = nullptr;
+  int variant = 0;
+  int last_launches = 0;
+  // fe_mf_apply_host workspace
+  double* ws_x = nullptr; double* ws_y = nullptr; size_t ws_elems = 0;
+  cudaStream_t hs[2] = {nullptr, nullptr};
+  std::string err;
+};
+
+static thread_local std::string g_create_err = "";
+
+namespace {
+
+int fail(fe_mf_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_err = msg;
+  return code;
+}
+
+#define FE_CUDA(c, call)                                                                      \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess)                                                                    \
+      return fail((c), FE_MF_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));       \
+  } while (0)
+
+struct DeviceGuard {
+  int prev = -1; bool ok = false;
+  explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess) ok = true; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+void cell_vertices(const fe_mf_ctx* c, const double* verts, const double lo[3], const double h[3], int ex, int ey,
+                   int ez, double v[8][3]) {
+  for (int k = 0; k < 8; ++k) {
+    int vx = ex + (k & 1), vy = ey + ((k >> 1) & 1), vz = ez + ((k >> 2) & 1);
+    if (verts) {
+      const double* s = verts + 3 * ((size_t)vx + (size_t)(c->ncx + 1) * ((size_t)vy + (size_t)(c->ncy + 1) * vz));
+      v[k][0] = s[0]; v[k][1] = s[1]; v[k][2] = s[2];
+    } else {
+      v[k][0] = lo[0] + h[0] * vx; v[k][1] = lo[1] + h[1] * vy; v[k][2] = lo[2] + h[2] * vz;
+    }
+  }
+}
+
+}  // namespace
+
+extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
+                            const double box_lo[3], const double box_hi[3], const double* vertices_host,
+                            int cuda_device) {
+  if (!out) return fail(nullptr, FE_MF_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (ncx < 1 || ncy < 1 || ncz < 1) return fail(nullptr, FE_MF_EINVAL, "cells per direction must be >= 1");
+  if (p < 1 || p > 8) return fail(nullptr, FE_MF_EINVAL, "p must be in 1..8");
+  if (bc != FE_BC_PERIODIC && bc != FE_BC_DIRICHLET) return fail(nullptr, FE_MF_EINVAL, "unknown bc");
+  if (geom != FE_GEOM_AFFINE && geom != FE_GEOM_QPOINT) return fail(nullptr, FE_MF_EINVAL, "unknown geom");
+  if (bc == FE_BC_PERIODIC && (ncx < 2 || ncy < 2 || ncz < 2))
+    return fail(nullptr, FE_MF_EINVAL, "periodic needs >= 2 cells per direction");
+  if (!vertices_host) {
+    if (!box_lo || !box_hi) return fail(nullptr, FE_MF_EINVAL, "box_lo/box_hi are NULL");
+    for (int d = 0; d < 3; ++d)
+      if (!(box_hi[d] > box_lo[d])) return fail(nullptr, FE_MF_EINVAL, "box_hi must exceed box_lo");
+  }
+  if ((long long)ncx * p + 1 > 2000000 || (long long)ncy * p + 1 > 2000000 || (long long)ncz * p + 1 > 2000000)
+    return fail(nullptr, FE_MF_EINVAL, "mesh too large");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev)
+    return fail(nullptr, FE_MF_ECUDA, "no such CUDA device (this library has no CPU fallback)");
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return fail(nullptr, FE_MF_ECUDA, "cudaGetDeviceProperties failed");
+  if (prop.major != 10) return fail(nullptr, FE_MF_EUNSUPPORTED, "device is not sm_100 (Blackwell B200)");
+
+  fe_mf_ctx* c = new (std::nothrow) fe_mf_ctx();
+  if (!c) return fail(nullptr, FE_MF_ENOMEM, "out of host memory");
+  c->ncx = ncx; c->ncy = ncy; c->ncz = ncz; c->p = p; c->n = p + 1; c->bc = bc; c->geom = geom;
+  const int add = (bc == FE_BC_DIRICHLET) ? 1 : 0;
+  c->ndx = ncx * p + add; c->ndy = ncy * p + add; c->ndz = ncz * p + add;
+  c->ndof = (long long)c->ndx * c->ndy * c->ndz;
+  c->ncells = (long long)ncx * ncy * ncz;
+  c->sigma = sigma; c->device = cuda_device;
+
+  DeviceGuard guard(cuda_device);
+  if (!guard.ok) { delete c; return fail(nullptr, FE_MF_ECUDA, "cudaSetDevice failed"); }
+
+  const fe::Tables1D tab = fe::make_tables(p);
+  const int n = p + 1, nn = n * n * n;
+  cudaError_t e;
+  e = cudaMemcpyToSymbol(fe::c_N, tab.N, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
+  if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_D, tab.Dt, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
+  if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
+  if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
+
+  double lo[3] = {0, 0, 0}, h[3] = {1, 1, 1};
+  if (!vertices_host) {
+    const int nc[3] = {ncx, ncy, ncz};
+    for (int d = 0; d < 3; ++d) { lo[d] = box_lo[d]; h[d] = (box_hi[d] - box_lo[d]) / nc[d]; }
+  }
+  const double centre[3] = {0.0, 0.0, 0.0};
+  if (!vertices_host && geom == FE_GEOM_AFFINE) {
+    c->geom_mode = 0;
+    double v[8][3], J[3][3];
+    cell_vertices(c, nullptr, lo, h, 0, 0, 0, v);
+    fe::trilinear_jacobian(v, centre, J);
+    if (!fe::metric_from_jacobian(J, c->ug)) { delete c; return fail(nullptr, FE_MF_EINVAL, "non-positive det J"); }
+    c->ug[6] *= sigma;
+  } else {
+    const bool perq = (geom == FE_GEOM_QPOINT);
+    c->geom_mode = perq ? 2 : 1;
+    const size_t per_cell = perq ? (size_t)7 * nn : 7;
+    std::vector<double> G;
+    try { G.resize(per_cell * (size_t)c->ncells); } catch (...) { delete c; return fail(nullptr, FE_MF_ENOMEM, "out of host memory (geometry)"); }
+    bool bad = false;
+    for (int ez = 0; ez < ncz; ++ez)
+      for (int ey = 0; ey < ncy; ++ey)
+        for (int ex = 0; ex < ncx; ++ex) {
+          double v[8][3], J[3][3], m[7];
+          cell_vertices(c, vertices_host, lo, h, ex, ey, ez, v);
+          const size_t cell = (size_t)ex + (size_t)ncx * ((size_t)ey + (size_t)ncy * ez);
+          double* g = G.data() + cell * per_cell;
+          if (!perq) {
+            fe::trilinear_jacobian(v, centre, J);
+            if (!fe::metric_from_jacobian(J, m)) { bad = true; continue; }
+            for (int k = 0; k < 6; ++k) g[k] = m[k];
+            g[6] = sigma * m[6];
+          } else {
+            for (int q3 = 0; q3 < n; ++q3)
+              for (int q2 = 0; q2 < n; ++q2)
+                for (int q1 = 0; q1 < n; ++q1) {
+                  const double xi[3] = {tab.xq[q1], tab.xq[q2], tab.xq[q3]};
+                  fe::trilinear_jacobian(v, xi, J);
+                  if (!fe::metric_from_jacobian(J, m)) { bad = true; continue; }
+                  const double wq = tab.w[q1] * tab.w[q2] * tab.w[q3];
+                  const int Q = q1 + n * (q2 + n * q3);
+                  for (int k = 0; k < 6; ++k) g[(size_t)k * nn + Q] = m[k] * wq;
+                  g[(size_t)6 * nn + Q] = sigma * m[6] * wq;
+                }
+          }
+        }
+    if (bad) { delete c; return fail(nullptr, FE_MF_EINVAL, "non-positive det J at a quadrature point"); }
+    e = cudaMalloc(&c->geom_dev, G.size() * sizeof(double));
+    if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ENOMEM, std::string("geometry cudaMalloc: ") + cudaGetErrorString(e)); }
+    e = cudaMemcpy(c->geom_dev, G.data(), G.size() * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(c->geom_dev); delete c; return fail(nullptr, FE_MF_ECUDA, std::string("geometry upload: ") + cudaGetErrorString(e)); }
+  }
+  *out = c;
+  return FE_MF_OK;
+}
+
+extern "C" long long fe_mf_ndofs(const fe_mf_ctx* ctx) { return ctx ? ctx->ndof : -1; }
+
+extern "C" const char* fe_mf_last_error(const fe_mf_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
+  if (!ctx) return;
+  DeviceGuard guard(ctx->device);
+  if (ctx->geom_dev) cudaFree(ctx->geom_dev);
+  if (ctx->ws_x) cudaFree(ctx->ws_x);
+  if (ctx->ws_y) cudaFree(ctx->ws_y);
+  for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
+  delete ctx;
+}
+
+#include "fe_dispatch.inl"

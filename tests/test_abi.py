@@ -1,0 +1,75 @@
+"""No-GPU checks of the boundary: the C-ABI library builds, loads, and exports every symbol that
+include/fe_mf.h declares; the binding's symbol table matches the header; the product path fails
+loudly without a device (no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_symbols():
+    src = open(os.path.join(ROOT, "include", "fe_mf.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(fe_[a-z0-9_]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def built_lib():
+    from paper_2208_07129_b200 import build
+    return build.build()
+
+
+def test_header_declares_the_north_star_entry_points():
+    syms = header_symbols()
+    for name in ("fe_mf_create", "fe_mf_apply", "fe_cheb_filter", "fe_mf_destroy", "fe_mf_ndofs", "fe_mf_last_error"):
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol(built_lib):
+    lib = ctypes.CDLL(built_lib)
+    for name in header_symbols():
+        assert hasattr(lib, name), name
+
+
+def test_binding_table_matches_header(built_lib):
+    from paper_2208_07129_b200 import binding
+    assert sorted(binding.SYMBOLS) == header_symbols()
+    binding.lib()
+
+
+def test_no_cpu_fallback(built_lib):
+    """Without a CUDA device fe_mf_create must fail with a CUDA error, not compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2208_07129_b200 import binding
+    with pytest.raises(binding.FeMfError) as e:
+        binding.FeMf((2, 2, 2), 2, 1.0, binding.FE_BC_PERIODIC)
+    assert e.value.code == binding.FE_MF_ECUDA
+
+
+def test_argument_validation_without_gpu(built_lib):
+    from paper_2208_07129_b200 import binding
+    l = binding.lib()
+    assert l.fe_mf_ndofs(None) == -1
+    assert l.fe_mf_apply(None, None, None, 1, None) == binding.FE_MF_EINVAL
+    ctx = ctypes.c_void_p()
+    lo = (ctypes.c_double * 3)(0, 0, 0); hi = (ctypes.c_double * 3)(1, 1, 1)
+    assert l.fe_mf_create(ctypes.byref(ctx), 2, 2, 2, 0, 1.0, 0, 0, lo, hi, None, 0) == binding.FE_MF_EINVAL
+    assert b"p must be" in l.fe_mf_last_error(None)
+    assert l.fe_mf_create(None, 2, 2, 2, 2, 1.0, 0, 0, lo, hi, None, 0) == binding.FE_MF_EINVAL
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2208_07129_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".inl")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt, f
+    orc = open(os.path.join(ROOT, "oracle", "fe_oracle.py")).read()
+    assert "paper_2208_07129_b200" not in orc.replace("`paper_2208_07129_b200/csrc`", "")
