@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py -- Helmholtz apply throughput (GDoF*vec/s, FP64) on BASELINE.json's metric config.
+
+    python bench.py --gpus 1 --steps 20 --warmup 5            # CUDA path, config 2 (p=6, 24^3, Dirichlet, 32 vec)
+    python bench.py --impl reference --steps 5 --warmup 1     # the CPU oracle on the same metric/config (bounded sample)
+    torchrun --nproc-per-node N bench.py --gpus N ...         # weak scaling: each rank its own 32-vector batch
+
+A step = one pass of the whole hot path (Y <- 0, gather ... scatter-add) over one batch of synthetic
+input (seeded counter generator, filled on the device).  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "helmholtz_apply_throughput"
+UNIT = "GDoF*vec/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 is the metric config")
+    ap.add_argument("--nvec", type=int, default=0, help="override the vector count (config 4 sweep)")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock / throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.max_mhz, self._stop_evt = [], set(), None, threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def workload_for(args):
+    from paper_2208_07129_b200 import inputs
+    w = inputs.configs()[args.config]
+    nvec = args.nvec if args.nvec > 0 else w.nvec
+    return w, nvec
+
+
+def config_dict(w, nvec, extra=None):
+    d = {"workload": w.name, "p": w.p, "cells": list(w.ncells), "bc": "dirichlet" if w.bc else "periodic",
+         "geometry": "per-q-point" if w.geom else "affine", "sigma": w.sigma, "ndof": w.ndof, "nvec": nvec,
+         "l2_policy": "inputs larger than L2 (X and Y %.0f MB each vs 126 MB L2); no flush needed" %
+                      (w.ndof * nvec * 8 / 1e6)}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def oracle_for(w):
+    from oracle import fe_oracle as orc
+    from paper_2208_07129_b200 import inputs
+    bc = "periodic" if w.bc == inputs.BC_PERIODIC else "dirichlet"
+    mesh = orc.Mesh(w.ncells, w.p, bc, w.box_lo, w.box_hi, vertices=inputs.workload_vertices(w))
+    return orc.Operator(mesh, w.sigma)
+
+
+def host_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i.get("num_threads", 0) for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def run_reference(args):
+    """The oracle, as it stands, on the host cores: each step = one apply on a bounded sample of the
+    workload (same recipe, 8^3 cells instead of the full mesh, same nvec)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np  # noqa: F401
+    from paper_2208_07129_b200 import inputs
+    w, nvec = workload_for(args)
+    ws = w.scaled(min(8, w.ncells[0]), nvec=nvec)
+    op = oracle_for(ws)
+    X = inputs.multivector(ws.seed, ws.ndof, nvec)
+    for _ in range(max(args.warmup, 1)):
+        op.apply(X)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        op.apply(X)
+    dt = time.perf_counter() - t0
+    val = ws.ndof * nvec * args.steps / dt / 1e9
+    sample = f"{ws.ncells[0]}^3-cell sub-mesh of {w.name} (ndof {ws.ndof}), nvec {nvec}, one oracle apply per step"
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, nvec, {"sample": sample}),
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_2208_07129_b200 import binding, build, inputs, roofline
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not os.path.exists(binding.LIB_PATH):
+        build.build()
+    binding.lib()
+
+    w, nvec = workload_for(args)
+    fp64_peak, copy_gbs = binding.probe_peaks(local)
+    op = binding.FeMf.from_workload(w, device=local)
+    if args.variant:
+        op.set_variant(args.variant)
+    count = w.ndof * nvec
+    X = torch.empty(count, dtype=torch.float64, device="cuda")
+    Y = torch.empty_like(X)
+    binding.fill_uniform(X, w.seed, offset=rank * count)     # weak scaling: rank r owns columns [r*nvec, (r+1)*nvec)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        op.apply(X, Y, nvec)
+    launches_per_step = op.last_launch_count()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        op.apply(X, Y, nvec)
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    # the dominant kernel alone (same launch configuration), events on the launching stream
+    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k0.record(stream)
+    for _ in range(args.steps):
+        op.accumulate(1.0, X, Y, nvec)
+    k1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms_kernel = k0.elapsed_time(k1) / args.steps
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * count / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        op.apply(X, Y, nvec)
+        Xh = torch.empty(count, dtype=torch.float64).pin_memory()
+        Yh = torch.empty(count, dtype=torch.float64).pin_memory()
+        Xh.copy_(X)
+        n_e2e = max(1, min(args.steps, 5))
+        op.apply_host(Xh, Yh, nvec)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            op.apply_host(Xh, Yh, nvec)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * count * n_e2e / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": count * 8,
+               "d2h_bytes_per_step": count * 8, "steps": n_e2e, "api": "fe_mf_apply_host (pinned host buffers)"}
+        y_host_check = float((Yh.cuda() - Y).abs().max().item())
+        e2e["max_abs_diff_vs_device_path"] = y_host_check
+
+    # ---- roofline of the dominant kernel
+    diag = (w.geom == inputs.GEOM_AFFINE)
+    bv = op.batch_width(nvec)
+    slots, flops = roofline.work_per_dof_vec(w.p, diag)
+    peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm_peak, hbm_src = roofline.HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+    if os.path.exists(peaks_file):
+        try:
+            hbm_peak, hbm_src = float(json.load(open(peaks_file))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    achieved_tf = count * slots * 2.0 / (ms_kernel * 1e-3) / 1e12
+    t_roof, t_alu, t_hbm = roofline.roofline_time_s(w.p, w.ndof, nvec, diag, w.geom == inputs.GEOM_QPOINT, bv,
+                                                    fp64_peak, hbm_peak)
+    traffic = None
+    tfile = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tfile):
+        try:
+            traffic = json.load(open(tfile)).get(f"cfg{args.config}_nvec{nvec}_variant{args.variant}")
+        except Exception:
+            traffic = None
+    roof = {"bound": "alu", "achieved": achieved_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved_tf / fp64_peak,
+            "traffic": traffic, "kernel": "fe_apply (fused cell kernel)", "kernel_ms": ms_kernel,
+            "peak_source": "fe_probe_peaks: FP64 FMA chain measured live in this run (burst)",
+            "flop_convention": "2 x algorithmic FP64 instructions of the even-odd method (%.1f instr, %.1f flops per DoF*vec)" % (slots, flops),
+            "t_roof_ms": t_roof * 1e3, "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
+            "frac_of_t_roof": t_roof * 1e3 / ms_kernel,
+            "hbm": {"achieved": count * roofline.bytes_per_dof_vec(w.p, w.geom == inputs.GEOM_QPOINT, bv) / (ms_kernel * 1e-3) / 1e9,
+                    "peak": hbm_peak, "unit": "GB/s", "peak_source": hbm_src, "copy_gbs_live": copy_gbs}}
+
+    # ---- the oracle timed on the host cores (rank 0, N = 1 only): full workload, also a full-size parity check
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        Xn = X.cpu().numpy().reshape(w.ndof, nvec)
+        orc_op = oracle_for(w)
+        cols = nvec
+        if w.geom == inputs.GEOM_QPOINT:
+            cols = min(nvec, 4)        # per-cell dense tables: bound the sample to 4 columns
+        Xs = np.ascontiguousarray(Xn[:, :cols])
+        t0 = time.perf_counter()
+        reps = 0
+        while True:
+            Yo = orc_op.apply(Xs)
+            reps += 1
+            if time.perf_counter() - t0 > 10.0 or reps >= 5:
+                break
+        dt = (time.perf_counter() - t0) / reps
+        op.apply(X, Y, nvec)
+        torch.cuda.synchronize()
+        Yg = Y.cpu().numpy().reshape(w.ndof, nvec)[:, :cols]
+        err = float(np.abs(Yg - Yo).max() / np.abs(Yo).max())
+        cpu = {"value": w.ndof * cols / dt / 1e9, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+               "sample": f"full mesh of {w.name}, {cols} of {nvec} columns, {reps} oracle applies (element matrices precomputed, untimed)",
+               "parity_rel_maxnorm_err_vs_gpu": err}
+
+    if rank == 0:
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+               "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+               "data": "synthetic", "config": config_dict(w, nvec, {"bv": bv, "variant": args.variant,
+                                                                     "sharding": "vector columns, no collective"}),
+               "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roof,
+               "cpu_baseline": cpu}
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -89,6 +89,14 @@ int fe_mf_apply_axpby(fe_mf_ctx *ctx, double alpha, const double *W_dev, double 
                       double *Z_dev, int nvec, void *cuda_stream);
 
 /*
+ * fe_mf_accumulate -- Z <- Z + alpha * A * W : the fused cell kernel alone (gather ... scatter-add,
+ * PAPER.md:690-740 Alg. 4) on an already initialised Z.  fe_mf_apply == (Z <- 0) + this call;
+ * bench.py times it to obtain the dominant kernel's own duration.
+ */
+int fe_mf_accumulate(fe_mf_ctx *ctx, double alpha, const double *W_dev, double *Z_dev, int nvec,
+                     void *cuda_stream);
+
+/*
  * fe_cheb_filter -- scaled Chebyshev filter of degree m (Alg. 6 lines 2-17, garbled
  * lines reconstructed as in SURVEY.md §8(c) step 6 / DESIGN.md reading 10):
  *     e=(b-a)/2; c=(b+a)/2; s=e/(a0-c); s1=s; g=2/s1; a1=s1/e; a2=-c;  Y = a1 A X + a1 a2 X;

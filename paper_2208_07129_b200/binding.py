@@ -28,6 +28,7 @@ SYMBOLS = {
     "fe_mf_ndofs": (C.c_longlong, [C.c_void_p]),
     "fe_mf_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "fe_mf_apply_axpby": (C.c_int, [C.c_void_p, _D, C.c_void_p, _D, _D, C.c_void_p, C.c_int, C.c_void_p]),
+    "fe_mf_accumulate": (C.c_int, [C.c_void_p, _D, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "fe_cheb_filter": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, _D, _D, _D, C.c_void_p]),
     "fe_mf_apply_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "fe_fill_uniform": (C.c_int, [C.c_void_p, C.c_longlong, C.c_ulonglong, C.c_longlong, C.c_void_p]),
@@ -121,6 +122,11 @@ class FeMf:
         _check_tensor(W, self.ndofs, nvec, "W"); _check_tensor(Z, self.ndofs, nvec, "Z")
         self._raise(self._l.fe_mf_apply_axpby(self._ctx, float(alpha), W.data_ptr(), float(beta), float(gamma),
                                               Z.data_ptr(), int(nvec), _stream_ptr(stream)))
+
+    def accumulate(self, alpha: float, W, Z, nvec: int, stream=None):
+        _check_tensor(W, self.ndofs, nvec, "W"); _check_tensor(Z, self.ndofs, nvec, "Z")
+        self._raise(self._l.fe_mf_accumulate(self._ctx, float(alpha), W.data_ptr(), Z.data_ptr(), int(nvec),
+                                             _stream_ptr(stream)))
 
     def cheb_filter(self, X, Y, nvec: int, m: int, a: float, b: float, a0: float, stream=None):
         _check_tensor(X, self.ndofs, nvec, "X"); _check_tensor(Y, self.ndofs, nvec, "Y")

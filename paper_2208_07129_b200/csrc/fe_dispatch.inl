@@ -108,6 +108,15 @@ extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_d
   return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st);
 }
 
+extern "C" int fe_mf_accumulate(fe_mf_ctx* ctx, double alpha, const double* W_dev, double* Z_dev, int nvec,
+                                void* cuda_stream) {
+  int rc = check_io(ctx, W_dev, Z_dev, nvec);
+  if (rc) return rc;
+  DeviceGuard guard(ctx->device);
+  ctx->last_launches = 0;
+  return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, (cudaStream_t)cuda_stream);
+}
+
 extern "C" int fe_mf_apply(fe_mf_ctx* ctx, const double* X_dev, double* Y_dev, int nvec, void* cuda_stream) {
   return fe_mf_apply_axpby(ctx, 1.0, X_dev, 0.0, 0.0, Y_dev, nvec, cuda_stream);
 }

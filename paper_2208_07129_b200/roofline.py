@@ -1,0 +1,58 @@
+"""Algorithmic work model of the hot path.  Pure counting, no kernels.
+
+Per cell and per vector, n = n_p = n_q = p+1, the method of BASELINE.json's north_star
+(sum factorisation with even-odd decomposed 1D contractions) executes
+  * 12 contractions, each n^2 lines; one even-odd line costs ceil(n/2)^2 + floor(n/2)^2 FMA and
+    4*floor(n/2) adds;
+  * the quadrature-point scaling: symmetric 3x3 metric + mass factor = 3 MUL + 6 FMA + 1 MUL per point
+    (general geometry), or 3 MUL + 1 MUL per point when the metric is diagonal (Cartesian cells).
+An "FP64 instruction" (issue slot) is one DFMA / DADD / DMUL per lane; the B200 FP64 pipe retires
+peak_tflops/2 of them per second.  Bytes: read X once + write Y once = 16 B per DoF*vector, plus
+56 B per quadrature point per block of `bv` vectors for per-q-point geometry; a Chebyshev step
+reads X, Y and writes X_new = 24 B per DoF*vector.
+"""
+from __future__ import annotations
+
+FP64_PEAK_FALLBACK_TFLOPS = 37.1   # this repo's fe_probe_peaks on a B200 at 1965 MHz (profiles/r1_box_peaks.md)
+HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback
+
+
+def fp64_instr_per_cell_vec(p: int, diagonal_metric: bool, even_odd: bool = True):
+    """(fma, add_or_mul) FP64 instructions per cell per vector."""
+    n = p + 1
+    if even_odd:
+        hi, lo = (n + 1) // 2, n // 2
+        fma_line, add_line = hi * hi + lo * lo, 4 * lo
+    else:
+        fma_line, add_line = n * n, 0
+    fma = 12 * n * n * fma_line
+    other = 12 * n * n * add_line
+    if diagonal_metric:
+        other += 4 * n ** 3
+    else:
+        fma += 6 * n ** 3
+        other += 4 * n ** 3
+    return fma, other
+
+
+def work_per_dof_vec(p: int, diagonal_metric: bool, even_odd: bool = True):
+    """FP64 instructions (issue slots) and flops (FMA = 2) per DoF*vector (cell work / p^3)."""
+    fma, other = fp64_instr_per_cell_vec(p, diagonal_metric, even_odd)
+    return (fma + other) / p ** 3, (2 * fma + other) / p ** 3
+
+
+def bytes_per_dof_vec(p: int, per_qpoint_geometry: bool, bv: int, chebyshev: bool = False) -> float:
+    n = p + 1
+    b = 24.0 if chebyshev else 16.0
+    if per_qpoint_geometry:
+        b += 56.0 * n ** 3 / (p ** 3 * bv)
+    return b
+
+
+def roofline_time_s(p, ndof, nvec, diagonal_metric, per_qpoint_geometry, bv, fp64_tflops, hbm_gbs, chebyshev=False):
+    """t_roof = max(bytes / BW, FP64 instructions / (peak/2))  (north_star's definition)."""
+    slots, _ = work_per_dof_vec(p, diagonal_metric)
+    units = float(ndof) * nvec
+    t_alu = units * slots / (fp64_tflops * 1e12 / 2.0)
+    t_hbm = units * bytes_per_dof_vec(p, per_qpoint_geometry, bv, chebyshev) / (hbm_gbs * 1e9)
+    return max(t_alu, t_hbm), t_alu, t_hbm
