@@ -27,6 +27,58 @@ cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStr
   return cudaGetLastError();
 }
 
+// ---- optimised Cartesian kernel (variant 0 on uniform meshes): launch geometry per degree
+template <int PDEG, int BV>
+struct CartCfg {
+  static constexpr int N = PDEG + 1;
+  static constexpr int TASKS = N * N * BV;
+  static constexpr int NT = (PDEG >= 5) ? TASKS / 2 : (TASKS < 32 ? 32 : TASKS);
+  static constexpr size_t SMEM = (size_t)2 * fe::Tile<PDEG, BV>::SIZE * sizeof(double);
+  static constexpr int BY_SMEM = (int)((kMaxSmem - 1024) / (SMEM + 1024));
+  static constexpr int BY_THREADS = 2048 / NT;
+  static constexpr int MINB0 = BY_SMEM < BY_THREADS ? BY_SMEM : BY_THREADS;
+  static constexpr int MINB = MINB0 > 4 ? 4 : (MINB0 < 1 ? 1 : MINB0);
+};
+
+template <int PDEG, int BV>
+cudaError_t launch_cart(const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
+  using C = CartCfg<PDEG, BV>;
+  static bool configured = false;
+  auto kern = fe::fe_apply_cart<PDEG, BV, C::NT, C::MINB>;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  kern<<<(unsigned)(ncells * prm.nvb), C::NT, C::SMEM, st>>>(prm);
+  return cudaGetLastError();
+}
+
+template <int BV>
+cudaError_t launch_cart_p(int p, const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
+  switch (p) {
+    case 1: return launch_cart<1, BV>(prm, ncells, st);
+    case 2: return launch_cart<2, BV>(prm, ncells, st);
+    case 3: return launch_cart<3, BV>(prm, ncells, st);
+    case 4: return launch_cart<4, BV>(prm, ncells, st);
+    case 5: return launch_cart<5, BV>(prm, ncells, st);
+    case 6: return launch_cart<6, BV>(prm, ncells, st);
+    case 7: return launch_cart<7, BV>(prm, ncells, st);
+    case 8: return launch_cart<8, BV>(prm, ncells, st);
+  }
+  return cudaErrorInvalidValue;
+}
+
+// Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
+// 3 = Cartesian even-odd BV=16.
+int pick_kernel(const fe_mf_ctx* c, int nvec) {
+  if (c->variant == 1) return 1;
+  const bool diag = (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
+  if (!diag || nvec < 4) return 1;
+  if (c->variant == 3 && c->p <= 6) return 3;
+  return 2;
+}
+
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
   fe::ApplyParams P;
   P.W = W; P.Z = Z; P.geom = c->geom_dev;
@@ -42,11 +94,14 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
 
 // Z += alpha * A * W  (Z already initialised).  Counts launches into c->last_launches.
 int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st) {
-  const int bv = general_bv(c->p, nvec);
+  const int kind = pick_kernel(c, nvec);
+  const int bv = kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : 16);
   const fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
-  switch (c->p) {
+  if (kind == 2) e = launch_cart_p<8>(c->p, P, c->ncells, st);
+  else if (kind == 3) e = launch_cart_p<16>(c->p, P, c->ncells, st);
+  else switch (c->p) {
     case 1: e = launch_general<1>(P, c->ncells, st); break;
     case 2: e = launch_general<2>(P, c->ncells, st); break;
     case 3: e = launch_general<3>(P, c->ncells, st); break;
@@ -222,14 +277,15 @@ extern "C" int fe_fill_uniform(double* out_dev, long long count, unsigned long l
 
 extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
   if (!ctx || nvec < 1) return -1;
-  return general_bv(ctx->p, nvec);
+  const int kind = pick_kernel(ctx, nvec);
+  return kind == 1 ? general_bv(ctx->p, nvec) : (kind == 2 ? 8 : 16);
 }
 
 extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx->last_launches : -1; }
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if (variant != 0) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if (variant < 0 || variant > 3) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "fe_kernels.cuh"
+#include "fe_kernels_eo.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {
@@ -48,6 +49,35 @@ struct DeviceGuard {
   explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess) ok = true; }
   ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
+
+// Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
+// 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4]) {
+  const int n = t.n, h = n / 2, m = n / 2;
+  long double M[4][fe::MAXN * fe::MAXN];
+  for (int q = 0; q < n; ++q)
+    for (int i = 0; i < n; ++i) {
+      const long double sq = sqrtl(t.wl[q]), si = sqrtl(t.wl[i]);
+      const long double ns = sq * t.Nl[q * n + i];
+      const long double ds = sq * t.Dl[q * n + i] / si;
+      M[0][q * n + i] = ns; M[1][i * n + q] = ns;
+      M[2][q * n + i] = ds; M[3][i * n + q] = ds;
+    }
+  for (int k = 0; k < 4; ++k) {
+    std::memset(&out[k], 0, sizeof(fe::EoTab));
+    for (int q = 0; q < h; ++q) {
+      for (int i = 0; i < h; ++i) {
+        out[k].P[q * h + i] = (double)(0.5L * (M[k][q * n + i] + M[k][q * n + (n - 1 - i)]));
+        out[k].Mn[q * h + i] = (double)(0.5L * (M[k][q * n + i] - M[k][q * n + (n - 1 - i)]));
+      }
+      if (n & 1) out[k].Pm[q] = (double)M[k][q * n + m];
+    }
+    if (n & 1) {
+      for (int i = 0; i < h; ++i) out[k].mid[i] = (double)M[k][m * n + i];
+      out[k].midm = (double)M[k][m * n + m];
+    }
+  }
+}
 
 void cell_vertices(const fe_mf_ctx* c, const double* verts, const double lo[3], const double h[3], int ex, int ey,
                    int ez, double v[8][3]) {
@@ -107,6 +137,11 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   e = cudaMemcpyToSymbol(fe::c_N, tab.N, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_D, tab.Dt, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
+  if (e == cudaSuccess) {
+    fe::EoTab eo[4];
+    make_eo_tables(tab, eo);
+    e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 4 * p);
+  }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
 
   double lo[3] = {0, 0, 0}, h[3] = {1, 1, 1};

@@ -16,6 +16,7 @@ struct Tables1D {
   double w[MAXN];            // Gauss-Legendre weights
   double N[MAXN * MAXN];     // N[q*n+i]  = l_i(xq_q)
   double Dt[MAXN * MAXN];    // Dt[q*n+r] = l~_r'(xq_q)
+  long double Nl[MAXN * MAXN], Dl[MAXN * MAXN], wl[MAXN];  // the same before rounding to double
 };
 
 inline void legendre(int n, long double x, long double& pn, long double& pnm1) {
@@ -80,13 +81,13 @@ inline Tables1D make_tables(int p) {
   long double xi[MAXN], xq[MAXN], w[MAXN];
   gll_nodes(p, xi);
   gauss_legendre(n, xq, w);
-  for (int i = 0; i < n; ++i) { t.xi[i] = (double)xi[i]; t.xq[i] = (double)xq[i]; t.w[i] = (double)w[i]; }
+  for (int i = 0; i < n; ++i) { t.xi[i] = (double)xi[i]; t.xq[i] = (double)xq[i]; t.w[i] = (double)w[i]; t.wl[i] = w[i]; }
   // N[q][i] = prod_{j != i} (xq_q - xi_j)/(xi_i - xi_j)
   for (int q = 0; q < n; ++q)
     for (int i = 0; i < n; ++i) {
       long double v = 1.0L;
       for (int j = 0; j < n; ++j) if (j != i) v *= (xq[q] - xi[j]) / (xi[i] - xi[j]);
-      t.N[q * n + i] = (double)v;
+      t.Nl[q * n + i] = v;
     }
   // Dt[q][r] = l~_r'(xq_q) on the quadrature points: barycentric form
   long double c[MAXN];
@@ -96,21 +97,22 @@ inline Tables1D make_tables(int p) {
       long double v = 0.0L;
       if (q != r) v = (c[q] / c[r]) / (xq[q] - xq[r]);
       else for (int j = 0; j < n; ++j) if (j != q) v += 1.0L / (xq[q] - xq[j]);
-      t.Dt[q * n + r] = (double)v;
+      t.Dl[q * n + r] = v;
     }
-  // enforce the exact centro-(anti)symmetry the even-odd kernels assume (SURVEY.md reading 14)
+  // enforce the exact centro-(anti)symmetry the even-odd kernels assume (reading 14)
   for (int q = 0; q < n; ++q)
     for (int i = 0; i < n; ++i) {
       int q2 = n - 1 - q, i2 = n - 1 - i;
       if (q * n + i < q2 * n + i2) {
-        double a = 0.5 * (t.N[q * n + i] + t.N[q2 * n + i2]);
-        t.N[q * n + i] = t.N[q2 * n + i2] = a;
-        double d = 0.5 * (t.Dt[q * n + i] - t.Dt[q2 * n + i2]);
-        t.Dt[q * n + i] = d; t.Dt[q2 * n + i2] = -d;
+        long double a = 0.5L * (t.Nl[q * n + i] + t.Nl[q2 * n + i2]);
+        t.Nl[q * n + i] = t.Nl[q2 * n + i2] = a;
+        long double d = 0.5L * (t.Dl[q * n + i] - t.Dl[q2 * n + i2]);
+        t.Dl[q * n + i] = d; t.Dl[q2 * n + i2] = -d;
       } else if (q * n + i == q2 * n + i2) {
-        t.Dt[q * n + i] = 0.0;  // centre of an odd-n table
+        t.Dl[q * n + i] = 0.0L;  // centre of an odd-n table
       }
     }
+  for (int k = 0; k < n * n; ++k) { t.N[k] = (double)t.Nl[k]; t.Dt[k] = (double)t.Dl[k]; }
   return t;
 }
 

@@ -216,3 +216,18 @@ def test_unit_cube_config5_interval_is_rejected(env):
     X = torch.zeros(op.ndofs, dtype=torch.float64, device="cuda"); Y = torch.zeros_like(X)
     with pytest.raises(binding.FeMfError):
         op.cheb_filter(X, Y, 1, 20, 2.0, 0.3, 0.0)
+
+
+@pytest.mark.parametrize("variant", [1, 3])
+@pytest.mark.parametrize("p,bc", [(6, inputs.BC_DIRICHLET), (7, inputs.BC_PERIODIC), (8, inputs.BC_PERIODIC), (4, inputs.BC_PERIODIC)])
+def test_kernel_variants(env, variant, p, bc):
+    """variant 1 = general kernel, 3 = even-odd Cartesian kernel with 16 vectors per block (default is 8)."""
+    torch, orc, binding = env
+    w = inputs.Workload(f"var_p{p}", p, (3, 2, 3), bc, inputs.GEOM_AFFINE, 0.8, (0.0, 0.0, 0.0), (1.5, 1.0, 2.0), 20, 500 + p)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    Yo = orc.Operator(oracle_mesh(orc, w), w.sigma).apply(X)
+    op = binding.FeMf.from_workload(w)
+    op.set_variant(variant)
+    Xd = torch.from_numpy(X).cuda(); Yd = torch.empty_like(Xd)
+    op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
+    assert relerr(Yd.cpu().numpy(), Yo) <= TOL
