@@ -69,14 +69,47 @@ cudaError_t launch_cart_p(int p, const fe::ApplyParams& prm, long long ncells, c
   return cudaErrorInvalidValue;
 }
 
+// ---- production Cartesian kernel (two vectors per thread)
+template <int PDEG> struct Cart2Cfg;
+template <> struct Cart2Cfg<1> { static constexpr int BV = 16, NT = 32, MINB = 4; };
+template <> struct Cart2Cfg<2> { static constexpr int BV = 16, NT = 96, MINB = 4; };
+template <> struct Cart2Cfg<3> { static constexpr int BV = 16, NT = 128, MINB = 4; };
+template <> struct Cart2Cfg<4> { static constexpr int BV = 16, NT = 112, MINB = 4; };
+template <> struct Cart2Cfg<5> { static constexpr int BV = 16, NT = 160, MINB = 3; };
+template <> struct Cart2Cfg<6> { static constexpr int BV = 16, NT = 224, MINB = 2; };
+template <> struct Cart2Cfg<7> { static constexpr int BV = 8, NT = 128, MINB = 3; };
+template <> struct Cart2Cfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
+
+template <int PDEG>
+cudaError_t launch_cart2(const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
+  using C = Cart2Cfg<PDEG>;
+  constexpr size_t SMEM = (size_t)2 * fe::Tile<PDEG, C::BV>::SIZE * sizeof(double);
+  static bool configured = false;
+  auto kern = fe::fe_apply_cart2<PDEG, C::BV, C::NT, C::MINB>;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  kern<<<(unsigned)(ncells * prm.nvb), C::NT, SMEM, st>>>(prm);
+  return cudaGetLastError();
+}
+
+int cart2_bv(int p) { return p >= 7 ? 8 : 16; }
+
 // Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
-// 3 = Cartesian even-odd BV=16.
-int pick_kernel(const fe_mf_ctx* c, int nvec) {
+// 4 = Cartesian even-odd, two vectors per thread (production; needs even nvec and 16-byte aligned pointers).
+int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 1) return 1;
   const bool diag = (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
   if (!diag || nvec < 4) return 1;
-  if (c->variant == 3 && c->p <= 6) return 3;
-  return 2;
+  if (c->variant == 2) return 2;
+  const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
+  if ((nvec & 1) || !aligned) return 2;
+  return 4;
+}
+int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
+  return kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : cart2_bv(c->p));
 }
 
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
@@ -94,14 +127,25 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
 
 // Z += alpha * A * W  (Z already initialised).  Counts launches into c->last_launches.
 int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st) {
-  const int kind = pick_kernel(c, nvec);
-  const int bv = kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : 16);
-  const fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
+  const int kind = pick_kernel(c, nvec, W, Z);
+  const int bv = kernel_bv(c, kind, nvec);
+  fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
   if (kind == 2) e = launch_cart_p<8>(c->p, P, c->ncells, st);
-  else if (kind == 3) e = launch_cart_p<16>(c->p, P, c->ncells, st);
-  else switch (c->p) {
+  else if (kind == 4) {
+    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // the result is linear in the metric constants
+    switch (c->p) {
+      case 1: e = launch_cart2<1>(P, c->ncells, st); break;
+      case 2: e = launch_cart2<2>(P, c->ncells, st); break;
+      case 3: e = launch_cart2<3>(P, c->ncells, st); break;
+      case 4: e = launch_cart2<4>(P, c->ncells, st); break;
+      case 5: e = launch_cart2<5>(P, c->ncells, st); break;
+      case 6: e = launch_cart2<6>(P, c->ncells, st); break;
+      case 7: e = launch_cart2<7>(P, c->ncells, st); break;
+      case 8: e = launch_cart2<8>(P, c->ncells, st); break;
+    }
+  } else switch (c->p) {
     case 1: e = launch_general<1>(P, c->ncells, st); break;
     case 2: e = launch_general<2>(P, c->ncells, st); break;
     case 3: e = launch_general<3>(P, c->ncells, st); break;
@@ -277,8 +321,8 @@ extern "C" int fe_fill_uniform(double* out_dev, long long count, unsigned long l
 
 extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
   if (!ctx || nvec < 1) return -1;
-  const int kind = pick_kernel(ctx, nvec);
-  return kind == 1 ? general_bv(ctx->p, nvec) : (kind == 2 ? 8 : 16);
+  const int kind = pick_kernel(ctx, nvec, nullptr, nullptr);
+  return kernel_bv(ctx, kind, nvec);
 }
 
 extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx->last_launches : -1; }

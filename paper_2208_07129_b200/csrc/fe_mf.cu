@@ -1,6 +1,7 @@
 // C-ABI of include/fe_mf.h: context, host-side setup, kernel dispatch.  sm_100a only.
 #include "../../include/fe_mf.h"
 
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -9,6 +10,7 @@
 
 #include "fe_kernels.cuh"
 #include "fe_kernels_eo.cuh"
+#include "fe_kernels_cart2.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {
