@@ -97,6 +97,76 @@ cudaError_t launch_cart2(const fe::ApplyParams& prm, long long ncells, cudaStrea
 
 int cart2_bv(int p) { return p >= 7 ? 8 : 16; }
 
+// ---- persistent TMA kernel
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+    (void)cudaGetLastError();
+  }
+  return fn;
+}
+
+// 4-D FP64 tensor map of a multivector [z][y][x][beta] with box (bv, n, n, n).
+bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)c->ndx, (cuuint64_t)c->ndy, (cuuint64_t)c->ndz};
+  const cuuint64_t strides[3] = {(cuuint64_t)nvec * 8, (cuuint64_t)nvec * 8 * c->ndx, (cuuint64_t)nvec * 8 * c->ndx * c->ndy};
+  if (strides[2] >= ((cuuint64_t)1 << 40)) return false;
+  const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)c->n, (cuuint32_t)c->n, (cuuint32_t)c->n};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int PDEG> struct TmaCfg;
+template <> struct TmaCfg<1> { static constexpr int BV = 16, NT = 32, MINB = 4; };
+template <> struct TmaCfg<2> { static constexpr int BV = 16, NT = 96, MINB = 4; };
+template <> struct TmaCfg<3> { static constexpr int BV = 16, NT = 128, MINB = 4; };
+template <> struct TmaCfg<4> { static constexpr int BV = 16, NT = 112, MINB = 4; };
+template <> struct TmaCfg<5> { static constexpr int BV = 16, NT = 160, MINB = 3; };
+template <> struct TmaCfg<6> { static constexpr int BV = 16, NT = 224, MINB = 2; };
+template <> struct TmaCfg<7> { static constexpr int BV = 16, NT = 256, MINB = 1; };
+template <> struct TmaCfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
+int tma_bv(int p) { return p == 8 ? 8 : 16; }
+
+template <int PDEG>
+cudaError_t launch_tma(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                       cudaStream_t st) {
+  using C = TmaCfg<PDEG>;
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  static int blocks_per_sm = 0;
+  static int nsm = 0;
+  auto kern = fe::fe_apply_cart_tma<PDEG, C::BV, C::NT, C::MINB>;
+  if (blocks_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
+    if (e != cudaSuccess) return e;
+    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, c->device);
+    if (e != cudaSuccess) return e;
+    nsm = prop.multiProcessorCount;
+  }
+  const long long nitems = c->ncells * prm.nvb;
+  long long grid = (long long)blocks_per_sm * nsm;
+  if (grid > nitems) grid = nitems;
+  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
+  return cudaGetLastError();
+}
+
 // Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
 // 4 = Cartesian even-odd, two vectors per thread (production; needs even nvec and 16-byte aligned pointers).
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
@@ -106,10 +176,13 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 2) return 2;
   const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
   if ((nvec & 1) || !aligned) return 2;
-  return 4;
+  if (c->variant == 4) return 4;
+  if (!encode_tiled_fn()) return 4;
+  if ((unsigned long long)nvec * 8ULL * c->ndx * c->ndy >= (1ULL << 40)) return 4;
+  return 5;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
-  return kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : cart2_bv(c->p));
+  return kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : tma_bv(c->p)));
 }
 
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
@@ -133,7 +206,22 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
   if (kind == 2) e = launch_cart_p<8>(c->p, P, c->ncells, st);
-  else if (kind == 4) {
+  else if (kind == 5) {
+    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
+    CUtensorMap tw, tz;
+    if (!make_tensor_map(&tw, c, W, nvec, bv) || !make_tensor_map(&tz, c, Z, nvec, bv))
+      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
+    switch (c->p) {
+      case 1: e = launch_tma<1>(c, P, tw, tz, st); break;
+      case 2: e = launch_tma<2>(c, P, tw, tz, st); break;
+      case 3: e = launch_tma<3>(c, P, tw, tz, st); break;
+      case 4: e = launch_tma<4>(c, P, tw, tz, st); break;
+      case 5: e = launch_tma<5>(c, P, tw, tz, st); break;
+      case 6: e = launch_tma<6>(c, P, tw, tz, st); break;
+      case 7: e = launch_tma<7>(c, P, tw, tz, st); break;
+      case 8: e = launch_tma<8>(c, P, tw, tz, st); break;
+    }
+  } else if (kind == 4) {
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // the result is linear in the metric constants
     switch (c->p) {
       case 1: e = launch_cart2<1>(P, c->ncells, st); break;
@@ -329,7 +417,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if (variant < 0 || variant > 3) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if (variant < 0 || variant > 4) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

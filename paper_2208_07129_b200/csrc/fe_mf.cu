@@ -11,6 +11,7 @@
 #include "fe_kernels.cuh"
 #include "fe_kernels_eo.cuh"
 #include "fe_kernels_cart2.cuh"
+#include "fe_kernels_tma.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {

@@ -218,10 +218,10 @@ def test_unit_cube_config5_interval_is_rejected(env):
         op.cheb_filter(X, Y, 1, 20, 2.0, 0.3, 0.0)
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 4])
 @pytest.mark.parametrize("p,bc", [(6, inputs.BC_DIRICHLET), (7, inputs.BC_PERIODIC), (8, inputs.BC_PERIODIC), (4, inputs.BC_PERIODIC)])
 def test_kernel_variants(env, variant, p, bc):
-    """variant 1 = general kernel, 2 = even-odd Cartesian kernel with one vector per thread (default: two)."""
+    """variant 1 = general kernel, 2 = even-odd Cartesian kernel with one vector per thread, 4 = two vectors per thread with LDG/RED (default 0: persistent TMA kernel)."""
     torch, orc, binding = env
     w = inputs.Workload(f"var_p{p}", p, (3, 2, 3), bc, inputs.GEOM_AFFINE, 0.8, (0.0, 0.0, 0.0), (1.5, 1.0, 2.0), 20, 500 + p)
     X = inputs.multivector(w.seed, w.ndof, w.nvec)
