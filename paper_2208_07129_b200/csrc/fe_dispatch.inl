@@ -136,15 +136,20 @@ template <> struct TmaCfg<2> { static constexpr int BV = 16, NT = 96, MINB = 4; 
 template <> struct TmaCfg<3> { static constexpr int BV = 16, NT = 128, MINB = 4; };
 template <> struct TmaCfg<4> { static constexpr int BV = 16, NT = 112, MINB = 4; };
 template <> struct TmaCfg<5> { static constexpr int BV = 16, NT = 160, MINB = 3; };
-template <> struct TmaCfg<6> { static constexpr int BV = 16, NT = 224, MINB = 2; };
+template <> struct TmaCfg<6> { static constexpr int BV = 16, NT = 256, MINB = 2; };
 template <> struct TmaCfg<7> { static constexpr int BV = 16, NT = 256, MINB = 1; };
 template <> struct TmaCfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
 int tma_bv(int p) { return p == 8 ? 8 : 16; }
 
-template <int PDEG>
+template <> struct TmaCfg<106> { static constexpr int BV = 8, NT = 128, MINB = 4; };   // alt p=6
+template <> struct TmaCfg<107> { static constexpr int BV = 8, NT = 128, MINB = 3; };   // alt p=7
+template <> struct TmaCfg<108> { static constexpr int BV = 8, NT = 352, MINB = 1; };   // alt p=8
+int tma_bv_alt(int p) { return 8; }
+
+template <int PDEG, int CFG = PDEG>
 cudaError_t launch_tma(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                        cudaStream_t st) {
-  using C = TmaCfg<PDEG>;
+  using C = TmaCfg<CFG>;
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
   static int blocks_per_sm = 0;
   static int nsm = 0;
@@ -182,7 +187,7 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   return 5;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
-  return kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : tma_bv(c->p)));
+  return kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : ((c->variant == 5 && c->p >= 6) ? 8 : tma_bv(c->p))));
 }
 
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
@@ -195,6 +200,7 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.nvec = nvec; P.bv = bv; P.nvb = (nvec + bv - 1) / bv;
   P.dirichlet = (c->bc == FE_BC_DIRICHLET) ? 1 : 0;
   P.geom_mode = c->geom_mode;
+  P.nsm = c->nsm;
   return P;
 }
 
@@ -217,9 +223,9 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
       case 3: e = launch_tma<3>(c, P, tw, tz, st); break;
       case 4: e = launch_tma<4>(c, P, tw, tz, st); break;
       case 5: e = launch_tma<5>(c, P, tw, tz, st); break;
-      case 6: e = launch_tma<6>(c, P, tw, tz, st); break;
-      case 7: e = launch_tma<7>(c, P, tw, tz, st); break;
-      case 8: e = launch_tma<8>(c, P, tw, tz, st); break;
+      case 6: e = (c->variant == 5) ? launch_tma<6, 106>(c, P, tw, tz, st) : launch_tma<6>(c, P, tw, tz, st); break;
+      case 7: e = (c->variant == 5) ? launch_tma<7, 107>(c, P, tw, tz, st) : launch_tma<7>(c, P, tw, tz, st); break;
+      case 8: e = (c->variant == 5) ? launch_tma<8, 108>(c, P, tw, tz, st) : launch_tma<8>(c, P, tw, tz, st); break;
     }
   } else if (kind == 4) {
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // the result is linear in the metric constants
@@ -417,7 +423,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if (variant < 0 || variant > 4) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if (variant < 0 || variant > 5) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -28,6 +28,7 @@ struct ApplyParams {
   int nvb;                        // ceil(nvec / bv)
   int dirichlet;                  // 1: boundary nodes read as 0 / not written
   int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
+  int nsm;                        // SM count (persistent kernels)
 };
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.

@@ -68,12 +68,22 @@ struct DenseTile {
   }
 };
 
+// Task loop of one phase: ROUNDS rounds of NT tasks; in the last (partial) round the tasks are rotated over
+// the warps by `rot` so that the SM sub-partition (warp % 4) that gets the extra warp-task differs between
+// the blocks resident on one SM and between successive items (FP64 issue is per sub-partition).
+#define FE_FOR_TASKS(t)                                                                          \
+  _Pragma("unroll 1") for (int r_ = 0, t = 0; r_ < ROUNDS; ++r_)                                  \
+    if ((t = (r_ < ROUNDS - 1 || !ROTATE) ? tid + r_ * NT : r_ * NT + rot_tid), t < TASKS)
+
 template <int PDEG, int BV, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                   const ApplyParams P, int nitems) {
   using TL = DenseTile<PDEG, BV>;
   constexpr int N = PDEG + 1, NL = N * N, TPL = BV / 2, TASKS = NL * TPL;
+  constexpr int ROUNDS = (TASKS + NT - 1) / NT;
+  constexpr bool ROTATE = (NT % 32 == 0) && (NT >= 128);
+  constexpr int NW = NT / 32;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* A = reinterpret_cast<double*>(smem_raw);
   double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);
@@ -97,7 +107,9 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG, ey * PDEG, ez * PDEG);
   }
   uint32_t parity = 0;
-  for (; item < nitems; item += gridDim.x) {
+  int rot = (blockIdx.x / P.nsm) & 3;
+  for (; item < nitems; item += gridDim.x, rot = (rot + 1) & 3) {
+    const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
@@ -109,7 +121,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     parity ^= 1u;
 
     // phase 0: Ns along x, in place in A; boundary masking / wrap patching
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N], y[N];
@@ -150,7 +162,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     }
     __syncthreads();
     // phase 1: Ns along y, in place
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<1>(l, base, stride);
       v2 x[N], y[N];
@@ -161,7 +173,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     if (tid == 0) tma_wait_read0();     // the previous item's reduction has finished reading tile B
     __syncthreads();
     // phase 2: Ns along z -> T (A); R = gm*T + Ds^T gzz Ds T along z -> B
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
       v2 x[N], tq[N], r[N];
@@ -175,7 +187,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     }
     __syncthreads();
     // phase 3: R += Ds^T gxx Ds T along x
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<0>(l, base, stride);
       v2 tq[N], r[N];
@@ -186,7 +198,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     }
     __syncthreads();
     // phase 4: R += Ds^T gyy Ds T along y, then Ns^T along y, in place in B
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<1>(l, base, stride);
       v2 tq[N], r[N], u[N];
@@ -208,7 +220,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
       }
     }
     // phase 5: Ns^T along x, in place
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N], y[N];
@@ -218,7 +230,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     }
     __syncthreads();
     // phase 6: Ns^T along z, in place; Dirichlet rows zeroed; wrap-around elements scattered by RED
-    for (int t = tid; t < TASKS; t += NT) {
+    FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
       v2 x[N], y[N];

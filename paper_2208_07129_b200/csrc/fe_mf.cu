@@ -20,6 +20,7 @@ struct fe_mf_ctx {
   long long ndof, ncells;
   double sigma;
   int device;
+  int nsm = 148;
   int geom_mode;            // 0 uniform, 1 per-cell, 2 per-q-point
   double ug[7];
   double* geom_dev = nullptr;
@@ -129,7 +130,7 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   c->ndx = ncx * p + add; c->ndy = ncy * p + add; c->ndz = ncz * p + add;
   c->ndof = (long long)c->ndx * c->ndy * c->ndz;
   c->ncells = (long long)ncx * ncy * ncz;
-  c->sigma = sigma; c->device = cuda_device;
+  c->sigma = sigma; c->device = cuda_device; c->nsm = prop.multiProcessorCount;
 
   DeviceGuard guard(cuda_device);
   if (!guard.ok) { delete c; return fail(nullptr, FE_MF_ECUDA, "cudaSetDevice failed"); }
