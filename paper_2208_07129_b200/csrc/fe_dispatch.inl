@@ -141,19 +141,19 @@ template <> struct TmaCfg<7> { static constexpr int BV = 16, NT = 256, MINB = 1;
 template <> struct TmaCfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
 int tma_bv(int p) { return p == 8 ? 8 : 16; }
 
-template <> struct TmaCfg<106> { static constexpr int BV = 8, NT = 128, MINB = 4; };   // alt p=6
+template <> struct TmaCfg<106> { static constexpr int BV = 8, NT = 128, MINB = 5; };   // alt p=6
 template <> struct TmaCfg<107> { static constexpr int BV = 8, NT = 128, MINB = 3; };   // alt p=7
 template <> struct TmaCfg<108> { static constexpr int BV = 8, NT = 352, MINB = 1; };   // alt p=8
 int tma_bv_alt(int p) { return 8; }
 
-template <int PDEG, int CFG = PDEG>
+template <int PDEG, int CFG = PDEG, bool TMA_OUT = true, int DBG = 0>
 cudaError_t launch_tma(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                        cudaStream_t st) {
   using C = TmaCfg<CFG>;
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
   static int blocks_per_sm = 0;
   static int nsm = 0;
-  auto kern = fe::fe_apply_cart_tma<PDEG, C::BV, C::NT, C::MINB>;
+  auto kern = fe::fe_apply_cart_tma<PDEG, C::BV, C::NT, C::MINB, TMA_OUT, DBG>;
   if (blocks_per_sm == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
     if (e != cudaSuccess) return e;
@@ -223,7 +223,7 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
       case 3: e = launch_tma<3>(c, P, tw, tz, st); break;
       case 4: e = launch_tma<4>(c, P, tw, tz, st); break;
       case 5: e = launch_tma<5>(c, P, tw, tz, st); break;
-      case 6: e = (c->variant == 5) ? launch_tma<6, 106>(c, P, tw, tz, st) : launch_tma<6>(c, P, tw, tz, st); break;
+      case 6: e = (c->variant == 5) ? launch_tma<6, 106>(c, P, tw, tz, st) : (c->variant == 6 ? launch_tma<6, 6, false>(c, P, tw, tz, st) : (c->variant == 101 ? launch_tma<6, 6, true, 1>(c, P, tw, tz, st) : (c->variant == 102 ? launch_tma<6, 6, true, 2>(c, P, tw, tz, st) : launch_tma<6>(c, P, tw, tz, st)))); break;
       case 7: e = (c->variant == 5) ? launch_tma<7, 107>(c, P, tw, tz, st) : launch_tma<7>(c, P, tw, tz, st); break;
       case 8: e = (c->variant == 5) ? launch_tma<8, 108>(c, P, tw, tz, st) : launch_tma<8>(c, P, tw, tz, st); break;
     }
@@ -423,7 +423,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if (variant < 0 || variant > 5) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 6) && variant != 101 && variant != 102) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -68,6 +68,26 @@ struct DenseTile {
   }
 };
 
+// timing experiments (never used by the product path): DBG 1 = no FP64 work, DBG 2 = no block barriers
+#define FE_SYNC() do { if (DBG != 2) __syncthreads(); } while (0)
+template <int PDEG, int MAT, bool TRANS, int DBG, typename T>
+__device__ __forceinline__ void eo2d(const T (&x)[PDEG + 1], T (&y)[PDEG + 1]) {
+  if (DBG == 1) {
+#pragma unroll
+    for (int i = 0; i <= PDEG; ++i) y[i] = x[i];
+  } else {
+    eo2<PDEG, MAT, TRANS>(x, y);
+  }
+}
+template <int PDEG, int DBG, typename T>
+__device__ __forceinline__ void kterm2d(const T (&t)[PDEG + 1], T (&r)[PDEG + 1], double g) {
+  if (DBG == 1) {
+#pragma unroll
+    for (int i = 0; i <= PDEG; ++i) r[i] = r[i] + vmul(g, t[i]);
+  } else {
+    kterm2<PDEG>(t, r, g);
+  }
+}
 // Task loop of one phase: ROUNDS rounds of NT tasks; in the last (partial) round the tasks are rotated over
 // the warps by `rot` so that the SM sub-partition (warp % 4) that gets the extra warp-task differs between
 // the blocks resident on one SM and between successive items (FP64 issue is per sub-partition).
@@ -75,7 +95,7 @@ struct DenseTile {
   _Pragma("unroll 1") for (int r_ = 0, t = 0; r_ < ROUNDS; ++r_)                                  \
     if ((t = (r_ < ROUNDS - 1 || !ROTATE) ? tid + r_ * NT : r_ * NT + rot_tid), t < TASKS)
 
-template <int PDEG, int BV, int NT, int MINB>
+template <int PDEG, int BV, int NT, int MINB, bool TMA_OUT, int DBG = 0>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                   const ApplyParams P, int nitems) {
@@ -97,7 +117,7 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
     mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
+  FE_SYNC();
 
   int item = blockIdx.x;
   if (tid == 0 && item < nitems) {
@@ -157,35 +177,35 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
           }
         }
       }
-      eo2<PDEG, MAT_NS, false>(x, y);
+      eo2d<PDEG, MAT_NS, false, DBG>(x, y);
       sts_line2<N>(A + base + b2, stride, y);
     }
-    __syncthreads();
+    FE_SYNC();
     // phase 1: Ns along y, in place
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<1>(l, base, stride);
       v2 x[N], y[N];
       lds_line2<N>(A + base + b2, stride, x);
-      eo2<PDEG, MAT_NS, false>(x, y);
+      eo2d<PDEG, MAT_NS, false, DBG>(x, y);
       sts_line2<N>(A + base + b2, stride, y);
     }
-    if (tid == 0) tma_wait_read0();     // the previous item's reduction has finished reading tile B
-    __syncthreads();
+    if (TMA_OUT && tid == 0) tma_wait_read0();     // the previous item's reduction has finished reading tile B
+    FE_SYNC();
     // phase 2: Ns along z -> T (A); R = gm*T + Ds^T gzz Ds T along z -> B
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
       v2 x[N], tq[N], r[N];
       lds_line2<N>(A + base + b2, stride, x);
-      eo2<PDEG, MAT_NS, false>(x, tq);
+      eo2d<PDEG, MAT_NS, false, DBG>(x, tq);
       sts_line2<N>(A + base + b2, stride, tq);
 #pragma unroll
       for (int i = 0; i < N; ++i) r[i] = vmul(gm, tq[i]);
-      kterm2<PDEG>(tq, r, gzz);
+      kterm2d<PDEG, DBG>(tq, r, gzz);
       sts_line2<N>(B + base + b2, stride, r);
     }
-    __syncthreads();
+    FE_SYNC();
     // phase 3: R += Ds^T gxx Ds T along x
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
@@ -193,10 +213,10 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
       v2 tq[N], r[N];
       lds_line2<N>(A + base + b2, stride, tq);
       lds_line2<N>(B + base + b2, stride, r);
-      kterm2<PDEG>(tq, r, gxx);
+      kterm2d<PDEG, DBG>(tq, r, gxx);
       sts_line2<N>(B + base + b2, stride, r);
     }
-    __syncthreads();
+    FE_SYNC();
     // phase 4: R += Ds^T gyy Ds T along y, then Ns^T along y, in place in B
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
@@ -204,11 +224,11 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
       v2 tq[N], r[N], u[N];
       lds_line2<N>(A + base + b2, stride, tq);
       lds_line2<N>(B + base + b2, stride, r);
-      kterm2<PDEG>(tq, r, gyy);
-      eo2<PDEG, MAT_NS, true>(r, u);
+      kterm2d<PDEG, DBG>(tq, r, gyy);
+      eo2d<PDEG, MAT_NS, true, DBG>(r, u);
       sts_line2<N>(B + base + b2, stride, u);
     }
-    __syncthreads();
+    FE_SYNC();
     // tile A is free: prefetch the next item's tile (overlaps phases 5-6)
     if (tid == 0) {
       const int nxt = item + gridDim.x;
@@ -225,17 +245,44 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N], y[N];
       lds_line2<N>(B + base + b2, stride, x);
-      eo2<PDEG, MAT_NS, true>(x, y);
+      eo2d<PDEG, MAT_NS, true, DBG>(x, y);
       sts_line2<N>(B + base + b2, stride, y);
     }
-    __syncthreads();
+    FE_SYNC();
     // phase 6: Ns^T along z, in place; Dirichlet rows zeroed; wrap-around elements scattered by RED
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
       v2 x[N], y[N];
       lds_line2<N>(B + base + b2, stride, x);
-      eo2<PDEG, MAT_NS, true>(x, y);
+      eo2d<PDEG, MAT_NS, true, DBG>(x, y);
+      if (!TMA_OUT) {
+        // direct scatter-add from registers (RED.F64): saves the tile write + TMA read of the result
+        const int i1 = l % N, i2 = l / N;
+        int ix = ex * PDEG + i1, iy = ey * PDEG + i2;
+        bool live = (v0 + b2) < P.nvec;
+        bool first_ok = true, last_ok = true;
+        const long long plane = (long long)P.ndx * P.ndy * nvec;
+        long long last_off = (long long)PDEG * plane;
+        if (dirichlet) {
+          if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1) live = false;
+          first_ok = (ez != 0); last_ok = (ez != P.ncz - 1);
+        } else {
+          if (ix >= P.ndx) ix -= P.ndx;
+          if (iy >= P.ndy) iy -= P.ndy;
+          if (wz) last_off -= (long long)P.ndz * plane;
+        }
+        if (live) {
+          double* dst = P.Z + ((long long)ix + (long long)P.ndx * iy) * nvec + (long long)ez * PDEG * plane + v0 + b2;
+#pragma unroll
+          for (int i = 0; i < N; ++i) {
+            const bool ok = (i == 0 ? first_ok : (i == N - 1 ? last_ok : true));
+            const long long off = (i == N - 1) ? last_off : (long long)i * plane;
+            if (ok) { atomicAdd(dst + off, y[i].a); atomicAdd(dst + off + 1, y[i].b); }
+          }
+        }
+        continue;
+      }
       if (special) {
         const int i1 = l % N, i2 = l / N;
         int ix = ex * PDEG + i1, iy = ey * PDEG + i2;
@@ -267,14 +314,16 @@ fe_apply_cart_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant
       }
       sts_line2<N>(B + base + b2, stride, y);
     }
-    fence_async_smem();
-    __syncthreads();
-    if (tid == 0) {
-      tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
-      tma_commit();
+    if (TMA_OUT) {
+      fence_async_smem();
+      FE_SYNC();
+      if (tid == 0) {
+        tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
+        tma_commit();
+      }
     }
   }
-  if (tid == 0) tma_wait_all0();
+  if (TMA_OUT && tid == 0) tma_wait_all0();
 }
 
 }  // namespace fe
