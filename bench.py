@@ -150,7 +150,7 @@ def run_reference(args):
 def run_ours(args):
     import numpy as np
     import torch
-    from paper_2208_07129_b200 import binding, build, inputs, roofline
+    from paper_2208_07129_b200 import binding, build, inputs, roofline, sharding
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -173,7 +173,8 @@ def run_ours(args):
     count = w.ndof * nvec
     X = torch.empty(count, dtype=torch.float64, device="cuda")
     Y = torch.empty_like(X)
-    binding.fill_uniform(X, w.seed, offset=rank * count)     # weak scaling: rank r owns columns [r*nvec, (r+1)*nvec)
+    # weak scaling: rank r owns its own nvec-column block (a distinct slice of the seeded stream)
+    binding.fill_uniform(X, w.seed, offset=sharding.generator_offset(rank, w.ndof, nvec))
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -203,12 +204,9 @@ def run_ours(args):
     torch.cuda.synchronize()
     clocks = sampler.stop()
     ms_kernel = k0.elapsed_time(k1) / args.steps
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = sharding.max_over_ranks(ms_total, dist, "cuda")
     ms_step = ms_total / args.steps
-    value = world * count / (ms_step * 1e-3) / 1e9
+    value = sharding.aggregate_throughput(count, world, ms_step * 1e-3) / 1e9
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -225,10 +223,7 @@ def run_ours(args):
             op.apply_host(Xh, Yh, nvec)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = sharding.max_over_ranks(dt, dist, "cuda")
         e2e = {"value": world * count * n_e2e / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": count * 8,
                "d2h_bytes_per_step": count * 8, "steps": n_e2e, "api": "fe_mf_apply_host (pinned host buffers)"}
         y_host_check = float((Yh.cuda() - Y).abs().max().item())
