@@ -172,14 +172,50 @@ cudaError_t launch_tma(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUt
   return cudaGetLastError();
 }
 
+// ---- persistent TMA kernel for a full symmetric metric (per-q-point / per-cell geometry)
+template <int PDEG> struct GenCfg;
+template <> struct GenCfg<1> { static constexpr int BV = 8, NT = 32, MINB = 4; };
+template <> struct GenCfg<2> { static constexpr int BV = 8, NT = 64, MINB = 4; };
+template <> struct GenCfg<3> { static constexpr int BV = 8, NT = 64, MINB = 4; };
+template <> struct GenCfg<4> { static constexpr int BV = 8, NT = 128, MINB = 3; };
+template <> struct GenCfg<5> { static constexpr int BV = 8, NT = 160, MINB = 2; };
+template <> struct GenCfg<6> { static constexpr int BV = 8, NT = 128, MINB = 3; };
+template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 128, MINB = 2; };
+template <> struct GenCfg<8> { static constexpr int BV = 4, NT = 192, MINB = 2; };
+int gen_bv(int p) { return p == 8 ? 4 : 8; }
+
+template <int PDEG>
+cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                       cudaStream_t st) {
+  using C = GenCfg<PDEG>;
+  constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  static int blocks_per_sm = 0;
+  auto kern = fe::fe_apply_gen_tma<PDEG, C::BV, C::NT, C::MINB>;
+  if (blocks_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
+    if (e != cudaSuccess) return e;
+    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+  }
+  const long long nitems = c->ncells * prm.nvb;
+  long long grid = (long long)blocks_per_sm * c->nsm;
+  if (grid > nitems) grid = nitems;
+  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
+  return cudaGetLastError();
+}
+
 // Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
 // 4 = Cartesian even-odd, two vectors per thread (production; needs even nvec and 16-byte aligned pointers).
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 1) return 1;
   const bool diag = (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
+  const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
+  const bool tma_ok = !(nvec & 1) && aligned && encode_tiled_fn() &&
+                      (unsigned long long)nvec * 8ULL * c->ndx * c->ndy < (1ULL << 40);
+  if ((!diag || c->variant == 7) && nvec >= 2 && tma_ok) return 6;   // full symmetric metric, TMA
   if (!diag || nvec < 4) return 1;
   if (c->variant == 2) return 2;
-  const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
   if ((nvec & 1) || !aligned) return 2;
   if (c->variant == 4) return 4;
   if (!encode_tiled_fn()) return 4;
@@ -187,7 +223,7 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   return 5;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
-  return kind == 1 ? general_bv(c->p, nvec) : (kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : ((c->variant == 5 && c->p >= 6) ? 8 : tma_bv(c->p))));
+  return kind == 1 ? general_bv(c->p, nvec) : (kind == 6 ? gen_bv(c->p) : kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : ((c->variant == 5 && c->p >= 6) ? 8 : tma_bv(c->p))));
 }
 
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
@@ -212,7 +248,21 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
   if (kind == 2) e = launch_cart_p<8>(c->p, P, c->ncells, st);
-  else if (kind == 5) {
+  else if (kind == 6) {
+    CUtensorMap tw, tz;
+    if (!make_tensor_map(&tw, c, W, nvec, bv) || !make_tensor_map(&tz, c, Z, nvec, bv))
+      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
+    switch (c->p) {
+      case 1: e = launch_gen<1>(c, P, tw, tz, st); break;
+      case 2: e = launch_gen<2>(c, P, tw, tz, st); break;
+      case 3: e = launch_gen<3>(c, P, tw, tz, st); break;
+      case 4: e = launch_gen<4>(c, P, tw, tz, st); break;
+      case 5: e = launch_gen<5>(c, P, tw, tz, st); break;
+      case 6: e = launch_gen<6>(c, P, tw, tz, st); break;
+      case 7: e = launch_gen<7>(c, P, tw, tz, st); break;
+      case 8: e = launch_gen<8>(c, P, tw, tz, st); break;
+    }
+  } else if (kind == 5) {
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
     CUtensorMap tw, tz;
     if (!make_tensor_map(&tw, c, W, nvec, bv) || !make_tensor_map(&tz, c, Z, nvec, bv))
@@ -423,7 +473,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 6) && variant != 101 && variant != 102) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 7) && variant != 101 && variant != 102) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -18,7 +18,7 @@ __constant__ double c_w[KMAXN][KMAXN];
 struct ApplyParams {
   const double* __restrict__ W;   // input multivector  [ndof][nvec]
   double* __restrict__ Z;         // output multivector [ndof][nvec], pre-initialised; Z += alpha*A*W
-  const double* __restrict__ geom;  // per-q-point: [cell][7][n^3]; per-cell: [cell][7]; or nullptr (uniform)
+  const double* __restrict__ geom;  // per-q-point: [cell][7][n^3]; per-cell: [cell][7]; or nullptr (uniform); no w_Q factor
   double ug[7];                   // uniform Cartesian: G00,G01,G02,G11,G12,G22 (x det J), sigma*det J
   double alpha;
   int ncx, ncy, ncz;
@@ -114,12 +114,12 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
     const int Q = t / bv;
     const int q1 = Q % N, q2 = (Q / N) % N, q3 = Q / (N * N);
     double g[7];
+    const double wq = c_w[PDEG][q1] * c_w[PDEG][q2] * c_w[PDEG][q3];
     if (P.geom_mode == 2) {
       const double* gp = P.geom + (size_t)cell * 7 * NN + Q;
 #pragma unroll
-      for (int k = 0; k < 7; ++k) g[k] = __ldg(gp + k * NN);
+      for (int k = 0; k < 7; ++k) g[k] = __ldg(gp + k * NN) * wq;
     } else {
-      const double wq = c_w[PDEG][q1] * c_w[PDEG][q2] * c_w[PDEG][q3];
       if (P.geom_mode == 1) {
 #pragma unroll
         for (int k = 0; k < 7; ++k) g[k] = __ldg(P.geom + (size_t)cell * 7 + k) * wq;

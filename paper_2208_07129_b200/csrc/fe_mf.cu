@@ -12,6 +12,7 @@
 #include "fe_kernels_eo.cuh"
 #include "fe_kernels_cart2.cuh"
 #include "fe_kernels_tma.cuh"
+#include "fe_kernels_gen.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {
@@ -161,6 +162,9 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
     fe::trilinear_jacobian(v, centre, J);
     if (!fe::metric_from_jacobian(J, c->ug)) { delete c; return fail(nullptr, FE_MF_EINVAL, "non-positive det J"); }
     c->ug[6] *= sigma;
+    e = cudaMalloc(&c->geom_dev, 7 * sizeof(double));   // the general TMA kernel reads the uniform metric from memory
+    if (e == cudaSuccess) e = cudaMemcpy(c->geom_dev, c->ug, 7 * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { if (c->geom_dev) cudaFree(c->geom_dev); delete c; return fail(nullptr, FE_MF_ECUDA, std::string("geometry upload: ") + cudaGetErrorString(e)); }
   } else {
     const bool perq = (geom == FE_GEOM_QPOINT);
     c->geom_mode = perq ? 2 : 1;
@@ -187,10 +191,9 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
                   const double xi[3] = {tab.xq[q1], tab.xq[q2], tab.xq[q3]};
                   fe::trilinear_jacobian(v, xi, J);
                   if (!fe::metric_from_jacobian(J, m)) { bad = true; continue; }
-                  const double wq = tab.w[q1] * tab.w[q2] * tab.w[q3];
                   const int Q = q1 + n * (q2 + n * q3);
-                  for (int k = 0; k < 6; ++k) g[(size_t)k * nn + Q] = m[k] * wq;
-                  g[(size_t)6 * nn + Q] = sigma * m[6] * wq;
+                  for (int k = 0; k < 6; ++k) g[(size_t)k * nn + Q] = m[k];
+                  g[(size_t)6 * nn + Q] = sigma * m[6];
                 }
           }
         }

@@ -231,3 +231,26 @@ def test_kernel_variants(env, variant, p, bc):
     Xd = torch.from_numpy(X).cuda(); Yd = torch.empty_like(Xd)
     op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6, 7, 8])
+def test_general_metric_tma_kernel_all_degrees(env, p, bc):
+    """Per-q-point geometry, even nvec: the persistent TMA kernel for a full symmetric metric (with vector tail)."""
+    nc = (3, 2, 3) if p <= 6 else (2, 2, 3)
+    w = inputs.Workload(f"gen_p{p}", p, nc, bc, inputs.GEOM_QPOINT, 0.9, (0.0, 0.0, 0.0), (1.5, 1.0, 2.0), 10, 3000 + p,
+                        perturb=0.15)
+    check_apply(env, w)
+
+
+@pytest.mark.parametrize("p", [3, 6, 8])
+def test_general_metric_kernel_on_uniform_mesh(env, p):
+    """variant 7 forces the full-metric kernel on a Cartesian mesh (metric read from memory, off-diagonals 0)."""
+    torch, orc, binding = env
+    w = inputs.Workload(f"gen_uniform_p{p}", p, (3, 2, 2), inputs.BC_PERIODIC, inputs.GEOM_AFFINE, 1.2, (0, 0, 0), (1.5, 1.0, 1.0), 8, 3100 + p)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    Yo = orc.Operator(oracle_mesh(orc, w), w.sigma).apply(X)
+    op = binding.FeMf.from_workload(w); op.set_variant(7)
+    Xd = torch.from_numpy(X).cuda(); Yd = torch.empty_like(Xd)
+    op.apply_axpby(0.5, Xd, 0.0, 0.0, Yd, w.nvec); torch.cuda.synchronize()
+    assert relerr(Yd.cpu().numpy(), 0.5 * Yo) <= TOL
