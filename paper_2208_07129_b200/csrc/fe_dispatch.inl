@@ -141,10 +141,16 @@ template <> struct TmaCfg<7> { static constexpr int BV = 16, NT = 256, MINB = 1;
 template <> struct TmaCfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
 int tma_bv(int p) { return p == 8 ? 8 : 16; }
 
+template <> struct TmaCfg<101> { static constexpr int BV = 8, NT = 32, MINB = 4; };
+template <> struct TmaCfg<102> { static constexpr int BV = 8, NT = 64, MINB = 4; };
+template <> struct TmaCfg<103> { static constexpr int BV = 8, NT = 64, MINB = 4; };
+template <> struct TmaCfg<104> { static constexpr int BV = 8, NT = 128, MINB = 4; };
+template <> struct TmaCfg<105> { static constexpr int BV = 8, NT = 160, MINB = 4; };
 template <> struct TmaCfg<106> { static constexpr int BV = 8, NT = 128, MINB = 5; };   // alt p=6
 template <> struct TmaCfg<107> { static constexpr int BV = 8, NT = 128, MINB = 3; };   // alt p=7
 template <> struct TmaCfg<108> { static constexpr int BV = 8, NT = 352, MINB = 1; };   // alt p=8
-int tma_bv_alt(int p) { return 8; }
+// 8 vectors per block when the call has at most 8 vectors (or on request): no lanes wasted on the vector tail
+bool tma_use_bv8(const fe_mf_ctx* c, int nvec) { return c->variant == 5 || nvec <= 8; }
 
 template <int PDEG, int CFG = PDEG, bool TMA_OUT = true, int DBG = 0>
 cudaError_t launch_tma(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
@@ -223,7 +229,7 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   return 5;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
-  return kind == 1 ? general_bv(c->p, nvec) : (kind == 6 ? gen_bv(c->p) : kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : ((c->variant == 5 && c->p >= 6) ? 8 : tma_bv(c->p))));
+  return kind == 1 ? general_bv(c->p, nvec) : (kind == 6 ? gen_bv(c->p) : kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : (tma_use_bv8(c, nvec) ? 8 : tma_bv(c->p))));
 }
 
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
@@ -267,14 +273,15 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
     CUtensorMap tw, tz;
     if (!make_tensor_map(&tw, c, W, nvec, bv) || !make_tensor_map(&tz, c, Z, nvec, bv))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
+    const bool alt = tma_use_bv8(c, nvec);
     switch (c->p) {
-      case 1: e = launch_tma<1>(c, P, tw, tz, st); break;
-      case 2: e = launch_tma<2>(c, P, tw, tz, st); break;
-      case 3: e = launch_tma<3>(c, P, tw, tz, st); break;
-      case 4: e = launch_tma<4>(c, P, tw, tz, st); break;
-      case 5: e = launch_tma<5>(c, P, tw, tz, st); break;
-      case 6: e = (c->variant == 5) ? launch_tma<6, 106>(c, P, tw, tz, st) : (c->variant == 6 ? launch_tma<6, 6, false>(c, P, tw, tz, st) : (c->variant == 101 ? launch_tma<6, 6, true, 1>(c, P, tw, tz, st) : (c->variant == 102 ? launch_tma<6, 6, true, 2>(c, P, tw, tz, st) : launch_tma<6>(c, P, tw, tz, st)))); break;
-      case 7: e = (c->variant == 5) ? launch_tma<7, 107>(c, P, tw, tz, st) : launch_tma<7>(c, P, tw, tz, st); break;
+      case 1: e = alt ? launch_tma<1, 101>(c, P, tw, tz, st) : launch_tma<1>(c, P, tw, tz, st); break;
+      case 2: e = alt ? launch_tma<2, 102>(c, P, tw, tz, st) : launch_tma<2>(c, P, tw, tz, st); break;
+      case 3: e = alt ? launch_tma<3, 103>(c, P, tw, tz, st) : launch_tma<3>(c, P, tw, tz, st); break;
+      case 4: e = alt ? launch_tma<4, 104>(c, P, tw, tz, st) : launch_tma<4>(c, P, tw, tz, st); break;
+      case 5: e = alt ? launch_tma<5, 105>(c, P, tw, tz, st) : launch_tma<5>(c, P, tw, tz, st); break;
+      case 6: e = alt ? launch_tma<6, 106>(c, P, tw, tz, st) : (c->variant == 6 ? launch_tma<6, 6, false>(c, P, tw, tz, st) : (c->variant == 101 ? launch_tma<6, 6, true, 1>(c, P, tw, tz, st) : launch_tma<6>(c, P, tw, tz, st))); break;
+      case 7: e = alt ? launch_tma<7, 107>(c, P, tw, tz, st) : launch_tma<7>(c, P, tw, tz, st); break;
       case 8: e = (c->variant == 5) ? launch_tma<8, 108>(c, P, tw, tz, st) : launch_tma<8>(c, P, tw, tz, st); break;
     }
   } else if (kind == 4) {
@@ -473,7 +480,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 7) && variant != 101 && variant != 102) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 7) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }
