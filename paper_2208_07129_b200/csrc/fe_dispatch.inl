@@ -117,12 +117,19 @@ EncodeTiledFn encode_tiled_fn() {
 }
 
 // 4-D FP64 tensor map of a multivector [z][y][x][beta] with box (bv, n, n, n).
-bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv) {
+// Dirichlet meshes, plane kernels: trim = 2 -> the map covers nodes 1 .. nd-2 in every direction, origin at node
+// (1,1,1), so that boundary nodes are out of bounds (zero on load; box coordinates shift by -1); trim = 1 -> nodes
+// 0 .. nd-2, origin unchanged (the last node is clipped on reduce).
+bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim = 0) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
-  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)c->ndx, (cuuint64_t)c->ndy, (cuuint64_t)c->ndz};
+  const int cut = trim;
+  const bool interior = (trim == 2);
+  if (trim && (c->ndx < 3 || c->ndy < 3 || c->ndz < 3)) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)(c->ndx - cut), (cuuint64_t)(c->ndy - cut), (cuuint64_t)(c->ndz - cut)};
   const cuuint64_t strides[3] = {(cuuint64_t)nvec * 8, (cuuint64_t)nvec * 8 * c->ndx, (cuuint64_t)nvec * 8 * c->ndx * c->ndy};
   if (strides[2] >= ((cuuint64_t)1 << 40)) return false;
+  if (interior) base = (const char*)base + (strides[0] + strides[1] + strides[2]);
   const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)c->n, (cuuint32_t)c->n, (cuuint32_t)c->n};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
@@ -211,6 +218,33 @@ cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUt
   return cudaGetLastError();
 }
 
+// ---- plane kernel (one thread = one n x n plane of one vector), uniform Cartesian cells
+template <int PDEG> struct PlaneCfg;
+template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 2; };
+template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };
+bool plane_ok(int p) { return p == 6 || p == 7; }
+
+template <int PDEG>
+cudaError_t launch_plane(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                         cudaStream_t st) {
+  using C = PlaneCfg<PDEG>;
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  static int blocks_per_sm = 0;
+  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB>;
+  if (blocks_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
+    if (e != cudaSuccess) return e;
+    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+  }
+  const long long nitems = c->ncells * prm.nvb;
+  long long grid = (long long)blocks_per_sm * c->nsm;
+  if (grid > nitems) grid = nitems;
+  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
+  return cudaGetLastError();
+}
+
 // Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
 // 4 = Cartesian even-odd, two vectors per thread (production; needs even nvec and 16-byte aligned pointers).
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
@@ -226,9 +260,11 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 4) return 4;
   if (!encode_tiled_fn()) return 4;
   if ((unsigned long long)nvec * 8ULL * c->ndx * c->ndy >= (1ULL << 40)) return 4;
+  if (c->variant == 8 && plane_ok(c->p)) return 8;
   return 5;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
+  if (kind == 8) return 16;
   return kind == 1 ? general_bv(c->p, nvec) : (kind == 6 ? gen_bv(c->p) : kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : (tma_use_bv8(c, nvec) ? 8 : tma_bv(c->p))));
 }
 
@@ -267,6 +303,16 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
       case 6: e = launch_gen<6>(c, P, tw, tz, st); break;
       case 7: e = launch_gen<7>(c, P, tw, tz, st); break;
       case 8: e = launch_gen<8>(c, P, tw, tz, st); break;
+    }
+  } else if (kind == 8) {
+    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
+    CUtensorMap tw, tz;
+    const bool dir = (c->bc == FE_BC_DIRICHLET);
+    if (!make_tensor_map(&tw, c, W, nvec, bv, dir ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, dir ? 1 : 0))
+      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
+    switch (c->p) {
+      case 6: e = launch_plane<6>(c, P, tw, tz, st); break;
+      case 7: e = launch_plane<7>(c, P, tw, tz, st); break;
     }
   } else if (kind == 5) {
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
@@ -480,7 +526,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 7) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 8) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -1,0 +1,333 @@
+// Device code, part 6: "plane" kernels -- one thread owns a whole n x n plane of the cell tile for ONE vector.
+//
+// Why: with line tasks (fe_kernels_tma.cuh) every 1D contraction is a shared-memory round trip (18 tile
+// accesses per point) and the shared-memory pipe (128 B/clk/SM) is as loaded as the FP64 pipe, with seven
+// block barriers per cell.  A thread that holds an n x n plane in registers applies the contractions of
+// TWO directions between one load and one store:
+//
+//   P1  xy-plane (i3 fixed):  A <- Ns_y Ns_x A                                       (S3, dims 1-2)
+//   P2  z-lines of an xz-plane: T = Ns_z A -> A ;  R = gm T + Ds_z^T gzz Ds_z T -> B  (S3 dim 3, S4-S6 z-part)
+//   P3  xy-plane: R += Ds_x^T gxx Ds_x T + Ds_y^T gyy Ds_y T ; B <- Ns_x^T Ns_y^T R   (S4-S6 x,y; S7 dims 1-2)
+//   P4  z-lines: B <- Ns_z^T B                                                        (S7 dim 3) -> TMA reduce (S8)
+//
+// 11 thread tile accesses per point (+2 by the TMA unit) and 4 barriers per cell.  Consecutive 1D operators
+// on the same line stay in the even/odd basis (no combine followed by split), and the quadrature-point
+// factor is folded into the accumulate FMA: 94.8 FP64 instructions per DoF*vector at p = 6 instead of 111.8.
+//
+// Even/odd algebra (derived from the centro-symmetry M[n-1-q][n-1-i] = s M[q][i], reading 14):
+//   split:    xp_i = x_i + x_{n-1-i},  xm_i = x_i - x_{n-1-i},  xc = x_mid
+//   mult:     u = P xp + Pm xc,  v = Mn xm,  m = mid . xp + midm xc  (s = +1)   |   m = mid . xm  (s = -1)
+//   combine:  y_q = u_q + v_q,  y_{n-1-q} = s (u_q - v_q),  y_mid = m
+// so y_q + y_{n-1-q} = 2u (s=+1) or 2v (s=-1) and y_q - y_{n-1-q} = 2v or 2u: the (u, v, m) of one operator
+// feed the next one directly; the missing factor 2 on (xp, xm) relative to xc is absorbed by halved
+// middle-column tables (HALF) and by the scalar of the final accumulate.
+#pragma once
+#include "fe_kernels_tma.cuh"
+
+namespace fe {
+
+struct EoTab2 {
+  double P[16], Mn[16];
+  double Pm[4], mid[4];
+  double Pmh[4], midh[4];   // Pm / 2, mid / 2
+  double midm, midmh;       // M[mid][mid] and half of it
+  double pad[2];
+};
+__constant__ EoTab2 c_eo2[KMAXN][2];   // [p][MAT_NS | MAT_DS]
+
+template <int N>
+__device__ __forceinline__ void eo_split(const double (&x)[N], double (&xp)[N / 2 > 0 ? N / 2 : 1],
+                                         double (&xm)[N / 2 > 0 ? N / 2 : 1]) {
+#pragma unroll
+  for (int i = 0; i < N / 2; ++i) { xp[i] = x[i] + x[N - 1 - i]; xm[i] = x[i] - x[N - 1 - i]; }
+}
+
+// (u, v, m) of y = M x (or M^T x) from (xp, xm, xc).  HALF: (xp, xm) carry half their true value relative to
+// xc; the outputs are then half the true (u, v, m).
+template <int PDEG, int MAT, bool TRANS, bool HALF>
+__device__ __forceinline__ void eo_mult(const double (&xp)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                        const double (&xm)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], double xc,
+                                        double (&u)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                        double (&v)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], double& m) {
+  constexpr int N = PDEG + 1, H = N / 2;
+  constexpr bool ODD = (N & 1) != 0, ANTI = (MAT == MAT_DS);
+  const EoTab2& t = c_eo2[PDEG][MAT];
+#pragma unroll
+  for (int q = 0; q < H; ++q) {
+    double a = (!TRANS ? t.P[q * H] : (ANTI ? t.Mn[q] : t.P[q])) * xp[0];
+#pragma unroll
+    for (int i = 1; i < H; ++i) a = fma(!TRANS ? t.P[q * H + i] : (ANTI ? t.Mn[i * H + q] : t.P[i * H + q]), xp[i], a);
+    if (ODD) a = fma(!TRANS ? (HALF ? t.Pmh[q] : t.Pm[q]) : (HALF ? t.midh[q] : t.mid[q]), xc, a);
+    double b = (!TRANS ? t.Mn[q * H] : (ANTI ? t.P[q] : t.Mn[q])) * xm[0];
+#pragma unroll
+    for (int i = 1; i < H; ++i) b = fma(!TRANS ? t.Mn[q * H + i] : (ANTI ? t.P[i * H + q] : t.Mn[i * H + q]), xm[i], b);
+    u[q] = a; v[q] = b;
+  }
+  m = 0.0;
+  if (ODD) {
+    if (ANTI) {
+      double c = (!TRANS ? t.mid[0] : t.Pm[0]) * xm[0];
+#pragma unroll
+      for (int i = 1; i < H; ++i) c = fma(!TRANS ? t.mid[i] : t.Pm[i], xm[i], c);
+      m = c;
+    } else {
+      double c = (HALF ? t.midmh : t.midm) * xc;
+#pragma unroll
+      for (int i = 0; i < H; ++i) c = fma(!TRANS ? t.mid[i] : t.Pm[i], xp[i], c);
+      m = c;
+    }
+  }
+}
+
+template <int N, bool ANTI>
+__device__ __forceinline__ void eo_combine(const double (&u)[N / 2 > 0 ? N / 2 : 1], const double (&v)[N / 2 > 0 ? N / 2 : 1],
+                                           double m, double (&y)[N]) {
+#pragma unroll
+  for (int q = 0; q < N / 2; ++q) { y[q] = u[q] + v[q]; y[N - 1 - q] = ANTI ? (v[q] - u[q]) : (u[q] - v[q]); }
+  if (N & 1) y[N / 2] = m;
+}
+
+// y = M x or M^T x, complete (split, mult, combine); x and y may be the same array.
+template <int PDEG, int MAT, bool TRANS>
+__device__ __forceinline__ void eo_full(const double (&x)[PDEG + 1], double (&y)[PDEG + 1]) {
+  constexpr int N = PDEG + 1, HH = N / 2 > 0 ? N / 2 : 1;
+  double xp[HH], xm[HH], u[HH], v[HH], m;
+  eo_split<N>(x, xp, xm);
+  eo_mult<PDEG, MAT, TRANS, false>(xp, xm, x[N / 2], u, v, m);
+  eo_combine<N, MAT == MAT_DS>(u, v, m, y);
+}
+
+// (u2, v2, m2) = HALF of the even/odd parts of Ds^T Ds t, from the line t.
+template <int PDEG>
+__device__ __forceinline__ void eo_dtd(const double (&t)[PDEG + 1], double (&u2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                       double (&v2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], double& m2) {
+  constexpr int N = PDEG + 1, HH = N / 2 > 0 ? N / 2 : 1;
+  double tp[HH], tm[HH], u1[HH], v1[HH], m1;
+  eo_split<N>(t, tp, tm);
+  eo_mult<PDEG, MAT_DS, false, false>(tp, tm, t[N / 2], u1, v1, m1);
+  eo_mult<PDEG, MAT_DS, true, true>(v1, u1, m1, u2, v2, m2);
+}
+
+// Periodic wrap fix-ups of the last cell in a direction, done cooperatively on the shared-memory tile so that
+// the plane phases stay branch-free: only the (up to three) wrapped faces i_d = N-1 are visited.
+// IN (OUT = false): fetch the wrap-around nodes the TMA box could not reach (it zero-filled them).
+// OUT: RED the wrap-around nodes that the clipped TMA reduction will not store.
+template <int PDEG, int BV, int NT, bool OUT>
+__device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams& P, int tid, int ex, int ey, int ez, int v0,
+                                                 bool wx, bool wy, bool wz) {
+  constexpr int N = PDEG + 1, HB = BV / 2, FACE = N * N * HB;
+  const long long nvec = P.nvec;
+#pragma unroll
+  for (int f = 0; f < 3; ++f) {
+    if (!(f == 0 ? wx : (f == 1 ? wy : wz))) continue;
+#pragma unroll 1
+    for (int r = tid; r < FACE; r += NT) {
+      const int b2 = (r % HB) * 2, a = (r / HB) % N, b = r / (HB * N);
+      int i1, i2, i3;
+      if (f == 0) { i1 = N - 1; i2 = a; i3 = b; }
+      else if (f == 1) { i2 = N - 1; i1 = a; i3 = b; if (wx && i1 == N - 1) continue; }
+      else { i3 = N - 1; i1 = a; i2 = b; if ((wx && i1 == N - 1) || (wy && i2 == N - 1)) continue; }
+      if ((v0 + b2) >= P.nvec) continue;
+      int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+      const long long g = ((long long)ix + (long long)P.ndx * ((long long)iy + (long long)P.ndy * iz)) * nvec + v0 + b2;
+      double2* s = reinterpret_cast<double2*>(tile + ((i3 * N + i2) * N + i1) * BV + b2);
+      if (!OUT) {
+        *s = __ldg(reinterpret_cast<const double2*>(P.W + g));
+      } else {
+        const double2 d = *s;
+        atomicAdd(P.Z + g, d.x); atomicAdd(P.Z + g + 1, d.y);
+      }
+    }
+  }
+}
+
+// Z += A W on uniform Cartesian cells (diagonal constant metric; alpha folded into P.ug).  One block = one
+// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta; N*BV <= NT.
+template <int PDEG, int BV, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
+fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
+                    const __grid_constant__ ApplyParams P, int nitems) {
+  using TL = DenseTile<PDEG, BV>;
+  constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1;
+  constexpr int S1 = BV, S2 = N * BV, S3 = N * N * BV;   // element strides along x, y, z
+  static_assert(N * BV <= NT, "one plane task per thread");
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  double* A = reinterpret_cast<double*>(smem_raw);
+  double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TL::PITCH);
+  const int tid = threadIdx.x;
+  const int beta = tid % BV, k = tid / BV;
+  const bool active = k < N;
+  // Dirichlet: the input tensor map covers the INTERIOR nodes only (origin = node (1,1,1)), so boundary nodes are
+  // out of bounds for the TMA unit and arrive as zeros (X read as 0).  A bulk tensor REDUCTION faults on negative
+  // coordinates (measured on sm_100a), so the output map keeps its origin at node 0 and drops only the last
+  // node per direction (clipped); the low boundary faces are zeroed in registers in P4 (Y rows stay 0).
+  const bool dirichlet = P.dirichlet != 0;
+  const int org = dirichlet ? -1 : 0;
+  const double g2x = 2.0 * P.ug[0], g2y = 2.0 * P.ug[3], g4y = 4.0 * P.ug[3], g4z = 4.0 * P.ug[5], gm = P.ug[6];
+
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  int item = blockIdx.x;
+  if (tid == 0 && item < nitems) {
+    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
+    mbar_expect_tx(bar, TL::BYTES);
+    tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + org);
+  }
+  uint32_t parity = 0;
+  for (; item < nitems; item += gridDim.x) {
+    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
+    const int v0 = vb * BV;
+    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
+    const bool special = wx || wy || wz;
+    const bool dlow = dirichlet && (ex == 0 || ey == 0 || ez == 0);
+    mbar_wait(bar, parity);
+    parity ^= 1u;
+    if (special) {
+      plane_wrap_fixup<PDEG, BV, NT, false>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
+      __syncthreads();
+    }
+
+    // P1: xy-plane i3 = k: Ns along x (rows) then along y (columns), in registers
+    if (active) {
+      double* a = A + k * S3 + beta;
+      double r[N][N];
+#pragma unroll
+      for (int j = 0; j < N; ++j)
+#pragma unroll
+        for (int i = 0; i < N; ++i) r[j][i] = a[j * S2 + i * S1];
+#pragma unroll
+      for (int j = 0; j < N; ++j) eo_full<PDEG, MAT_NS, false>(r[j], r[j]);
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        double c[N];
+#pragma unroll
+        for (int j = 0; j < N; ++j) c[j] = r[j][i];
+        eo_full<PDEG, MAT_NS, false>(c, c);
+#pragma unroll
+        for (int j = 0; j < N; ++j) a[j * S2 + i * S1] = c[j];
+      }
+    }
+    if (tid == 0) tma_wait_read0();   // the previous item's reduction has finished reading tile B
+    __syncthreads();
+
+    // P2: z-lines (i1, i2 = k): T = Ns_z A -> A ; R = gm T + 4 gzz (DtD T)/4 -> B
+    if (active) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        double* a = A + k * S2 + i * S1 + beta;
+        double* b = B + k * S2 + i * S1 + beta;
+        double x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u1[HH], v1[HH], m1, u2[HH], v2[HH], m2;
+#pragma unroll
+        for (int j = 0; j < N; ++j) x[j] = a[j * S3];
+        eo_split<N>(x, xp, xm);
+        eo_mult<PDEG, MAT_NS, false, false>(xp, xm, x[H], u, v, m);
+        eo_combine<N, false>(u, v, m, tq);
+#pragma unroll
+        for (int j = 0; j < N; ++j) a[j * S3] = tq[j];
+        eo_mult<PDEG, MAT_DS, false, true>(u, v, m, u1, v1, m1);      // half of Ds T
+        eo_mult<PDEG, MAT_DS, true, true>(v1, u1, m1, u2, v2, m2);    // quarter of Ds^T Ds T
+#pragma unroll
+        for (int q = 0; q < H; ++q) {
+          b[q * S3] = fma(g4z, u2[q] + v2[q], gm * tq[q]);
+          b[(N - 1 - q) * S3] = fma(g4z, v2[q] - u2[q], gm * tq[N - 1 - q]);
+        }
+        if (N & 1) b[H * S3] = fma(g4z, m2, gm * tq[H]);
+      }
+    }
+    __syncthreads();
+
+    // P3: xy-plane i3 = k: R += Kx T (rows) ; R += Ky T, Ns^T along y (columns) ; Ns^T along x (rows)
+    if (active) {
+      const double* a = A + k * S3 + beta;
+      double* b = B + k * S3 + beta;
+      double r[N][N];
+#pragma unroll
+      for (int j = 0; j < N; ++j)
+#pragma unroll
+        for (int i = 0; i < N; ++i) r[j][i] = b[j * S2 + i * S1];
+#pragma unroll
+      for (int j = 0; j < N; ++j) {
+        double t[N], u2[HH], v2[HH], m2;
+#pragma unroll
+        for (int i = 0; i < N; ++i) t[i] = a[j * S2 + i * S1];
+        eo_dtd<PDEG>(t, u2, v2, m2);
+#pragma unroll
+        for (int q = 0; q < H; ++q) {
+          r[j][q] = fma(g2x, u2[q] + v2[q], r[j][q]);
+          r[j][N - 1 - q] = fma(g2x, v2[q] - u2[q], r[j][N - 1 - q]);
+        }
+        if (N & 1) r[j][H] = fma(g2x, m2, r[j][H]);
+      }
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        double t[N], c[N], u2[HH], v2[HH], m2, rp[HH], rm[HH], u[HH], v[HH], m;
+#pragma unroll
+        for (int j = 0; j < N; ++j) { t[j] = a[j * S2 + i * S1]; c[j] = r[j][i]; }
+        eo_dtd<PDEG>(t, u2, v2, m2);
+        eo_split<N>(c, rp, rm);
+#pragma unroll
+        for (int q = 0; q < H; ++q) { rp[q] = fma(g4y, v2[q], rp[q]); rm[q] = fma(g4y, u2[q], rm[q]); }
+        const double rc = (N & 1) ? fma(g2y, m2, c[H]) : 0.0;
+        eo_mult<PDEG, MAT_NS, true, false>(rp, rm, rc, u, v, m);
+        eo_combine<N, false>(u, v, m, c);
+#pragma unroll
+        for (int j = 0; j < N; ++j) r[j][i] = c[j];
+      }
+#pragma unroll
+      for (int j = 0; j < N; ++j) {
+        eo_full<PDEG, MAT_NS, true>(r[j], r[j]);
+#pragma unroll
+        for (int i = 0; i < N; ++i) b[j * S2 + i * S1] = r[j][i];
+      }
+    }
+    __syncthreads();
+    // tile A is free: prefetch the next item's tile (overlaps P4 and the other resident block)
+    if (tid == 0) {
+      const int nxt = item + gridDim.x;
+      if (nxt < nitems) {
+        const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
+        const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
+        mbar_expect_tx(bar, TL::BYTES);
+        tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + org);
+      }
+    }
+    // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
+    if (active) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        double* b = B + k * S2 + i * S1 + beta;
+        double x[N];
+#pragma unroll
+        for (int j = 0; j < N; ++j) x[j] = b[j * S3];
+        eo_full<PDEG, MAT_NS, true>(x, x);
+        if (dlow) {
+          const bool zl = (ey == 0 && k == 0) || (ex == 0 && i == 0);
+#pragma unroll
+          for (int j = 0; j < N; ++j)
+            if (zl || (j == 0 && ez == 0)) x[j] = 0.0;
+        }
+#pragma unroll
+        for (int j = 0; j < N; ++j) b[j * S3] = x[j];
+      }
+    }
+    fence_async_smem();
+    __syncthreads();
+    if (special) plane_wrap_fixup<PDEG, BV, NT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
+    if (tid == 0) {
+      tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
+      tma_commit();
+    }
+  }
+  if (tid == 0) tma_wait_all0();
+}
+
+}  // namespace fe

@@ -13,6 +13,7 @@
 #include "fe_kernels_cart2.cuh"
 #include "fe_kernels_tma.cuh"
 #include "fe_kernels_gen.cuh"
+#include "fe_kernels_plane.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {
@@ -57,7 +58,7 @@ struct DeviceGuard {
 
 // Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
 // 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
-void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4]) {
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4], fe::EoTab2 out2[2]) {
   const int n = t.n, h = n / 2, m = n / 2;
   long double M[4][fe::MAXN * fe::MAXN];
   for (int q = 0; q < n; ++q)
@@ -81,6 +82,15 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4]) {
       for (int i = 0; i < h; ++i) out[k].mid[i] = (double)M[k][m * n + i];
       out[k].midm = (double)M[k][m * n + m];
     }
+  }
+  // the plane kernels' tables: Ns and Ds only (the transposes reuse them), plus the halved middle column / row
+  for (int k2 = 0; k2 < 2; ++k2) {
+    const fe::EoTab& s = out[2 * k2];
+    fe::EoTab2& d = out2[k2];
+    std::memset(&d, 0, sizeof(fe::EoTab2));
+    for (int i = 0; i < 16; ++i) { d.P[i] = s.P[i]; d.Mn[i] = s.Mn[i]; }
+    for (int i = 0; i < 4; ++i) { d.Pm[i] = s.Pm[i]; d.mid[i] = s.mid[i]; d.Pmh[i] = 0.5 * s.Pm[i]; d.midh[i] = 0.5 * s.mid[i]; }
+    d.midm = s.midm; d.midmh = 0.5 * s.midm;
   }
 }
 
@@ -144,8 +154,10 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
   if (e == cudaSuccess) {
     fe::EoTab eo[4];
-    make_eo_tables(tab, eo);
+    fe::EoTab2 eo2[2];
+    make_eo_tables(tab, eo, eo2);
     e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 4 * p);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 2 * p);
   }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
 
