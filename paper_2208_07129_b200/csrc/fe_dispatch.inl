@@ -220,17 +220,18 @@ cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUt
 
 // ---- plane kernel (one thread = one n x n plane of one vector), uniform Cartesian cells
 template <int PDEG> struct PlaneCfg;
-template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 2; };
-template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };
+template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 2, NH = 1; };
+template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1, NH = 1; };
+template <> struct PlaneCfg<106> { static constexpr int BV = 16, NT = 256, MINB = 1, NH = 2; };   // two groups in lockstep
 bool plane_ok(int p) { return p == 6 || p == 7; }
 
-template <int PDEG>
+template <int PDEG, int CFG = PDEG>
 cudaError_t launch_plane(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                          cudaStream_t st) {
-  using C = PlaneCfg<PDEG>;
-  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  using C = PlaneCfg<CFG>;
+  constexpr size_t SMEM = (size_t)2 * C::NH * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
   static int blocks_per_sm = 0;
-  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB>;
+  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, C::NH>;
   if (blocks_per_sm == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
     if (e != cudaSuccess) return e;
@@ -240,7 +241,7 @@ cudaError_t launch_plane(const fe_mf_ctx* c, const fe::ApplyParams& prm, const C
   }
   const long long nitems = c->ncells * prm.nvb;
   long long grid = (long long)blocks_per_sm * c->nsm;
-  if (grid > nitems) grid = nitems;
+  if (grid > (nitems + C::NH - 1) / C::NH) grid = (nitems + C::NH - 1) / C::NH;
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
 }
@@ -260,7 +261,7 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 4) return 4;
   if (!encode_tiled_fn()) return 4;
   if ((unsigned long long)nvec * 8ULL * c->ndx * c->ndy >= (1ULL << 40)) return 4;
-  if (c->variant == 8 && plane_ok(c->p)) return 8;
+  if ((c->variant == 8 || c->variant == 9) && plane_ok(c->p)) return 8;
   return 5;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
@@ -311,7 +312,7 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
     if (!make_tensor_map(&tw, c, W, nvec, bv, dir ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, dir ? 1 : 0))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
     switch (c->p) {
-      case 6: e = launch_plane<6>(c, P, tw, tz, st); break;
+      case 6: e = (c->variant == 9) ? launch_plane<6, 106>(c, P, tw, tz, st) : launch_plane<6>(c, P, tw, tz, st); break;
       case 7: e = launch_plane<7>(c, P, tw, tz, st); break;
     }
   } else if (kind == 5) {
@@ -526,7 +527,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 8) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 9) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

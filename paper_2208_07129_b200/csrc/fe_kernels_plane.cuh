@@ -24,6 +24,10 @@
 #pragma once
 #include "fe_kernels_tma.cuh"
 
+#ifndef FE_ZLOOP_PRAGMA   // the z-line loops of P2 / P4: rolled (small code) or unrolled (loads hoisted)
+#define FE_ZLOOP_PRAGMA _Pragma("unroll 1")
+#endif
+
 namespace fe {
 
 struct EoTab2 {
@@ -145,20 +149,24 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
 }
 
 // Z += A W on uniform Cartesian cells (diagonal constant metric; alpha folded into P.ug).  One block = one
-// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta; N*BV <= NT.
-template <int PDEG, int BV, int NT, int MINB>
+// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta.  A block holds NH groups of
+// GT = NT/NH threads; each group works on its own item with its own tiles, and the groups share the block
+// barriers, so that the warps of one SM sub-partition walk through the (long, straight-line) code together and
+// share its instruction-cache lines.
+template <int PDEG, int BV, int NT, int MINB, int NH>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                     const __grid_constant__ ApplyParams P, int nitems) {
   using TL = DenseTile<PDEG, BV>;
   constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1;
   constexpr int S1 = BV, S2 = N * BV, S3 = N * N * BV;   // element strides along x, y, z
-  static_assert(N * BV <= NT, "one plane task per thread");
+  constexpr int GT = NT / NH;
+  static_assert(N * BV <= GT && GT % 128 == 0, "one plane task per thread; whole warps on every sub-partition");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  double* A = reinterpret_cast<double*>(smem_raw);
-  double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TL::PITCH);
-  const int tid = threadIdx.x;
+  const int grp = threadIdx.x / GT, tid = threadIdx.x % GT;
+  double* A = reinterpret_cast<double*>(smem_raw + (2 * grp) * TL::PITCH);
+  double* B = reinterpret_cast<double*>(smem_raw + (2 * grp + 1) * TL::PITCH);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * NH * TL::PITCH) + grp;
   const int beta = tid % BV, k = tid / BV;
   const bool active = k < N;
   // Dirichlet: the input tensor map covers the INTERIOR nodes only (origin = node (1,1,1)), so boundary nodes are
@@ -174,7 +182,8 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  int item = blockIdx.x;
+  const int stride = gridDim.x * NH;
+  int item = blockIdx.x * NH + grp;
   if (tid == 0 && item < nitems) {
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
@@ -182,22 +191,25 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + org);
   }
   uint32_t parity = 0;
-  for (; item < nitems; item += gridDim.x) {
+  for (int base = blockIdx.x * NH; base < nitems; base += stride, item += stride) {
+    const bool valid = item < nitems;   // a group without an item still joins the block barriers
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
-    const bool special = wx || wy || wz;
+    const bool special = valid && (wx || wy || wz);
     const bool dlow = dirichlet && (ex == 0 || ey == 0 || ez == 0);
-    mbar_wait(bar, parity);
+    const bool work = active && valid;
+    if (valid) mbar_wait(bar, parity);
     parity ^= 1u;
     if (special) {
-      plane_wrap_fixup<PDEG, BV, NT, false>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
-      __syncthreads();
+      plane_wrap_fixup<PDEG, BV, GT, false>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
+      if (NH == 1) __syncthreads();
+      else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "n"(GT) : "memory");
     }
 
     // P1: xy-plane i3 = k: Ns along x (rows) then along y (columns), in registers
-    if (active) {
+    if (work) {
       double* a = A + k * S3 + beta;
       double r[N][N];
 #pragma unroll
@@ -220,14 +232,21 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     __syncthreads();
 
     // P2: z-lines (i1, i2 = k): T = Ns_z A -> A ; R = gm T + 4 gzz (DtD T)/4 -> B
-    if (active) {
+    if (work) {
+      double xn[N];   // software pipeline: the next line is in flight while this one is computed
 #pragma unroll
+      for (int j = 0; j < N; ++j) xn[j] = A[k * S2 + beta + j * S3];
+FE_ZLOOP_PRAGMA
       for (int i = 0; i < N; ++i) {
         double* a = A + k * S2 + i * S1 + beta;
         double* b = B + k * S2 + i * S1 + beta;
         double x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u1[HH], v1[HH], m1, u2[HH], v2[HH], m2;
 #pragma unroll
-        for (int j = 0; j < N; ++j) x[j] = a[j * S3];
+        for (int j = 0; j < N; ++j) x[j] = xn[j];
+        if (i + 1 < N) {
+#pragma unroll
+          for (int j = 0; j < N; ++j) xn[j] = a[S1 + j * S3];
+        }
         eo_split<N>(x, xp, xm);
         eo_mult<PDEG, MAT_NS, false, false>(xp, xm, x[H], u, v, m);
         eo_combine<N, false>(u, v, m, tq);
@@ -246,7 +265,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     __syncthreads();
 
     // P3: xy-plane i3 = k: R += Kx T (rows) ; R += Ky T, Ns^T along y (columns) ; Ns^T along x (rows)
-    if (active) {
+    if (work) {
       const double* a = A + k * S3 + beta;
       double* b = B + k * S3 + beta;
       double r[N][N];
@@ -292,7 +311,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     __syncthreads();
     // tile A is free: prefetch the next item's tile (overlaps P4 and the other resident block)
     if (tid == 0) {
-      const int nxt = item + gridDim.x;
+      const int nxt = item + stride;
       if (nxt < nitems) {
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
@@ -301,13 +320,20 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
       }
     }
     // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
-    if (active) {
+    if (work) {
+      double xn[N];
 #pragma unroll
+      for (int j = 0; j < N; ++j) xn[j] = B[k * S2 + beta + j * S3];
+FE_ZLOOP_PRAGMA
       for (int i = 0; i < N; ++i) {
         double* b = B + k * S2 + i * S1 + beta;
         double x[N];
 #pragma unroll
-        for (int j = 0; j < N; ++j) x[j] = b[j * S3];
+        for (int j = 0; j < N; ++j) x[j] = xn[j];
+        if (i + 1 < N) {
+#pragma unroll
+          for (int j = 0; j < N; ++j) xn[j] = b[S1 + j * S3];
+        }
         eo_full<PDEG, MAT_NS, true>(x, x);
         if (dlow) {
           const bool zl = (ey == 0 && k == 0) || (ex == 0 && i == 0);
@@ -321,8 +347,8 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     }
     fence_async_smem();
     __syncthreads();
-    if (special) plane_wrap_fixup<PDEG, BV, NT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
-    if (tid == 0) {
+    if (special) plane_wrap_fixup<PDEG, BV, GT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
+    if (tid == 0 && valid) {
       tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
       tma_commit();
     }
