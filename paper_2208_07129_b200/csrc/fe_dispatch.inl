@@ -193,15 +193,16 @@ template <> struct GenCfg<3> { static constexpr int BV = 8, NT = 64, MINB = 4; }
 template <> struct GenCfg<4> { static constexpr int BV = 8, NT = 128, MINB = 3; };
 template <> struct GenCfg<5> { static constexpr int BV = 8, NT = 160, MINB = 2; };
 template <> struct GenCfg<6> { static constexpr int BV = 8, NT = 128, MINB = 3; };
-template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 128, MINB = 2; };
-template <> struct GenCfg<8> { static constexpr int BV = 4, NT = 192, MINB = 2; };
-int gen_bv(int p) { return p == 8 ? 4 : 8; }
+template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 256, MINB = 1; };
+template <> struct GenCfg<8> { static constexpr int BV = 8, NT = 384, MINB = 1; };
+int gen_bv(int p) { (void)p; return 8; }
 
 template <int PDEG>
 cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                        cudaStream_t st) {
   using C = GenCfg<PDEG>;
-  constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  constexpr int NN = (PDEG + 1) * (PDEG + 1) * (PDEG + 1);
+  constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, C::BV>::PITCH + ((size_t)7 * NN * 8 + 15) / 16 * 16 + 64;
   static int blocks_per_sm = 0;
   auto kern = fe::fe_apply_gen_tma<PDEG, C::BV, C::NT, C::MINB>;
   if (blocks_per_sm == 0) {
@@ -280,6 +281,7 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.dirichlet = (c->bc == FE_BC_DIRICHLET) ? 1 : 0;
   P.geom_mode = c->geom_mode;
   P.nsm = c->nsm;
+  P.geom_stride = c->geom_stride;
   return P;
 }
 

@@ -29,6 +29,7 @@ struct ApplyParams {
   int dirichlet;                  // 1: boundary nodes read as 0 / not written
   int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
   int nsm;                        // SM count (persistent kernels)
+  long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
 };
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.
@@ -116,7 +117,7 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
     double g[7];
     const double wq = c_w[PDEG][q1] * c_w[PDEG][q2] * c_w[PDEG][q3];
     if (P.geom_mode == 2) {
-      const double* gp = P.geom + (size_t)cell * 7 * NN + Q;
+      const double* gp = P.geom + (size_t)cell * P.geom_stride + Q;
 #pragma unroll
       for (int k = 0; k < 7; ++k) g[k] = __ldg(gp + k * NN) * wq;
     } else {

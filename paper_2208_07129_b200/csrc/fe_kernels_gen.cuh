@@ -13,6 +13,8 @@
 //   ph7 y : A <- Ns_y^T A          ph8 x : A <- Ns_x^T A ; TMA reduce-add A -> Z
 //
 // 25 thread tile accesses per point + 2 by the TMA unit.  The tile roles rotate (A,B,C) <- (B,C,A) per item.
+// The cell's geometric factors (7 n^3 doubles, or 7 constants) are staged in shared memory by one bulk copy
+// (cp.async.bulk, mbarrier-tracked) issued one item ahead, so that ph4 never waits on global memory.
 #pragma once
 #include "fe_kernels_tma.cuh"
 
@@ -32,7 +34,11 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
   double* A = reinterpret_cast<double*>(smem_raw);
   double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);
   double* C = reinterpret_cast<double*>(smem_raw + 2 * TL::PITCH);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 3 * TL::PITCH);
+  constexpr int GBYTES = ((7 * NN * 8) + 15) / 16 * 16;
+  double* GS = reinterpret_cast<double*>(smem_raw + 3 * TL::PITCH);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 3 * TL::PITCH + GBYTES);
+  uint64_t* gbar = bar + 1;
+  const bool perq = (P.geom_mode == 2);
   const int tid = threadIdx.x;
   const long long nvec = P.nvec;
   const bool dirichlet = P.dirichlet != 0;
@@ -40,6 +46,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
 
   if (tid == 0) {
     mbar_init(bar, 1);
+    mbar_init(gbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -50,8 +57,12 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     mbar_expect_tx(bar, TL::BYTES);
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG, ey * PDEG, ez * PDEG);
+    if (perq) {
+      mbar_expect_tx(gbar, GBYTES);
+      bulk_load(GS, P.geom + (size_t)cell * P.geom_stride, GBYTES, gbar);
+    }
   }
-  uint32_t parity = 0;
+  uint32_t parity = 0, gparity = 0;
   int rot = (blockIdx.x / P.nsm) & 3;
   for (; item < nitems; item += gridDim.x, rot = (rot + 1) & 3) {
     const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
@@ -61,6 +72,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
     const bool special = dirichlet ? (ex == 0 || ex == P.ncx - 1 || ey == 0 || ey == P.ncy - 1 || ez == 0 || ez == P.ncz - 1)
                                    : (wx || wy || wz);
+    if (!perq && tid < 7) GS[tid] = __ldg(P.geom + (P.geom_mode == 1 ? (size_t)cell * 7 : 0) + tid);   // visible after the barriers below
     mbar_wait(bar, parity);
     parity ^= 1u;
 
@@ -142,6 +154,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       sts_line2<N>(B + base + b2, stride, d);
     }
     __syncthreads();
+    if (perq) { mbar_wait(gbar, gparity); gparity ^= 1u; }
     // ph4: T1 = Ds_y T; quadrature-point scaling with the symmetric metric (Alg. 2 l.5-6; Eq. 8, 22-23);
     //      R = Sm + Ds_y^T S1 -> A ; S0 -> B ; S2 -> C
     FE_FOR_TASKS(t) {
@@ -151,16 +164,15 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       v2 tq[N], t1[N], r[N];
       lds_line2<N>(A + base + b2, stride, tq);
       eo2<PDEG, MAT_DS, false>(tq, t1);
-      // geom: [cell][7][n^3] (per q-point), [cell][7] (per cell) or [7] (uniform); no w_Q factor (sqrt(w) tables)
-      const double* gp = (P.geom_mode == 2) ? P.geom + (size_t)cell * 7 * NN + (i1 + N * N * i3)
-                                            : (P.geom_mode == 1 ? P.geom + (size_t)cell * 7 : P.geom);
-      const int gstep = (P.geom_mode == 2) ? NN : 1;       // stride between the 7 factors
-      const int qstep = (P.geom_mode == 2) ? N : 0;        // stride between points along the y-line
+      // staged geometry: [7][n^3] (per q-point) or [7] (per cell / uniform); no w_Q factor (sqrt(w) tables)
+      const double* gp = perq ? GS + (i1 + N * N * i3) : GS;
+      const int gstep = perq ? NN : 1;       // stride between the 7 factors
+      const int qstep = perq ? N : 0;        // stride between points along the y-line
 #pragma unroll
       for (int i = 0; i < N; ++i) {
         const double* g = gp + i * qstep;
-        const double g00 = __ldg(g), g01 = __ldg(g + gstep), g02 = __ldg(g + 2 * gstep), g11 = __ldg(g + 3 * gstep),
-                     g12 = __ldg(g + 4 * gstep), g22 = __ldg(g + 5 * gstep), gm = __ldg(g + 6 * gstep);
+        const double g00 = g[0], g01 = g[gstep], g02 = g[2 * gstep], g11 = g[3 * gstep],
+                     g12 = g[4 * gstep], g22 = g[5 * gstep], gm = g[6 * gstep];
         const double2 a0 = *reinterpret_cast<const double2*>(B + base + b2 + i * stride);
         const double2 a2 = *reinterpret_cast<const double2*>(C + base + b2 + i * stride);
         const v2 t0 = {a0.x, a0.y}, t2 = {a2.x, a2.y}, t1i = t1[i];
@@ -178,6 +190,14 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       sts_line2<N>(A + base + b2, stride, r);
     }
     __syncthreads();
+    // the staged geometry is consumed: fetch the next item's
+    if (tid == 0 && perq) {
+      const int nxt = item + gridDim.x;
+      if (nxt < nitems) {
+        mbar_expect_tx(gbar, GBYTES);
+        bulk_load(GS, P.geom + (size_t)(nxt / P.nvb) * P.geom_stride, GBYTES, gbar);
+      }
+    }
     // ph5: R += Ds_x^T S0 -> A
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;

@@ -26,6 +26,7 @@ struct fe_mf_ctx {
   int geom_mode;            // 0 uniform, 1 per-cell, 2 per-q-point
   double ug[7];
   double* geom_dev = nullptr;
+  long long geom_stride = 7;   // doubles per cell in geom_dev
   int variant = 0;
   int last_launches = 0;
   // fe_mf_apply_host workspace
@@ -180,7 +181,8 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   } else {
     const bool perq = (geom == FE_GEOM_QPOINT);
     c->geom_mode = perq ? 2 : 1;
-    const size_t per_cell = perq ? (size_t)7 * nn : 7;
+    const size_t per_cell = perq ? (((size_t)7 * nn + 1) & ~(size_t)1) : 7;   // even: 16-byte bulk copies
+    c->geom_stride = (long long)per_cell;
     std::vector<double> G;
     try { G.resize(per_cell * (size_t)c->ncells); } catch (...) { delete c; return fail(nullptr, FE_MF_ENOMEM, "out of host memory (geometry)"); }
     bool bad = false;
