@@ -247,6 +247,39 @@ cudaError_t launch_plane(const fe_mf_ctx* c, const fe::ApplyParams& prm, const C
   return cudaGetLastError();
 }
 
+// ---- second-generation line kernel (two vectors per thread, fused even/odd chains)
+template <int CFG> struct LineCfg : TmaCfg<CFG> {};
+template <> struct LineCfg<207> { static constexpr int BV = 8, NT = 256, MINB = 2; };   // p=7: two blocks per SM
+template <> struct LineCfg<307> { static constexpr int BV = 16, NT = 512, MINB = 1; };  // p=7: one round per pass
+template <> struct LineCfg<407> { static constexpr int BV = 8, NT = 128, MINB = 3; };   // p=7: three blocks per SM
+template <> struct LineCfg<208> { static constexpr int BV = 8, NT = 384, MINB = 1; };   // p=8: one round per pass
+
+template <int PDEG, int CFG = PDEG>
+cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                        cudaStream_t st) {
+  using C = LineCfg<CFG>;
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  static int blocks_per_sm = 0;
+  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB>;
+  if (blocks_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
+    if (e != cudaSuccess) return e;
+    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+  }
+  const long long nitems = c->ncells * prm.nvb;
+  long long grid = (long long)blocks_per_sm * c->nsm;
+  if (grid > nitems) grid = nitems;
+  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
+  return cudaGetLastError();
+}
+// vectors per block of the line kernel for (p, variant)
+int line_bv(const fe_mf_ctx* c, int nvec) {
+  if (c->variant == 11 || c->variant == 12 || nvec <= 8) return 8;
+  return tma_bv(c->p);
+}
+
 // Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
 // 4 = Cartesian even-odd, two vectors per thread (production; needs even nvec and 16-byte aligned pointers).
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
@@ -262,11 +295,17 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 4) return 4;
   if (!encode_tiled_fn()) return 4;
   if ((unsigned long long)nvec * 8ULL * c->ndx * c->ndy >= (1ULL << 40)) return 4;
+  if (c->variant == 5 || c->variant == 6 || c->variant == 101) return 5;   // first-generation line kernel (kept for comparison)
+  if (c->variant >= 10 && c->variant <= 13) return 9;
+  // plane kernel: one plane of ONE vector per thread, 16 vectors per block; worth it when the last block is mostly full
+  const int tail = nvec % 16;
+  if (plane_ok(c->p) && c->p == 6 && nvec >= 12 && (tail == 0 || tail >= 12)) return 8;
   if ((c->variant == 8 || c->variant == 9) && plane_ok(c->p)) return 8;
-  return 5;
+  return 9;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
   if (kind == 8) return 16;
+  if (kind == 9) return line_bv(c, nvec);
   return kind == 1 ? general_bv(c->p, nvec) : (kind == 6 ? gen_bv(c->p) : kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : (tma_use_bv8(c, nvec) ? 8 : tma_bv(c->p))));
 }
 
@@ -316,6 +355,24 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
     switch (c->p) {
       case 6: e = (c->variant == 9) ? launch_plane<6, 106>(c, P, tw, tz, st) : launch_plane<6>(c, P, tw, tz, st); break;
       case 7: e = launch_plane<7>(c, P, tw, tz, st); break;
+    }
+  } else if (kind == 9) {
+    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
+    CUtensorMap tw, tz;
+    const bool dir = (c->bc == FE_BC_DIRICHLET);
+    if (!make_tensor_map(&tw, c, W, nvec, bv, dir ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, dir ? 1 : 0))
+      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
+    const bool alt = (bv == 8);
+    switch (c->p) {
+      case 1: e = alt ? launch_line<1, 101>(c, P, tw, tz, st) : launch_line<1>(c, P, tw, tz, st); break;
+      case 2: e = alt ? launch_line<2, 102>(c, P, tw, tz, st) : launch_line<2>(c, P, tw, tz, st); break;
+      case 3: e = alt ? launch_line<3, 103>(c, P, tw, tz, st) : launch_line<3>(c, P, tw, tz, st); break;
+      case 4: e = alt ? launch_line<4, 104>(c, P, tw, tz, st) : launch_line<4>(c, P, tw, tz, st); break;
+      case 5: e = alt ? launch_line<5, 105>(c, P, tw, tz, st) : launch_line<5>(c, P, tw, tz, st); break;
+      case 6: e = alt ? launch_line<6, 106>(c, P, tw, tz, st) : launch_line<6>(c, P, tw, tz, st); break;
+      case 7: e = alt ? (c->variant == 11 ? launch_line<7, 207>(c, P, tw, tz, st) : launch_line<7, 407>(c, P, tw, tz, st))
+                      : (c->variant == 13 ? launch_line<7, 307>(c, P, tw, tz, st) : launch_line<7>(c, P, tw, tz, st)); break;
+      case 8: e = (c->variant == 11) ? launch_line<8, 208>(c, P, tw, tz, st) : launch_line<8>(c, P, tw, tz, st); break;
     }
   } else if (kind == 5) {
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
@@ -529,7 +586,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 9) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 13) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -39,74 +39,79 @@ struct EoTab2 {
 };
 __constant__ EoTab2 c_eo2[KMAXN][2];   // [p][MAT_NS | MAT_DS]
 
-template <int N>
-__device__ __forceinline__ void eo_split(const double (&x)[N], double (&xp)[N / 2 > 0 ? N / 2 : 1],
-                                         double (&xm)[N / 2 > 0 ? N / 2 : 1]) {
+// The primitives are generic in the value type T: double (one vector per thread, plane kernels) or v2 (two
+// vectors per thread, line kernels).
+__device__ __forceinline__ double vmul(double c, double x) { return c * x; }
+__device__ __forceinline__ double vfma(double c, double x, double y) { return fma(c, x, y); }
+__device__ __forceinline__ void vzero(double& x) { x = 0.0; }
+__device__ __forceinline__ void vzero(v2& x) { x = {0.0, 0.0}; }
+
+template <int N, typename T>
+__device__ __forceinline__ void eo_split(const T (&x)[N], T (&xp)[N / 2 > 0 ? N / 2 : 1], T (&xm)[N / 2 > 0 ? N / 2 : 1]) {
 #pragma unroll
   for (int i = 0; i < N / 2; ++i) { xp[i] = x[i] + x[N - 1 - i]; xm[i] = x[i] - x[N - 1 - i]; }
 }
 
 // (u, v, m) of y = M x (or M^T x) from (xp, xm, xc).  HALF: (xp, xm) carry half their true value relative to
 // xc; the outputs are then half the true (u, v, m).
-template <int PDEG, int MAT, bool TRANS, bool HALF>
-__device__ __forceinline__ void eo_mult(const double (&xp)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
-                                        const double (&xm)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], double xc,
-                                        double (&u)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
-                                        double (&v)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], double& m) {
+template <int PDEG, int MAT, bool TRANS, bool HALF, typename T>
+__device__ __forceinline__ void eo_mult(const T (&xp)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                        const T (&xm)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], T xc,
+                                        T (&u)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                        T (&v)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], T& m) {
   constexpr int N = PDEG + 1, H = N / 2;
   constexpr bool ODD = (N & 1) != 0, ANTI = (MAT == MAT_DS);
   const EoTab2& t = c_eo2[PDEG][MAT];
 #pragma unroll
   for (int q = 0; q < H; ++q) {
-    double a = (!TRANS ? t.P[q * H] : (ANTI ? t.Mn[q] : t.P[q])) * xp[0];
+    T a = vmul(!TRANS ? t.P[q * H] : (ANTI ? t.Mn[q] : t.P[q]), xp[0]);
 #pragma unroll
-    for (int i = 1; i < H; ++i) a = fma(!TRANS ? t.P[q * H + i] : (ANTI ? t.Mn[i * H + q] : t.P[i * H + q]), xp[i], a);
-    if (ODD) a = fma(!TRANS ? (HALF ? t.Pmh[q] : t.Pm[q]) : (HALF ? t.midh[q] : t.mid[q]), xc, a);
-    double b = (!TRANS ? t.Mn[q * H] : (ANTI ? t.P[q] : t.Mn[q])) * xm[0];
+    for (int i = 1; i < H; ++i) a = vfma(!TRANS ? t.P[q * H + i] : (ANTI ? t.Mn[i * H + q] : t.P[i * H + q]), xp[i], a);
+    if (ODD) a = vfma(!TRANS ? (HALF ? t.Pmh[q] : t.Pm[q]) : (HALF ? t.midh[q] : t.mid[q]), xc, a);
+    T b = vmul(!TRANS ? t.Mn[q * H] : (ANTI ? t.P[q] : t.Mn[q]), xm[0]);
 #pragma unroll
-    for (int i = 1; i < H; ++i) b = fma(!TRANS ? t.Mn[q * H + i] : (ANTI ? t.P[i * H + q] : t.Mn[i * H + q]), xm[i], b);
+    for (int i = 1; i < H; ++i) b = vfma(!TRANS ? t.Mn[q * H + i] : (ANTI ? t.P[i * H + q] : t.Mn[i * H + q]), xm[i], b);
     u[q] = a; v[q] = b;
   }
-  m = 0.0;
+  vzero(m);
   if (ODD) {
     if (ANTI) {
-      double c = (!TRANS ? t.mid[0] : t.Pm[0]) * xm[0];
+      T c = vmul(!TRANS ? t.mid[0] : t.Pm[0], xm[0]);
 #pragma unroll
-      for (int i = 1; i < H; ++i) c = fma(!TRANS ? t.mid[i] : t.Pm[i], xm[i], c);
+      for (int i = 1; i < H; ++i) c = vfma(!TRANS ? t.mid[i] : t.Pm[i], xm[i], c);
       m = c;
     } else {
-      double c = (HALF ? t.midmh : t.midm) * xc;
+      T c = vmul(HALF ? t.midmh : t.midm, xc);
 #pragma unroll
-      for (int i = 0; i < H; ++i) c = fma(!TRANS ? t.mid[i] : t.Pm[i], xp[i], c);
+      for (int i = 0; i < H; ++i) c = vfma(!TRANS ? t.mid[i] : t.Pm[i], xp[i], c);
       m = c;
     }
   }
 }
 
-template <int N, bool ANTI>
-__device__ __forceinline__ void eo_combine(const double (&u)[N / 2 > 0 ? N / 2 : 1], const double (&v)[N / 2 > 0 ? N / 2 : 1],
-                                           double m, double (&y)[N]) {
+template <int N, bool ANTI, typename T>
+__device__ __forceinline__ void eo_combine(const T (&u)[N / 2 > 0 ? N / 2 : 1], const T (&v)[N / 2 > 0 ? N / 2 : 1], T m, T (&y)[N]) {
 #pragma unroll
   for (int q = 0; q < N / 2; ++q) { y[q] = u[q] + v[q]; y[N - 1 - q] = ANTI ? (v[q] - u[q]) : (u[q] - v[q]); }
   if (N & 1) y[N / 2] = m;
 }
 
 // y = M x or M^T x, complete (split, mult, combine); x and y may be the same array.
-template <int PDEG, int MAT, bool TRANS>
-__device__ __forceinline__ void eo_full(const double (&x)[PDEG + 1], double (&y)[PDEG + 1]) {
+template <int PDEG, int MAT, bool TRANS, typename T>
+__device__ __forceinline__ void eo_full(const T (&x)[PDEG + 1], T (&y)[PDEG + 1]) {
   constexpr int N = PDEG + 1, HH = N / 2 > 0 ? N / 2 : 1;
-  double xp[HH], xm[HH], u[HH], v[HH], m;
+  T xp[HH], xm[HH], u[HH], v[HH], m;
   eo_split<N>(x, xp, xm);
   eo_mult<PDEG, MAT, TRANS, false>(xp, xm, x[N / 2], u, v, m);
   eo_combine<N, MAT == MAT_DS>(u, v, m, y);
 }
 
 // (u2, v2, m2) = HALF of the even/odd parts of Ds^T Ds t, from the line t.
-template <int PDEG>
-__device__ __forceinline__ void eo_dtd(const double (&t)[PDEG + 1], double (&u2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
-                                       double (&v2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], double& m2) {
+template <int PDEG, typename T>
+__device__ __forceinline__ void eo_dtd(const T (&t)[PDEG + 1], T (&u2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                       T (&v2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], T& m2) {
   constexpr int N = PDEG + 1, HH = N / 2 > 0 ? N / 2 : 1;
-  double tp[HH], tm[HH], u1[HH], v1[HH], m1;
+  T tp[HH], tm[HH], u1[HH], v1[HH], m1;
   eo_split<N>(t, tp, tm);
   eo_mult<PDEG, MAT_DS, false, false>(tp, tm, t[N / 2], u1, v1, m1);
   eo_mult<PDEG, MAT_DS, true, true>(v1, u1, m1, u2, v2, m2);

@@ -14,6 +14,7 @@
 #include "fe_kernels_tma.cuh"
 #include "fe_kernels_gen.cuh"
 #include "fe_kernels_plane.cuh"
+#include "fe_kernels_line.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {

@@ -218,7 +218,7 @@ def test_unit_cube_config5_interval_is_rejected(env):
         op.cheb_filter(X, Y, 1, 20, 2.0, 0.3, 0.0)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 4, 5, 6, 8, 9])
+@pytest.mark.parametrize("variant", [1, 2, 4, 5, 6, 8, 9, 10, 11])
 @pytest.mark.parametrize("p,bc", [(6, inputs.BC_DIRICHLET), (7, inputs.BC_PERIODIC), (8, inputs.BC_PERIODIC), (4, inputs.BC_PERIODIC)])
 def test_kernel_variants(env, variant, p, bc):
     """variant 1 = general kernel, 2 = even-odd Cartesian kernel with one vector per thread, 4 = two vectors per thread with LDG/RED (default 0: persistent TMA kernel)."""
