@@ -215,36 +215,62 @@ cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUt
   const long long nitems = c->ncells * prm.nvb;
   long long grid = (long long)blocks_per_sm * c->nsm;
   if (grid > nitems) grid = nitems;
+  cudaError_t e0 = cudaMemsetAsync(c->ctrl, 0, 16, st);   // work counter
+  if (e0 != cudaSuccess) return e0;
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
 }
 
 // ---- plane kernel (one thread = one n x n plane of one vector), uniform Cartesian cells
 template <int PDEG> struct PlaneCfg;
-template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 2, NH = 1; };
-template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1, NH = 1; };
-template <> struct PlaneCfg<106> { static constexpr int BV = 16, NT = 256, MINB = 1, NH = 2; };   // two groups in lockstep
+template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 2; };
+template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };
 bool plane_ok(int p) { return p == 6 || p == 7; }
 
-template <int PDEG, int CFG = PDEG>
-cudaError_t launch_plane(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
-                         cudaStream_t st) {
-  using C = PlaneCfg<CFG>;
-  constexpr size_t SMEM = (size_t)2 * C::NH * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
-  static int blocks_per_sm = 0;
-  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, C::NH>;
+// Launch of a persistent TMA kernel `kern(tw, tz, prm, init, nitems)`: plain when the kernel only accumulates,
+// cooperative (all blocks co-resident) when it also initialises Z ahead of itself (fe_init_ahead.cuh).  The
+// per-context counters advance by `grid` per fused launch.
+template <typename Kern>
+cudaError_t launch_persistent(fe_mf_ctx* c, Kern kern, int nt, size_t smem, int& blocks_per_sm, const fe::ApplyParams& prm,
+                              fe::InitParams init, const CUtensorMap& tw, const CUtensorMap& tz, cudaStream_t st) {
   if (blocks_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, nt, smem);
     if (e != cudaSuccess) return e;
     if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
   }
-  const long long nitems = c->ncells * prm.nvb;
+  const long long nitems_ll = c->ncells * prm.nvb;
   long long grid = (long long)blocks_per_sm * c->nsm;
-  if (grid > (nitems + C::NH - 1) / C::NH) grid = (nitems + C::NH - 1) / C::NH;
-  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
-  return cudaGetLastError();
+  if (grid > nitems_ll) grid = nitems_ll;
+  int nitems = (int)nitems_ll;
+  {
+    cudaError_t e = cudaMemsetAsync(c->ctrl, 0, init.mode == fe::INIT_NONE ? 16 : c->ctrl_bytes, st);
+    if (e != cudaSuccess) return e;
+  }
+  if (init.mode == fe::INIT_NONE && c->variant != 17) {
+    kern<<<(unsigned)grid, nt, smem, st>>>(tw, tz, prm, init, nitems);
+    return cudaGetLastError();
+  }
+  if (init.mode == fe::INIT_NONE) {   // timing experiment: the accumulate-only kernel, launched cooperatively
+    void* args0[] = {(void*)&tw, (void*)&tz, (void*)&prm, (void*)&init, (void*)&nitems};
+    return cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3(nt), args0, smem, st);
+  }
+  init.slice_ctr = c->ctrl + 4;
+  init.done = c->ctrl + 4 + c->ncz;
+  void* args[] = {(void*)&tw, (void*)&tz, (void*)&prm, (void*)&init, (void*)&nitems};
+  return cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3(nt), args, smem, st);
+}
+
+template <int PDEG, int CFG = PDEG>
+cudaError_t launch_plane(fe_mf_ctx* c, const fe::ApplyParams& prm, const fe::InitParams& init, const CUtensorMap& tw,
+                         const CUtensorMap& tz, cudaStream_t st) {
+  using C = PlaneCfg<CFG>;
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  static int bps[3] = {0, 0, 0};
+  if (init.mode == fe::INIT_NONE) return launch_persistent(c, fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, 0>, C::NT, SMEM, bps[0], prm, init, tw, tz, st);
+  if (init.mode == fe::INIT_ZERO) return launch_persistent(c, fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, 1>, C::NT, SMEM, bps[1], prm, init, tw, tz, st);
+  return launch_persistent(c, fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, 2>, C::NT, SMEM, bps[2], prm, init, tw, tz, st);
 }
 
 // ---- second-generation line kernel (two vectors per thread, fused even/odd chains)
@@ -271,6 +297,8 @@ cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CU
   const long long nitems = c->ncells * prm.nvb;
   long long grid = (long long)blocks_per_sm * c->nsm;
   if (grid > nitems) grid = nitems;
+  cudaError_t e0 = cudaMemsetAsync(c->ctrl, 0, 16, st);   // work counter
+  if (e0 != cudaSuccess) return e0;
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
 }
@@ -300,7 +328,7 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   // plane kernel: one plane of ONE vector per thread, 16 vectors per block; worth it when the last block is mostly full
   const int tail = nvec % 16;
   if (plane_ok(c->p) && c->p == 6 && nvec >= 12 && (tail == 0 || tail >= 12)) return 8;
-  if ((c->variant == 8 || c->variant == 9) && plane_ok(c->p)) return 8;
+  if ((c->variant == 8 || c->variant >= 14) && plane_ok(c->p)) return 8;
   return 9;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
@@ -321,11 +349,21 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.geom_mode = c->geom_mode;
   P.nsm = c->nsm;
   P.geom_stride = c->geom_stride;
+  P.item_ctr = reinterpret_cast<int*>(c->ctrl);
   return P;
 }
 
-// Z += alpha * A * W  (Z already initialised).  Counts launches into c->last_launches.
-int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st) {
+// Can this kernel kind initialise Z itself (cooperative launch available)?
+bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
+  const long long chunk2 = (long long)(c->p + 1) * c->ndx * c->ndy * nvec / 2;   // double2 elements of the largest chunk
+  return kind == 8 && c->coop && (c->variant == 15 || c->variant == 16 || c->variant == 18 || c->variant == 19) && chunk2 < (1LL << 31) &&
+         c->ncells * ((nvec + 15) / 16) < (1LL << 31);
+}
+
+// Z += alpha * A * W  (Z already initialised), or with init.mode != INIT_NONE (only if kind_fuses_init):
+// Z <- beta Z + gamma W + alpha A W in ONE launch.  Counts launches into c->last_launches.
+int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st,
+                      fe::InitParams init = fe::InitParams{fe::INIT_NONE, 0, 0.0, 0.0, nullptr, nullptr}) {
   const int kind = pick_kernel(c, nvec, W, Z);
   const int bv = kernel_bv(c, kind, nvec);
   fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
@@ -353,8 +391,8 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
     if (!make_tensor_map(&tw, c, W, nvec, bv, dir ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, dir ? 1 : 0))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
     switch (c->p) {
-      case 6: e = (c->variant == 9) ? launch_plane<6, 106>(c, P, tw, tz, st) : launch_plane<6>(c, P, tw, tz, st); break;
-      case 7: e = launch_plane<7>(c, P, tw, tz, st); break;
+      case 6: e = launch_plane<6>(c, P, init, tw, tz, st); break;
+      case 7: e = launch_plane<7>(c, P, init, tw, tz, st); break;
     }
   } else if (kind == 9) {
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
@@ -459,6 +497,11 @@ extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_d
   cudaStream_t st = (cudaStream_t)cuda_stream;
   ctx->last_launches = 0;
   const size_t count = (size_t)ctx->ndof * nvec;
+  const int kind = pick_kernel(ctx, nvec, W_dev, Z_dev);
+  if (kind_fuses_init(ctx, kind, nvec)) {   // S1 folded into the apply kernel (fe_init_ahead.cuh): one launch
+    fe::InitParams init{beta == 0.0 ? (gamma == 0.0 ? fe::INIT_ZERO : fe::INIT_SCALE) : fe::INIT_AXPBY, ctx->variant == 15 ? 1 : (ctx->variant == 16 ? 2 : (ctx->variant == 18 ? 4 : 0)), beta, gamma, nullptr, nullptr};
+    return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st, init);
+  }
   rc = launch_init(ctx, Z_dev, W_dev, beta, gamma, count, st);
   if (rc) return rc;
   return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st);
@@ -582,11 +625,16 @@ extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
   return kernel_bv(ctx, kind, nvec);
 }
 
+extern "C" int fe_mf_debug_ctrl(fe_mf_ctx* ctx, unsigned* out4) {   // diagnostics: the first control words after a launch
+  if (!ctx || !out4) return FE_MF_EINVAL;
+  return cudaMemcpy(out4, ctx->ctrl, 16, cudaMemcpyDeviceToHost) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
+}
+
 extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx->last_launches : -1; }
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 13) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  if ((variant < 0 || variant > 19) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

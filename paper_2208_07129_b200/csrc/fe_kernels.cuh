@@ -30,6 +30,7 @@ struct ApplyParams {
   int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
   int nsm;                        // SM count (persistent kernels)
   long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
+  int* item_ctr;                  // persistent kernels: work counter (0 at launch); item = gridDim.x + atomicAdd after the first
 };
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.

@@ -38,6 +38,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
   double* GS = reinterpret_cast<double*>(smem_raw + 3 * TL::PITCH);
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 3 * TL::PITCH + GBYTES);
   uint64_t* gbar = bar + 1;
+  int* s_next = reinterpret_cast<int*>(bar + 2);
   const bool perq = (P.geom_mode == 2);
   const int tid = threadIdx.x;
   const long long nvec = P.nvec;
@@ -64,7 +65,10 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
   }
   uint32_t parity = 0, gparity = 0;
   int rot = (blockIdx.x / P.nsm) & 3;
-  for (; item < nitems; item += gridDim.x, rot = (rot + 1) & 3) {
+  // items are handed out dynamically after the first one (co-resident blocks do not run at the same speed)
+  for (; item < nitems; rot = (rot + 1) & 3) {
+    unsigned nxt_raw = 0;
+    if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
     const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
@@ -191,8 +195,9 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     }
     __syncthreads();
     // the staged geometry is consumed: fetch the next item's
+    if (tid == 0) *s_next = (int)(gridDim.x + nxt_raw);
     if (tid == 0 && perq) {
-      const int nxt = item + gridDim.x;
+      const int nxt = (int)(gridDim.x + nxt_raw);
       if (nxt < nitems) {
         mbar_expect_tx(gbar, GBYTES);
         bulk_load(GS, P.geom + (size_t)(nxt / P.nvb) * P.geom_stride, GBYTES, gbar);
@@ -213,7 +218,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     __syncthreads();
     // tile B is free: prefetch the next item's tile into it (it becomes tile A of the next item)
     if (tid == 0) {
-      const int nxt = item + gridDim.x;
+      const int nxt = (int)(gridDim.x + nxt_raw);
       if (nxt < nitems) {
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
@@ -290,6 +295,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       tma_commit();
     }
     { double* t_ = A; A = B; B = C; C = t_; }   // (A,B,C) <- (B,C,A)
+    item = *s_next;   // written during ph5, several barriers ago
   }
   if (tid == 0) tma_wait_all0();
 }

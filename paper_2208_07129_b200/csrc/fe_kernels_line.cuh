@@ -25,6 +25,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
   double* A = reinterpret_cast<double*>(smem_raw);
   double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TL::PITCH);
+  int* s_next = reinterpret_cast<int*>(bar + 1);
   const int tid = threadIdx.x;
   const bool dirichlet = P.dirichlet != 0;
   const int org = dirichlet ? -1 : 0;   // see fe_apply_cart_plane: interior input map on Dirichlet meshes
@@ -44,7 +45,10 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
   }
   uint32_t parity = 0;
   int rot = (blockIdx.x / P.nsm) & 3;
-  for (; item < nitems; item += gridDim.x, rot = (rot + 1) & 3) {
+  // items are handed out dynamically after the first one (co-resident blocks do not run at the same speed)
+  for (; item < nitems; rot = (rot + 1) & 3) {
+    unsigned nxt_raw = 0;
+    if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
     const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
@@ -138,7 +142,8 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     __syncthreads();
     // tile A is free: prefetch the next item's tile (overlaps ph5-ph6)
     if (tid == 0) {
-      const int nxt = item + gridDim.x;
+      const int nxt = (int)(gridDim.x + nxt_raw);
+      *s_next = nxt;
       if (nxt < nitems) {
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
@@ -180,6 +185,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
       tma_commit();
     }
+    item = *s_next;   // written before the barrier that ended ph6
   }
   if (tid == 0) tma_wait_all0();
 }

@@ -23,6 +23,7 @@
 // middle-column tables (HALF) and by the scalar of the final accumulate.
 #pragma once
 #include "fe_kernels_tma.cuh"
+#include "fe_init_ahead.cuh"
 
 #ifndef FE_ZLOOP_PRAGMA   // the z-line loops of P2 / P4: rolled (small code) or unrolled (loads hoisted)
 #define FE_ZLOOP_PRAGMA _Pragma("unroll 1")
@@ -153,25 +154,23 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
   }
 }
 
-// Z += A W on uniform Cartesian cells (diagonal constant metric; alpha folded into P.ug).  One block = one
-// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta.  A block holds NH groups of
-// GT = NT/NH threads; each group works on its own item with its own tiles, and the groups share the block
-// barriers, so that the warps of one SM sub-partition walk through the (long, straight-line) code together and
-// share its instruction-cache lines.
-template <int PDEG, int BV, int NT, int MINB, int NH>
+// Z (+)= A W on uniform Cartesian cells (diagonal constant metric; alpha folded into P.ug).  One block = one
+// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta.  With I.mode != INIT_NONE the
+// kernel also initialises Z (fe_init_ahead.cuh) and must be launched cooperatively.
+template <int PDEG, int BV, int NT, int MINB, int IM>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
-                    const __grid_constant__ ApplyParams P, int nitems) {
+                    const __grid_constant__ ApplyParams P, const __grid_constant__ InitParams I, int nitems) {
   using TL = DenseTile<PDEG, BV>;
   constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1;
   constexpr int S1 = BV, S2 = N * BV, S3 = N * N * BV;   // element strides along x, y, z
-  constexpr int GT = NT / NH;
-  static_assert(N * BV <= GT && GT % 128 == 0, "one plane task per thread; whole warps on every sub-partition");
+  static_assert(N * BV <= NT && NT % 128 == 0, "one plane task per thread; whole warps on every sub-partition");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  const int grp = threadIdx.x / GT, tid = threadIdx.x % GT;
-  double* A = reinterpret_cast<double*>(smem_raw + (2 * grp) * TL::PITCH);
-  double* B = reinterpret_cast<double*>(smem_raw + (2 * grp + 1) * TL::PITCH);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * NH * TL::PITCH) + grp;
+  double* A = reinterpret_cast<double*>(smem_raw);
+  double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * TL::PITCH);
+  int* s_next = reinterpret_cast<int*>(bar + 1);
+  const int tid = threadIdx.x;
   const int beta = tid % BV, k = tid / BV;
   const bool active = k < N;
   // Dirichlet: the input tensor map covers the INTERIOR nodes only (origin = node (1,1,1)), so boundary nodes are
@@ -181,14 +180,17 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   const bool dirichlet = P.dirichlet != 0;
   const int org = dirichlet ? -1 : 0;
   const double g2x = 2.0 * P.ug[0], g2y = 2.0 * P.ug[3], g4y = 4.0 * P.ug[3], g4z = 4.0 * P.ug[5], gm = P.ug[6];
+  constexpr bool init = (IM != 0);
+  constexpr int LOOK = 3;   // the items of layer L initialise chunk L+LOOK; layer L adds into chunks L and L+1
+  const int layer_items = P.ncx * P.ncy * P.nvb;
+  InitAhead<NT, IM> ia(I, P, PDEG, tid, layer_items);
 
   if (tid == 0) {
     mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  const int stride = gridDim.x * NH;
-  int item = blockIdx.x * NH + grp;
+  int item = blockIdx.x;
   if (tid == 0 && item < nitems) {
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
@@ -196,25 +198,33 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + org);
   }
   uint32_t parity = 0;
-  for (int base = blockIdx.x * NH; base < nitems; base += stride, item += stride) {
-    const bool valid = item < nitems;   // a group without an item still joins the block barriers
+  ia.startup(LOOK);
+  if (init && tid == 0) { s_next[1] = 0; s_next[2] = 1 << 30; }   // nothing reserved for the first item
+  // Items are handed out dynamically (the first one is blockIdx.x): co-resident blocks do not run at the same
+  // speed (the warp arbiter favours one of them), and a static round-robin would leave the slow ones behind.
+  while (item < nitems) {
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
-    const bool special = valid && (wx || wy || wz);
+    const bool special = wx || wy || wz;
     const bool dlow = dirichlet && (ex == 0 || ey == 0 || ez == 0);
-    const bool work = active && valid;
-    if (valid) mbar_wait(bar, parity);
+    // the next item and (init-ahead) this item's slices of chunk ez+LOOK: both consumed later, latency hidden
+    // (asm volatile: the compiler must not schedule anything that depends on the results up here)
+    unsigned nxt_raw = 0, sl0 = 0;
+    if (tid == 0) {
+      asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
+      if (init) sl0 = ia.grab(ez + LOOK);
+    }
+    mbar_wait(bar, parity);
     parity ^= 1u;
     if (special) {
-      plane_wrap_fixup<PDEG, BV, GT, false>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
-      if (NH == 1) __syncthreads();
-      else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "n"(GT) : "memory");
+      plane_wrap_fixup<PDEG, BV, NT, false>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
+      __syncthreads();
     }
 
     // P1: xy-plane i3 = k: Ns along x (rows) then along y (columns), in registers
-    if (work) {
+    if (active) {
       double* a = A + k * S3 + beta;
       double r[N][N];
 #pragma unroll
@@ -233,11 +243,16 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
         for (int j = 0; j < N; ++j) a[j * S2 + i * S1] = c[j];
       }
     }
-    if (tid == 0) tma_wait_read0();   // the previous item's reduction has finished reading tile B
+    if (tid == 0) {
+      tma_wait_read0();   // the previous item's reduction has finished reading tile B
+    }
     __syncthreads();
 
     // P2: z-lines (i1, i2 = k): T = Ns_z A -> A ; R = gm T + 4 gzz (DtD T)/4 -> B
-    if (work) {
+    // (init-ahead: the zero stores, or the loads of a first batch, are issued here and fly during P2)
+    // (the slices were reserved during the block's PREVIOUS item, so that the atomic's latency is never waited for)
+    if (init) { ia.accept(s_next[2], (unsigned)s_next[1]); ia.batch_begin(); }
+    if (active) {
       double xn[N];   // software pipeline: the next line is in flight while this one is computed
 #pragma unroll
       for (int j = 0; j < N; ++j) xn[j] = A[k * S2 + beta + j * S3];
@@ -267,10 +282,11 @@ FE_ZLOOP_PRAGMA
         if (N & 1) b[H * S3] = fma(g4z, m2, gm * tq[H]);
       }
     }
+    if (init) ia.batch_end();
     __syncthreads();
 
     // P3: xy-plane i3 = k: R += Kx T (rows) ; R += Ky T, Ns^T along y (columns) ; Ns^T along x (rows)
-    if (work) {
+    if (active) {
       const double* a = A + k * S3 + beta;
       double* b = B + k * S3 + beta;
       double r[N][N];
@@ -316,7 +332,9 @@ FE_ZLOOP_PRAGMA
     __syncthreads();
     // tile A is free: prefetch the next item's tile (overlaps P4 and the other resident block)
     if (tid == 0) {
-      const int nxt = item + stride;
+      const int nxt = (int)(gridDim.x + nxt_raw);
+      *s_next = nxt;
+      if (init) { s_next[1] = (int)sl0; s_next[2] = ez + LOOK; }
       if (nxt < nitems) {
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
@@ -325,7 +343,8 @@ FE_ZLOOP_PRAGMA
       }
     }
     // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
-    if (work) {
+    if (init) ia.batch_begin();
+    if (active) {
       double xn[N];
 #pragma unroll
       for (int j = 0; j < N; ++j) xn[j] = B[k * S2 + beta + j * S3];
@@ -350,14 +369,26 @@ FE_ZLOOP_PRAGMA
         for (int j = 0; j < N; ++j) b[j * S3] = x[j];
       }
     }
+    if (init) {
+      ia.batch_end();
+      ia.drain();
+      ia.wait_ready(ez + 1);   // the planes this cell adds into are initialised
+    }
     fence_async_smem();
     __syncthreads();
-    if (special) plane_wrap_fixup<PDEG, BV, GT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
-    if (tid == 0 && valid) {
+    ia.publish_point();
+    if (special) plane_wrap_fixup<PDEG, BV, NT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
+    if (tid == 0) {
       tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
       tma_commit();
     }
+    item = *s_next;   // written before the barrier that ended P4
   }
+  if (init) {   // the slices reserved during the last item
+    ia.accept(s_next[2], (unsigned)s_next[1]);
+    ia.batch_begin(); ia.batch_end(); ia.drain();
+  }
+  ia.finish();
   if (tid == 0) tma_wait_all0();
 }
 

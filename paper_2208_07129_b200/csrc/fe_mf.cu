@@ -28,6 +28,11 @@ struct fe_mf_ctx {
   double ug[7];
   double* geom_dev = nullptr;
   long long geom_stride = 7;   // doubles per cell in geom_dev
+  // control words of the persistent kernels, zeroed on the stream before each launch:
+  // [0] item counter, [4 .. 4+ncz) slice_ctr, [4+ncz .. 4+2 ncz) done  (fe_init_ahead.cuh)
+  unsigned* ctrl = nullptr;
+  size_t ctrl_bytes = 0;
+  bool coop = false;           // cooperative launches supported
   int variant = 0;
   int last_launches = 0;
   // fe_mf_apply_host workspace
@@ -218,6 +223,9 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
     e = cudaMemcpy(c->geom_dev, G.data(), G.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(c->geom_dev); delete c; return fail(nullptr, FE_MF_ECUDA, std::string("geometry upload: ") + cudaGetErrorString(e)); }
   }
+  c->coop = prop.cooperativeLaunch != 0;
+  c->ctrl_bytes = sizeof(unsigned) * (4 + 2 * (size_t)ncz);
+  if (cudaMalloc(&c->ctrl, c->ctrl_bytes) != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ENOMEM, "cudaMalloc (control words) failed"); }
   *out = c;
   return FE_MF_OK;
 }
@@ -230,6 +238,7 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
   if (!ctx) return;
   DeviceGuard guard(ctx->device);
   if (ctx->geom_dev) cudaFree(ctx->geom_dev);
+  if (ctx->ctrl) cudaFree(ctx->ctrl);
   if (ctx->ws_x) cudaFree(ctx->ws_x);
   if (ctx->ws_y) cudaFree(ctx->ws_y);
   for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
