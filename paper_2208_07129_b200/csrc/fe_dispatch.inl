@@ -305,6 +305,7 @@ cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CU
 // vectors per block of the line kernel for (p, variant)
 int line_bv(const fe_mf_ctx* c, int nvec) {
   if (c->variant == 11 || c->variant == 12 || nvec <= 8) return 8;
+  if (c->p == 7 && c->variant != 10 && c->variant != 13) return 8;   // p = 7: three 8-vector blocks per SM beat one 16-vector block
   return tma_bv(c->p);
 }
 
