@@ -1,10 +1,20 @@
 // Included by fe_mf.cu: kernel selection and the stream-ordered entry points.
+//
+// Kernels:
+//   kind 8  fe_apply_cart_plane  uniform Cartesian cells, p = 6: one n x n plane of one vector per thread
+//   kind 9  fe_apply_cart_line   uniform Cartesian cells, any p: one line of two vectors per thread
+//   kind 6  fe_apply_gen_tma     full symmetric metric (per-q-point or per-cell geometry)
+//   kind 2  fe_apply_cart        Cartesian, odd nvec or unaligned pointers (LDG gather / RED scatter)
+//   kind 1  fe_apply_general     anything else (nvec = 1, odd nvec with a full metric): plain contractions
+// fe_mf_set_variant forces a kind for tests and experiments: 1 -> kind 1, 2 -> kind 2, 7 -> kind 6 on a Cartesian
+// mesh, 8 -> plane, 10 -> line with 16-vector blocks, 11 -> line with 8-vector blocks, 19 -> plane kernel that
+// also initialises Z (fe_init_ahead.cuh; measured neutral, off by default).
 
 namespace {
 
 constexpr size_t kMaxSmem = 232448;  // 227 KB opt-in per block on sm_100
 
-// General kernel: 4 tiles of n^3*bv doubles.  Keep >= 2 blocks per SM resident.
+// ---- kind 1: general fallback, 4 tiles of n^3*bv doubles; keep >= 2 blocks per SM resident
 int general_bv(int p, int nvec) {
   const int nn = (p + 1) * (p + 1) * (p + 1);
   int bv = 32;
@@ -22,15 +32,14 @@ cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStr
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  const long long grid = ncells * prm.nvb;
-  fe::fe_apply_general<PDEG><<<(unsigned)grid, 256, smem, st>>>(prm);
+  fe::fe_apply_general<PDEG><<<(unsigned)(ncells * prm.nvb), 256, smem, st>>>(prm);
   return cudaGetLastError();
 }
 
-// ---- optimised Cartesian kernel (variant 0 on uniform meshes): launch geometry per degree
-template <int PDEG, int BV>
+// ---- kind 2: even-odd Cartesian kernel, one vector per thread, 8 vectors per block
+template <int PDEG>
 struct CartCfg {
-  static constexpr int N = PDEG + 1;
+  static constexpr int BV = 8, N = PDEG + 1;
   static constexpr int TASKS = N * N * BV;
   static constexpr int NT = (PDEG >= 5) ? TASKS / 2 : (TASKS < 32 ? 32 : TASKS);
   static constexpr size_t SMEM = (size_t)2 * fe::Tile<PDEG, BV>::SIZE * sizeof(double);
@@ -40,11 +49,11 @@ struct CartCfg {
   static constexpr int MINB = MINB0 > 4 ? 4 : (MINB0 < 1 ? 1 : MINB0);
 };
 
-template <int PDEG, int BV>
+template <int PDEG>
 cudaError_t launch_cart(const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
-  using C = CartCfg<PDEG, BV>;
+  using C = CartCfg<PDEG>;
   static bool configured = false;
-  auto kern = fe::fe_apply_cart<PDEG, BV, C::NT, C::MINB>;
+  auto kern = fe::fe_apply_cart<PDEG, C::BV, C::NT, C::MINB>;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
@@ -54,50 +63,7 @@ cudaError_t launch_cart(const fe::ApplyParams& prm, long long ncells, cudaStream
   return cudaGetLastError();
 }
 
-template <int BV>
-cudaError_t launch_cart_p(int p, const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
-  switch (p) {
-    case 1: return launch_cart<1, BV>(prm, ncells, st);
-    case 2: return launch_cart<2, BV>(prm, ncells, st);
-    case 3: return launch_cart<3, BV>(prm, ncells, st);
-    case 4: return launch_cart<4, BV>(prm, ncells, st);
-    case 5: return launch_cart<5, BV>(prm, ncells, st);
-    case 6: return launch_cart<6, BV>(prm, ncells, st);
-    case 7: return launch_cart<7, BV>(prm, ncells, st);
-    case 8: return launch_cart<8, BV>(prm, ncells, st);
-  }
-  return cudaErrorInvalidValue;
-}
-
-// ---- production Cartesian kernel (two vectors per thread)
-template <int PDEG> struct Cart2Cfg;
-template <> struct Cart2Cfg<1> { static constexpr int BV = 16, NT = 32, MINB = 4; };
-template <> struct Cart2Cfg<2> { static constexpr int BV = 16, NT = 96, MINB = 4; };
-template <> struct Cart2Cfg<3> { static constexpr int BV = 16, NT = 128, MINB = 4; };
-template <> struct Cart2Cfg<4> { static constexpr int BV = 16, NT = 112, MINB = 4; };
-template <> struct Cart2Cfg<5> { static constexpr int BV = 16, NT = 160, MINB = 3; };
-template <> struct Cart2Cfg<6> { static constexpr int BV = 16, NT = 224, MINB = 2; };
-template <> struct Cart2Cfg<7> { static constexpr int BV = 8, NT = 128, MINB = 3; };
-template <> struct Cart2Cfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
-
-template <int PDEG>
-cudaError_t launch_cart2(const fe::ApplyParams& prm, long long ncells, cudaStream_t st) {
-  using C = Cart2Cfg<PDEG>;
-  constexpr size_t SMEM = (size_t)2 * fe::Tile<PDEG, C::BV>::SIZE * sizeof(double);
-  static bool configured = false;
-  auto kern = fe::fe_apply_cart2<PDEG, C::BV, C::NT, C::MINB>;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  kern<<<(unsigned)(ncells * prm.nvb), C::NT, SMEM, st>>>(prm);
-  return cudaGetLastError();
-}
-
-int cart2_bv(int p) { return p >= 7 ? 8 : 16; }
-
-// ---- persistent TMA kernel
+// ---- tensor maps
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -117,19 +83,17 @@ EncodeTiledFn encode_tiled_fn() {
 }
 
 // 4-D FP64 tensor map of a multivector [z][y][x][beta] with box (bv, n, n, n).
-// Dirichlet meshes, plane kernels: trim = 2 -> the map covers nodes 1 .. nd-2 in every direction, origin at node
-// (1,1,1), so that boundary nodes are out of bounds (zero on load; box coordinates shift by -1); trim = 1 -> nodes
-// 0 .. nd-2, origin unchanged (the last node is clipped on reduce).
+// Dirichlet meshes (Cartesian kernels): trim = 2 -> the map covers nodes 1 .. nd-2 in every direction, origin at
+// node (1,1,1), so that boundary nodes are out of bounds (zero on load; box coordinates shift by -1); trim = 1 ->
+// nodes 0 .. nd-2, origin unchanged (the last node is clipped on reduce).
 bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim = 0) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
-  const int cut = trim;
-  const bool interior = (trim == 2);
   if (trim && (c->ndx < 3 || c->ndy < 3 || c->ndz < 3)) return false;
-  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)(c->ndx - cut), (cuuint64_t)(c->ndy - cut), (cuuint64_t)(c->ndz - cut)};
+  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)(c->ndx - trim), (cuuint64_t)(c->ndy - trim), (cuuint64_t)(c->ndz - trim)};
   const cuuint64_t strides[3] = {(cuuint64_t)nvec * 8, (cuuint64_t)nvec * 8 * c->ndx, (cuuint64_t)nvec * 8 * c->ndx * c->ndy};
   if (strides[2] >= ((cuuint64_t)1 << 40)) return false;
-  if (interior) base = (const char*)base + (strides[0] + strides[1] + strides[2]);
+  if (trim == 2) base = (const char*)base + (strides[0] + strides[1] + strides[2]);
   const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)c->n, (cuuint32_t)c->n, (cuuint32_t)c->n};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
@@ -137,55 +101,23 @@ bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int 
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int PDEG> struct TmaCfg;
-template <> struct TmaCfg<1> { static constexpr int BV = 16, NT = 32, MINB = 4; };
-template <> struct TmaCfg<2> { static constexpr int BV = 16, NT = 96, MINB = 4; };
-template <> struct TmaCfg<3> { static constexpr int BV = 16, NT = 128, MINB = 4; };
-template <> struct TmaCfg<4> { static constexpr int BV = 16, NT = 112, MINB = 4; };
-template <> struct TmaCfg<5> { static constexpr int BV = 16, NT = 160, MINB = 3; };
-template <> struct TmaCfg<6> { static constexpr int BV = 16, NT = 256, MINB = 2; };
-template <> struct TmaCfg<7> { static constexpr int BV = 16, NT = 256, MINB = 1; };
-template <> struct TmaCfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
-int tma_bv(int p) { return p == 8 ? 8 : 16; }
-
-template <> struct TmaCfg<101> { static constexpr int BV = 8, NT = 32, MINB = 4; };
-template <> struct TmaCfg<102> { static constexpr int BV = 8, NT = 64, MINB = 4; };
-template <> struct TmaCfg<103> { static constexpr int BV = 8, NT = 64, MINB = 4; };
-template <> struct TmaCfg<104> { static constexpr int BV = 8, NT = 128, MINB = 4; };
-template <> struct TmaCfg<105> { static constexpr int BV = 8, NT = 160, MINB = 4; };
-template <> struct TmaCfg<106> { static constexpr int BV = 8, NT = 128, MINB = 5; };   // alt p=6
-template <> struct TmaCfg<107> { static constexpr int BV = 8, NT = 128, MINB = 3; };   // alt p=7
-template <> struct TmaCfg<108> { static constexpr int BV = 8, NT = 352, MINB = 1; };   // alt p=8
-// 8 vectors per block when the call has at most 8 vectors (or on request): no lanes wasted on the vector tail
-bool tma_use_bv8(const fe_mf_ctx* c, int nvec) { return c->variant == 5 || nvec <= 8; }
-
-template <int PDEG, int CFG = PDEG, bool TMA_OUT = true, int DBG = 0>
-cudaError_t launch_tma(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
-                       cudaStream_t st) {
-  using C = TmaCfg<CFG>;
-  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
-  static int blocks_per_sm = 0;
-  static int nsm = 0;
-  auto kern = fe::fe_apply_cart_tma<PDEG, C::BV, C::NT, C::MINB, TMA_OUT, DBG>;
+// ---- persistent kernels: grid = resident blocks; the work counter is zeroed on the stream before each launch
+template <typename Kern>
+cudaError_t persistent_grid(Kern kern, int nt, size_t smem, int& blocks_per_sm, const fe_mf_ctx* c, long long nitems,
+                            long long& grid) {
   if (blocks_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, nt, smem);
     if (e != cudaSuccess) return e;
     if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
-    cudaDeviceProp prop;
-    e = cudaGetDeviceProperties(&prop, c->device);
-    if (e != cudaSuccess) return e;
-    nsm = prop.multiProcessorCount;
   }
-  const long long nitems = c->ncells * prm.nvb;
-  long long grid = (long long)blocks_per_sm * nsm;
+  grid = (long long)blocks_per_sm * c->nsm;
   if (grid > nitems) grid = nitems;
-  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
-  return cudaGetLastError();
+  return cudaSuccess;
 }
 
-// ---- persistent TMA kernel for a full symmetric metric (per-q-point / per-cell geometry)
+// ---- kind 6: full symmetric metric
 template <int PDEG> struct GenCfg;
 template <> struct GenCfg<1> { static constexpr int BV = 8, NT = 32, MINB = 4; };
 template <> struct GenCfg<2> { static constexpr int BV = 8, NT = 64, MINB = 4; };
@@ -195,7 +127,7 @@ template <> struct GenCfg<5> { static constexpr int BV = 8, NT = 160, MINB = 2; 
 template <> struct GenCfg<6> { static constexpr int BV = 8, NT = 128, MINB = 3; };
 template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 256, MINB = 1; };
 template <> struct GenCfg<8> { static constexpr int BV = 8, NT = 384, MINB = 1; };
-int gen_bv(int p) { (void)p; return 8; }
+constexpr int kGenBv = 8;
 
 template <int PDEG>
 cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
@@ -203,139 +135,122 @@ cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUt
   using C = GenCfg<PDEG>;
   constexpr int NN = (PDEG + 1) * (PDEG + 1) * (PDEG + 1);
   constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, C::BV>::PITCH + ((size_t)7 * NN * 8 + 15) / 16 * 16 + 64;
-  static int blocks_per_sm = 0;
+  static int bps = 0;
   auto kern = fe::fe_apply_gen_tma<PDEG, C::BV, C::NT, C::MINB>;
-  if (blocks_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
-    if (e != cudaSuccess) return e;
-    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
-  }
   const long long nitems = c->ncells * prm.nvb;
-  long long grid = (long long)blocks_per_sm * c->nsm;
-  if (grid > nitems) grid = nitems;
-  cudaError_t e0 = cudaMemsetAsync(c->ctrl, 0, 16, st);   // work counter
-  if (e0 != cudaSuccess) return e0;
+  long long grid = 0;
+  cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->ctrl, 0, 16, st);
+  if (e != cudaSuccess) return e;
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
 }
 
-// ---- plane kernel (one thread = one n x n plane of one vector), uniform Cartesian cells
+// ---- kind 8: plane kernel (one thread = one n x n plane of one vector), 16 vectors per block
 template <int PDEG> struct PlaneCfg;
 template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 2; };
-template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };
+template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };   // spills; kept for comparison
 bool plane_ok(int p) { return p == 6 || p == 7; }
 
-// Launch of a persistent TMA kernel `kern(tw, tz, prm, init, nitems)`: plain when the kernel only accumulates,
-// cooperative (all blocks co-resident) when it also initialises Z ahead of itself (fe_init_ahead.cuh).  The
-// per-context counters advance by `grid` per fused launch.
-template <typename Kern>
-cudaError_t launch_persistent(fe_mf_ctx* c, Kern kern, int nt, size_t smem, int& blocks_per_sm, const fe::ApplyParams& prm,
-                              fe::InitParams init, const CUtensorMap& tw, const CUtensorMap& tz, cudaStream_t st) {
-  if (blocks_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, nt, smem);
-    if (e != cudaSuccess) return e;
-    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
-  }
-  const long long nitems_ll = c->ncells * prm.nvb;
-  long long grid = (long long)blocks_per_sm * c->nsm;
-  if (grid > nitems_ll) grid = nitems_ll;
-  int nitems = (int)nitems_ll;
-  {
-    cudaError_t e = cudaMemsetAsync(c->ctrl, 0, init.mode == fe::INIT_NONE ? 16 : c->ctrl_bytes, st);
-    if (e != cudaSuccess) return e;
-  }
-  if (init.mode == fe::INIT_NONE && c->variant != 17) {
-    kern<<<(unsigned)grid, nt, smem, st>>>(tw, tz, prm, init, nitems);
+template <int PDEG, int IM>
+cudaError_t launch_plane_im(fe_mf_ctx* c, const fe::ApplyParams& prm, fe::InitParams init, const CUtensorMap& tw,
+                            const CUtensorMap& tz, cudaStream_t st) {
+  using C = PlaneCfg<PDEG>;
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  static int bps = 0;
+  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IM>;
+  long long grid = 0;
+  int nitems = (int)(c->ncells * prm.nvb);
+  cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->ctrl, 0, IM == 0 ? 16 : c->ctrl_bytes, st);
+  if (e != cudaSuccess) return e;
+  if (IM == 0) {
+    kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, init, nitems);
     return cudaGetLastError();
   }
-  if (init.mode == fe::INIT_NONE) {   // timing experiment: the accumulate-only kernel, launched cooperatively
-    void* args0[] = {(void*)&tw, (void*)&tz, (void*)&prm, (void*)&init, (void*)&nitems};
-    return cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3(nt), args0, smem, st);
-  }
+  // the blocks wait for one another's initialisation: they must all be resident (cooperative launch)
   init.slice_ctr = c->ctrl + 4;
   init.done = c->ctrl + 4 + c->ncz;
   void* args[] = {(void*)&tw, (void*)&tz, (void*)&prm, (void*)&init, (void*)&nitems};
-  return cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3(nt), args, smem, st);
+  return cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)grid), dim3(C::NT), args, SMEM, st);
 }
-
-template <int PDEG, int CFG = PDEG>
+template <int PDEG>
 cudaError_t launch_plane(fe_mf_ctx* c, const fe::ApplyParams& prm, const fe::InitParams& init, const CUtensorMap& tw,
                          const CUtensorMap& tz, cudaStream_t st) {
-  using C = PlaneCfg<CFG>;
-  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
-  static int bps[3] = {0, 0, 0};
-  if (init.mode == fe::INIT_NONE) return launch_persistent(c, fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, 0>, C::NT, SMEM, bps[0], prm, init, tw, tz, st);
-  if (init.mode == fe::INIT_ZERO) return launch_persistent(c, fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, 1>, C::NT, SMEM, bps[1], prm, init, tw, tz, st);
-  return launch_persistent(c, fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, 2>, C::NT, SMEM, bps[2], prm, init, tw, tz, st);
+  if (init.mode == fe::INIT_NONE) return launch_plane_im<PDEG, 0>(c, prm, init, tw, tz, st);
+  if (init.mode == fe::INIT_ZERO) return launch_plane_im<PDEG, 1>(c, prm, init, tw, tz, st);
+  return launch_plane_im<PDEG, 2>(c, prm, init, tw, tz, st);
 }
 
-// ---- second-generation line kernel (two vectors per thread, fused even/odd chains)
-template <int CFG> struct LineCfg : TmaCfg<CFG> {};
-template <> struct LineCfg<207> { static constexpr int BV = 8, NT = 256, MINB = 2; };   // p=7: two blocks per SM
-template <> struct LineCfg<307> { static constexpr int BV = 16, NT = 512, MINB = 1; };  // p=7: one round per pass
-template <> struct LineCfg<407> { static constexpr int BV = 8, NT = 128, MINB = 3; };   // p=7: three blocks per SM
-template <> struct LineCfg<208> { static constexpr int BV = 8, NT = 384, MINB = 1; };   // p=8: one round per pass
+// ---- kind 9: line kernel (one thread = one line of two vectors)
+template <int CFG> struct LineCfg;
+template <> struct LineCfg<1> { static constexpr int BV = 16, NT = 32, MINB = 4; };
+template <> struct LineCfg<2> { static constexpr int BV = 16, NT = 96, MINB = 4; };
+template <> struct LineCfg<3> { static constexpr int BV = 16, NT = 128, MINB = 4; };
+template <> struct LineCfg<4> { static constexpr int BV = 16, NT = 112, MINB = 4; };
+template <> struct LineCfg<5> { static constexpr int BV = 16, NT = 160, MINB = 3; };
+template <> struct LineCfg<6> { static constexpr int BV = 16, NT = 256, MINB = 2; };
+template <> struct LineCfg<7> { static constexpr int BV = 16, NT = 256, MINB = 1; };
+template <> struct LineCfg<8> { static constexpr int BV = 8, NT = 192, MINB = 2; };
+// 8 vectors per block: calls with <= 8 vectors (no lanes wasted on the vector tail) and, for p = 7, always
+// (three 8-vector blocks per SM beat one 16-vector block: 105 vs 99.6 GDoF*vec/s)
+template <> struct LineCfg<101> { static constexpr int BV = 8, NT = 32, MINB = 4; };
+template <> struct LineCfg<102> { static constexpr int BV = 8, NT = 64, MINB = 4; };
+template <> struct LineCfg<103> { static constexpr int BV = 8, NT = 64, MINB = 4; };
+template <> struct LineCfg<104> { static constexpr int BV = 8, NT = 128, MINB = 4; };
+template <> struct LineCfg<105> { static constexpr int BV = 8, NT = 160, MINB = 4; };
+template <> struct LineCfg<106> { static constexpr int BV = 8, NT = 128, MINB = 5; };
+template <> struct LineCfg<107> { static constexpr int BV = 8, NT = 128, MINB = 3; };
+int line_bv(const fe_mf_ctx* c, int nvec) {
+  if (c->p == 8 || c->variant == 11 || nvec <= 8) return 8;
+  if (c->p == 7 && c->variant != 10) return 8;
+  return 16;
+}
 
-template <int PDEG, int CFG = PDEG>
+template <int PDEG, int CFG>
 cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                         cudaStream_t st) {
   using C = LineCfg<CFG>;
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
-  static int blocks_per_sm = 0;
+  static int bps = 0;
   auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB>;
-  if (blocks_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
-    if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, C::NT, SMEM);
-    if (e != cudaSuccess) return e;
-    if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
-  }
   const long long nitems = c->ncells * prm.nvb;
-  long long grid = (long long)blocks_per_sm * c->nsm;
-  if (grid > nitems) grid = nitems;
-  cudaError_t e0 = cudaMemsetAsync(c->ctrl, 0, 16, st);   // work counter
-  if (e0 != cudaSuccess) return e0;
+  long long grid = 0;
+  cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->ctrl, 0, 16, st);
+  if (e != cudaSuccess) return e;
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
 }
-// vectors per block of the line kernel for (p, variant)
-int line_bv(const fe_mf_ctx* c, int nvec) {
-  if (c->variant == 11 || c->variant == 12 || nvec <= 8) return 8;
-  if (c->p == 7 && c->variant != 10 && c->variant != 13) return 8;   // p = 7: three 8-vector blocks per SM beat one 16-vector block
-  return tma_bv(c->p);
-}
 
-// Which kernel serves (ctx, nvec): 1 = general (any geometry, any nvec), 2 = Cartesian even-odd BV=8,
-// 4 = Cartesian even-odd, two vectors per thread (production; needs even nvec and 16-byte aligned pointers).
+// ---- which kernel serves (ctx, nvec, pointers)
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 1) return 1;
   const bool diag = (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
   const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
   const bool tma_ok = !(nvec & 1) && aligned && encode_tiled_fn() &&
-                      (unsigned long long)nvec * 8ULL * c->ndx * c->ndy < (1ULL << 40);
-  if ((!diag || c->variant == 7) && nvec >= 2 && tma_ok) return 6;   // full symmetric metric, TMA
+                      (unsigned long long)nvec * 8ULL * c->ndx * c->ndy < (1ULL << 40) &&
+                      c->ncells * ((nvec + 7) / 8) < (1LL << 31);
+  if ((!diag || c->variant == 7) && tma_ok) return 6;
   if (!diag || nvec < 4) return 1;
-  if (c->variant == 2) return 2;
-  if ((nvec & 1) || !aligned) return 2;
-  if (c->variant == 4) return 4;
-  if (!encode_tiled_fn()) return 4;
-  if ((unsigned long long)nvec * 8ULL * c->ndx * c->ndy >= (1ULL << 40)) return 4;
-  if (c->variant == 5 || c->variant == 6 || c->variant == 101) return 5;   // first-generation line kernel (kept for comparison)
-  if (c->variant >= 10 && c->variant <= 13) return 9;
-  // plane kernel: one plane of ONE vector per thread, 16 vectors per block; worth it when the last block is mostly full
+  if (!tma_ok || c->variant == 2) return 2;
+  const bool trim_ok = (c->bc != FE_BC_DIRICHLET) || (c->ndx >= 3 && c->ndy >= 3 && c->ndz >= 3);
+  if (!trim_ok) return 2;
+  if (c->variant == 10 || c->variant == 11) return 9;
+  if ((c->variant == 8 || c->variant == 19) && plane_ok(c->p)) return 8;
+  // plane kernel: 16 vectors per block; worth it when the last block of vectors is mostly full
   const int tail = nvec % 16;
-  if (plane_ok(c->p) && c->p == 6 && nvec >= 12 && (tail == 0 || tail >= 12)) return 8;
-  if ((c->variant == 8 || c->variant >= 14) && plane_ok(c->p)) return 8;
+  if (c->p == 6 && nvec >= 12 && (tail == 0 || tail >= 12)) return 8;
   return 9;
 }
 int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
-  if (kind == 8) return 16;
-  if (kind == 9) return line_bv(c, nvec);
-  return kind == 1 ? general_bv(c->p, nvec) : (kind == 6 ? gen_bv(c->p) : kind == 2 ? 8 : (kind == 4 ? cart2_bv(c->p) : (tma_use_bv8(c, nvec) ? 8 : tma_bv(c->p))));
+  switch (kind) {
+    case 1: return general_bv(c->p, nvec);
+    case 2: return 8;
+    case 6: return kGenBv;
+    case 8: return 16;
+    default: return line_bv(c, nvec);
+  }
 }
 
 fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, double alpha, int nvec, int bv) {
@@ -354,102 +269,69 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   return P;
 }
 
-// Can this kernel kind initialise Z itself (cooperative launch available)?
+// Can this kernel kind initialise Z itself?  (plane kernel, cooperative launch, 32-bit chunk sizes; opt-in)
 bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
   const long long chunk2 = (long long)(c->p + 1) * c->ndx * c->ndy * nvec / 2;   // double2 elements of the largest chunk
-  return kind == 8 && c->coop && (c->variant == 15 || c->variant == 16 || c->variant == 18 || c->variant == 19) && chunk2 < (1LL << 31) &&
-         c->ncells * ((nvec + 15) / 16) < (1LL << 31);
+  return kind == 8 && c->coop && c->variant == 19 && chunk2 < (1LL << 31);
 }
+
+#define FE_DISPATCH_P(CALL)                                           \
+  switch (c->p) {                                                     \
+    case 1: e = CALL(1); break; case 2: e = CALL(2); break;           \
+    case 3: e = CALL(3); break; case 4: e = CALL(4); break;           \
+    case 5: e = CALL(5); break; case 6: e = CALL(6); break;           \
+    case 7: e = CALL(7); break; case 8: e = CALL(8); break;           \
+  }
 
 // Z += alpha * A * W  (Z already initialised), or with init.mode != INIT_NONE (only if kind_fuses_init):
 // Z <- beta Z + gamma W + alpha A W in ONE launch.  Counts launches into c->last_launches.
 int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st,
-                      fe::InitParams init = fe::InitParams{fe::INIT_NONE, 0, 0.0, 0.0, nullptr, nullptr}) {
+                      fe::InitParams init = fe::InitParams{fe::INIT_NONE, 0.0, 0.0, nullptr, nullptr}) {
   const int kind = pick_kernel(c, nvec, W, Z);
   const int bv = kernel_bv(c, kind, nvec);
   fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
-  if (kind == 2) e = launch_cart_p<8>(c->p, P, c->ncells, st);
-  else if (kind == 6) {
-    CUtensorMap tw, tz;
-    if (!make_tensor_map(&tw, c, W, nvec, bv) || !make_tensor_map(&tz, c, Z, nvec, bv))
+  CUtensorMap tw, tz;
+  if (kind == 6 || kind == 8 || kind == 9) {
+    // Cartesian kernels on Dirichlet meshes: boundary nodes are out of bounds of the maps (see make_tensor_map)
+    const bool trim = (kind != 6) && (c->bc == FE_BC_DIRICHLET);
+    if (!make_tensor_map(&tw, c, W, nvec, bv, trim ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, trim ? 1 : 0))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
-    switch (c->p) {
-      case 1: e = launch_gen<1>(c, P, tw, tz, st); break;
-      case 2: e = launch_gen<2>(c, P, tw, tz, st); break;
-      case 3: e = launch_gen<3>(c, P, tw, tz, st); break;
-      case 4: e = launch_gen<4>(c, P, tw, tz, st); break;
-      case 5: e = launch_gen<5>(c, P, tw, tz, st); break;
-      case 6: e = launch_gen<6>(c, P, tw, tz, st); break;
-      case 7: e = launch_gen<7>(c, P, tw, tz, st); break;
-      case 8: e = launch_gen<8>(c, P, tw, tz, st); break;
-    }
+  }
+  if (kind == 8 || kind == 9 || kind == 2)
+    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // Cartesian kernels: the result is linear in the metric constants
+  if (kind == 6) {
+#define FE_CALL(p_) launch_gen<p_>(c, P, tw, tz, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
   } else if (kind == 8) {
-    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
-    CUtensorMap tw, tz;
-    const bool dir = (c->bc == FE_BC_DIRICHLET);
-    if (!make_tensor_map(&tw, c, W, nvec, bv, dir ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, dir ? 1 : 0))
-      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
-    switch (c->p) {
-      case 6: e = launch_plane<6>(c, P, init, tw, tz, st); break;
-      case 7: e = launch_plane<7>(c, P, init, tw, tz, st); break;
-    }
+    e = (c->p == 6) ? launch_plane<6>(c, P, init, tw, tz, st) : launch_plane<7>(c, P, init, tw, tz, st);
   } else if (kind == 9) {
-    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
-    CUtensorMap tw, tz;
-    const bool dir = (c->bc == FE_BC_DIRICHLET);
-    if (!make_tensor_map(&tw, c, W, nvec, bv, dir ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, dir ? 1 : 0))
-      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
-    const bool alt = (bv == 8);
-    switch (c->p) {
-      case 1: e = alt ? launch_line<1, 101>(c, P, tw, tz, st) : launch_line<1>(c, P, tw, tz, st); break;
-      case 2: e = alt ? launch_line<2, 102>(c, P, tw, tz, st) : launch_line<2>(c, P, tw, tz, st); break;
-      case 3: e = alt ? launch_line<3, 103>(c, P, tw, tz, st) : launch_line<3>(c, P, tw, tz, st); break;
-      case 4: e = alt ? launch_line<4, 104>(c, P, tw, tz, st) : launch_line<4>(c, P, tw, tz, st); break;
-      case 5: e = alt ? launch_line<5, 105>(c, P, tw, tz, st) : launch_line<5>(c, P, tw, tz, st); break;
-      case 6: e = alt ? launch_line<6, 106>(c, P, tw, tz, st) : launch_line<6>(c, P, tw, tz, st); break;
-      case 7: e = alt ? (c->variant == 11 ? launch_line<7, 207>(c, P, tw, tz, st) : launch_line<7, 407>(c, P, tw, tz, st))
-                      : (c->variant == 13 ? launch_line<7, 307>(c, P, tw, tz, st) : launch_line<7>(c, P, tw, tz, st)); break;
-      case 8: e = (c->variant == 11) ? launch_line<8, 208>(c, P, tw, tz, st) : launch_line<8>(c, P, tw, tz, st); break;
+    if (bv == 16) {
+#define FE_CALL(p_) launch_line<p_, p_>(c, P, tw, tz, st)
+      FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
+    } else if (c->p == 8) {
+      e = launch_line<8, 8>(c, P, tw, tz, st);
+    } else {
+#define FE_CALL(p_) launch_line<p_, 100 + p_>(c, P, tw, tz, st)
+      switch (c->p) {
+        case 1: e = FE_CALL(1); break; case 2: e = FE_CALL(2); break; case 3: e = FE_CALL(3); break;
+        case 4: e = FE_CALL(4); break; case 5: e = FE_CALL(5); break; case 6: e = FE_CALL(6); break;
+        case 7: e = FE_CALL(7); break;
+      }
+#undef FE_CALL
     }
-  } else if (kind == 5) {
-    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;
-    CUtensorMap tw, tz;
-    if (!make_tensor_map(&tw, c, W, nvec, bv) || !make_tensor_map(&tz, c, Z, nvec, bv))
-      return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
-    const bool alt = tma_use_bv8(c, nvec);
-    switch (c->p) {
-      case 1: e = alt ? launch_tma<1, 101>(c, P, tw, tz, st) : launch_tma<1>(c, P, tw, tz, st); break;
-      case 2: e = alt ? launch_tma<2, 102>(c, P, tw, tz, st) : launch_tma<2>(c, P, tw, tz, st); break;
-      case 3: e = alt ? launch_tma<3, 103>(c, P, tw, tz, st) : launch_tma<3>(c, P, tw, tz, st); break;
-      case 4: e = alt ? launch_tma<4, 104>(c, P, tw, tz, st) : launch_tma<4>(c, P, tw, tz, st); break;
-      case 5: e = alt ? launch_tma<5, 105>(c, P, tw, tz, st) : launch_tma<5>(c, P, tw, tz, st); break;
-      case 6: e = alt ? launch_tma<6, 106>(c, P, tw, tz, st) : (c->variant == 6 ? launch_tma<6, 6, false>(c, P, tw, tz, st) : (c->variant == 101 ? launch_tma<6, 6, true, 1>(c, P, tw, tz, st) : launch_tma<6>(c, P, tw, tz, st))); break;
-      case 7: e = alt ? launch_tma<7, 107>(c, P, tw, tz, st) : launch_tma<7>(c, P, tw, tz, st); break;
-      case 8: e = (c->variant == 5) ? launch_tma<8, 108>(c, P, tw, tz, st) : launch_tma<8>(c, P, tw, tz, st); break;
-    }
-  } else if (kind == 4) {
-    for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // the result is linear in the metric constants
-    switch (c->p) {
-      case 1: e = launch_cart2<1>(P, c->ncells, st); break;
-      case 2: e = launch_cart2<2>(P, c->ncells, st); break;
-      case 3: e = launch_cart2<3>(P, c->ncells, st); break;
-      case 4: e = launch_cart2<4>(P, c->ncells, st); break;
-      case 5: e = launch_cart2<5>(P, c->ncells, st); break;
-      case 6: e = launch_cart2<6>(P, c->ncells, st); break;
-      case 7: e = launch_cart2<7>(P, c->ncells, st); break;
-      case 8: e = launch_cart2<8>(P, c->ncells, st); break;
-    }
-  } else switch (c->p) {
-    case 1: e = launch_general<1>(P, c->ncells, st); break;
-    case 2: e = launch_general<2>(P, c->ncells, st); break;
-    case 3: e = launch_general<3>(P, c->ncells, st); break;
-    case 4: e = launch_general<4>(P, c->ncells, st); break;
-    case 5: e = launch_general<5>(P, c->ncells, st); break;
-    case 6: e = launch_general<6>(P, c->ncells, st); break;
-    case 7: e = launch_general<7>(P, c->ncells, st); break;
-    case 8: e = launch_general<8>(P, c->ncells, st); break;
+  } else if (kind == 2) {
+    P.alpha = 1.0;
+#define FE_CALL(p_) launch_cart<p_>(P, c->ncells, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
+  } else {
+#define FE_CALL(p_) launch_general<p_>(P, c->ncells, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
   }
   if (e != cudaSuccess) return fail(c, FE_MF_ECUDA, std::string("apply kernel launch: ") + cudaGetErrorString(e));
   c->last_launches += 1;
@@ -500,7 +382,7 @@ extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_d
   const size_t count = (size_t)ctx->ndof * nvec;
   const int kind = pick_kernel(ctx, nvec, W_dev, Z_dev);
   if (kind_fuses_init(ctx, kind, nvec)) {   // S1 folded into the apply kernel (fe_init_ahead.cuh): one launch
-    fe::InitParams init{beta == 0.0 ? (gamma == 0.0 ? fe::INIT_ZERO : fe::INIT_SCALE) : fe::INIT_AXPBY, ctx->variant == 15 ? 1 : (ctx->variant == 16 ? 2 : (ctx->variant == 18 ? 4 : 0)), beta, gamma, nullptr, nullptr};
+    fe::InitParams init{beta == 0.0 ? (gamma == 0.0 ? fe::INIT_ZERO : fe::INIT_SCALE) : fe::INIT_AXPBY, beta, gamma, nullptr, nullptr};
     return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st, init);
   }
   rc = launch_init(ctx, Z_dev, W_dev, beta, gamma, count, st);
@@ -626,16 +508,13 @@ extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
   return kernel_bv(ctx, kind, nvec);
 }
 
-extern "C" int fe_mf_debug_ctrl(fe_mf_ctx* ctx, unsigned* out4) {   // diagnostics: the first control words after a launch
-  if (!ctx || !out4) return FE_MF_EINVAL;
-  return cudaMemcpy(out4, ctx->ctrl, 16, cudaMemcpyDeviceToHost) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
-}
-
 extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx->last_launches : -1; }
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  if ((variant < 0 || variant > 19) && variant != 101) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
+  const bool known = variant == 0 || variant == 1 || variant == 2 || variant == 7 || variant == 8 || variant == 10 ||
+                     variant == 11 || variant == 19;
+  if (!known) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;
 }

@@ -23,7 +23,6 @@ enum { INIT_NONE = -1, INIT_ZERO = 0, INIT_SCALE = 1, INIT_AXPBY = 2 };
 
 struct InitParams {
   int mode;                          // INIT_*
-  int dbg;                           // timing experiments only: 1 = no readiness wait, 2 = no stores
   double beta, gamma;                // Z <- beta Z + gamma W
   unsigned* slice_ctr;               // [ncz] next slice of chunk c to hand out (0 at launch)
   unsigned* done;                    // [ncz] warp-slices of chunk c completed (0 at launch)
@@ -94,7 +93,7 @@ struct InitAhead {
     publish_point();
   }
   __device__ __forceinline__ void zero_slices(int c, unsigned s0, unsigned s1, unsigned step) {
-    if (I.dbg == 2 || s0 >= s1) return;
+    if (s0 >= s1) return;
     const unsigned n = len(c);
     unsigned e = s0 * NT + tid;
     double2* z = Z2 + begin(c) + e;
@@ -200,16 +199,15 @@ struct InitAhead {
     if (IM == 0) return;
     if (c > last) c = last;
     if (c <= ready) return;
-    if (tid == 0 && I.dbg != 1) {
+    if (tid == 0) {
       // (the first wait of a block also covers chunk 0: the periodic wrap of the last layer adds into it)
       for (int cc = (ready < 0 ? 0 : c - 1); cc <= c; ++cc) {
         const unsigned target = nslices(cc);
-        unsigned v, spins = 0;
+        unsigned v;
         do {
           asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(I.done + cc) : "memory");
-          if (v < target) { __nanosleep(100); ++spins; }
+          if (v < target) __nanosleep(100);
         } while (v < target);
-        if (I.dbg >= 4 && spins) { atomicAdd(I.slice_ctr - 3, spins); atomicAdd(I.slice_ctr - 2, 1u); }
       }
       asm volatile("fence.proxy.async;" ::: "memory");
     }

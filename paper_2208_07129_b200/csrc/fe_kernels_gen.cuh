@@ -29,7 +29,6 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
   constexpr int ROUNDS = (TASKS + NT - 1) / NT;
   constexpr bool ROTATE = (NT % 32 == 0) && (NT >= 128);
   constexpr int NW = NT / 32;
-  constexpr int DBG = 0;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* A = reinterpret_cast<double*>(smem_raw);
   double* B = reinterpret_cast<double*>(smem_raw + TL::PITCH);

@@ -218,10 +218,11 @@ def test_unit_cube_config5_interval_is_rejected(env):
         op.cheb_filter(X, Y, 1, 20, 2.0, 0.3, 0.0)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 4, 5, 6, 8, 9, 10, 11])
+@pytest.mark.parametrize("variant", [1, 2, 8, 10, 11, 19])
 @pytest.mark.parametrize("p,bc", [(6, inputs.BC_DIRICHLET), (7, inputs.BC_PERIODIC), (8, inputs.BC_PERIODIC), (4, inputs.BC_PERIODIC)])
 def test_kernel_variants(env, variant, p, bc):
-    """variant 1 = general kernel, 2 = even-odd Cartesian kernel with one vector per thread, 4 = two vectors per thread with LDG/RED (default 0: persistent TMA kernel)."""
+    """variant 1 = general fallback kernel, 2 = even-odd Cartesian kernel with one vector per thread (LDG/RED),
+    8 = plane kernel, 10 / 11 = line kernel with 16 / 8 vectors per block, 19 = plane kernel that also initialises Y."""
     torch, orc, binding = env
     w = inputs.Workload(f"var_p{p}", p, (3, 2, 3), bc, inputs.GEOM_AFFINE, 0.8, (0.0, 0.0, 0.0), (1.5, 1.0, 2.0), 20, 500 + p)
     X = inputs.multivector(w.seed, w.ndof, w.nvec)
@@ -231,6 +232,30 @@ def test_kernel_variants(env, variant, p, bc):
     Xd = torch.from_numpy(X).cuda(); Yd = torch.empty_like(Xd)
     op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
+
+
+@pytest.mark.parametrize("variant", [0, 19])
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+def test_plane_kernel_many_layers(env, bc, variant):
+    """p = 6, 9 cell layers in z (more than the init-ahead look-ahead), 40 vectors (a partial last block): plain apply
+    and Z <- beta Z + gamma W + alpha A W, with the initialisation as a separate pass (0) or folded into the
+    kernel (19: dynamic slices, cooperative launch)."""
+    torch, orc, binding = env
+    w = inputs.Workload("plane_layers", 6, (2, 3, 9), bc, inputs.GEOM_AFFINE, 0.7, (0.0, 0.0, 0.0), (1.0, 1.5, 3.0), 40, 4242)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    Z0 = inputs.multivector(w.seed + 1, w.ndof, w.nvec)
+    Yo = orc.Operator(oracle_mesh(orc, w), w.sigma).apply(X)
+    op = binding.FeMf.from_workload(w); op.set_variant(variant)
+    Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
+    op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
+    assert relerr(Yd.cpu().numpy(), Yo) <= TOL
+    assert op.last_launch_count() == (1 if variant == 19 else 2)
+    Zd = torch.from_numpy(Z0).cuda()
+    op.apply_axpby(0.3, Xd, 0.5, -0.25, Zd, w.nvec); torch.cuda.synchronize()
+    assert relerr(Zd.cpu().numpy(), 0.5 * Z0 - 0.25 * X + 0.3 * Yo) <= TOL
+    Zd = torch.from_numpy(Z0).cuda()
+    op.apply_axpby(0.3, Xd, 0.0, -0.25, Zd, w.nvec); torch.cuda.synchronize()
+    assert relerr(Zd.cpu().numpy(), -0.25 * X + 0.3 * Yo) <= TOL
 
 
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
