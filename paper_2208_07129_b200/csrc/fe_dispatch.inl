@@ -5,6 +5,7 @@
 //   kind 9  fe_apply_cart_line   uniform Cartesian cells, any p: one line of two vectors per thread
 //   kind 6  fe_apply_gen_tma     full symmetric metric (per-q-point or per-cell geometry)
 //   kind 2  fe_apply_cart        Cartesian, odd nvec or unaligned pointers (LDG gather / RED scatter)
+//   kind 3  fe_apply_cart<CELLS> Cartesian, 1-3 vectors: the tile slots hold several cells of an x-row
 //   kind 1  fe_apply_general     anything else (nvec = 1, odd nvec with a full metric): plain contractions
 // fe_mf_set_variant forces a kind for tests and experiments: 1 -> kind 1, 2 -> kind 2, 7 -> kind 6 on a Cartesian
 // mesh, 8 -> plane, 10 -> line with 16-vector blocks, 11 -> line with 8-vector blocks, 19 -> plane kernel that
@@ -60,6 +61,25 @@ cudaError_t launch_cart(const fe::ApplyParams& prm, long long ncells, cudaStream
     configured = true;
   }
   kern<<<(unsigned)(ncells * prm.nvb), C::NT, C::SMEM, st>>>(prm);
+  return cudaGetLastError();
+}
+
+// kind 3: the same kernel with the 8 tile slots holding 1-3 vectors of 8 / nvec consecutive cells of an x-row
+template <int PDEG>
+cudaError_t launch_cart_cells(const fe::ApplyParams& prm, const fe_mf_ctx* c, cudaStream_t st) {
+  using C = CartCfg<PDEG>;
+  static bool configured = false;
+  auto kern = fe::fe_apply_cart<PDEG, C::BV, C::NT, C::MINB, true>;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int cb = C::BV / prm.nvec;                      // cells per block
+  const long long groups = (c->ncx + cb - 1) / cb;
+  const long long grid = groups * c->ncy * c->ncz;
+  if (grid > 2147483647LL) return cudaErrorInvalidValue;
+  kern<<<(unsigned)grid, C::NT, C::SMEM, st>>>(prm);
   return cudaGetLastError();
 }
 
@@ -232,7 +252,8 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
                       (unsigned long long)nvec * 8ULL * c->ndx * c->ndy < (1ULL << 40) &&
                       c->ncells * ((nvec + 7) / 8) < (1LL << 31);
   if ((!diag || c->variant == 7) && tma_ok) return 6;
-  if (!diag || nvec < 4) return 1;
+  if (!diag) return 1;
+  if (nvec < 4) return 3;
   if (!tma_ok || c->variant == 2) return 2;
   const bool trim_ok = (c->bc != FE_BC_DIRICHLET) || (c->ndx >= 3 && c->ndy >= 3 && c->ndz >= 3);
   if (!trim_ok) return 2;
@@ -247,6 +268,7 @@ int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
   switch (kind) {
     case 1: return general_bv(c->p, nvec);
     case 2: return 8;
+    case 3: return nvec;
     case 6: return kGenBv;
     case 8: return 16;
     default: return line_bv(c, nvec);
@@ -299,7 +321,7 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
     if (!make_tensor_map(&tw, c, W, nvec, bv, trim ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, trim ? 1 : 0))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
   }
-  if (kind == 8 || kind == 9 || kind == 2)
+  if (kind == 8 || kind == 9 || kind == 2 || kind == 3)
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // Cartesian kernels: the result is linear in the metric constants
   if (kind == 6) {
 #define FE_CALL(p_) launch_gen<p_>(c, P, tw, tz, st)
@@ -323,6 +345,11 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
       }
 #undef FE_CALL
     }
+  } else if (kind == 3) {
+    P.alpha = 1.0;
+#define FE_CALL(p_) launch_cart_cells<p_>(P, c, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
   } else if (kind == 2) {
     P.alpha = 1.0;
 #define FE_CALL(p_) launch_cart<p_>(P, c->ncells, st)

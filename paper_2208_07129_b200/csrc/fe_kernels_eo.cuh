@@ -109,7 +109,10 @@ __device__ __forceinline__ void sts_line(double* s, int stride, const double (&x
 
 // Fused apply for cells whose metric is diagonal and constant per cell (uniform Cartesian meshes: configs
 // 1, 2, 4, 5).  Z += alpha * A * W.  One block = one cell x BV vectors; NT threads; 2 tiles of shared memory.
-template <int PDEG, int BV, int NT, int MINB>
+// CELLS (calls with 1-3 vectors, e.g. the single-vector point of config 4's sweep): the BV slots of a tile hold
+// P.nvec vectors of BV / P.nvec consecutive cells of an x-row instead of BV vectors of one cell, so that the
+// lanes stay busy and the shared-memory layout (slot innermost) stays conflict-free.
+template <int PDEG, int BV, int NT, int MINB, bool CELLS = false>
 __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
   using TL = Tile<PDEG, BV>;
   constexpr int N = PDEG + 1, NL = N * N, TASKS = NL * BV;
@@ -117,10 +120,12 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
   double* A = smem;
   double* B = smem + TL::SIZE;
   const int tid = threadIdx.x;
-  const int vb = blockIdx.x % P.nvb;
-  const int cell = blockIdx.x / P.nvb;
-  const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
-  const int v0 = vb * BV;
+  const int nvb = CELLS ? (P.ncx + (BV / P.nvec) - 1) / (BV / P.nvec) : P.nvb;   // CELLS: cell groups per x-row
+  const int vb = blockIdx.x % nvb;
+  const int cell = CELLS ? (blockIdx.x / nvb) * P.ncx : blockIdx.x / P.nvb;      // CELLS: first cell of the x-row
+  const int ex0 = CELLS ? vb * (BV / P.nvec) : cell % P.ncx;
+  const int ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
+  const int v0 = CELLS ? 0 : vb * BV;
   const double gxx = P.ug[0], gyy = P.ug[3], gzz = P.ug[5], gm = P.ug[6];
 
   // phase 0: gather x-lines (S2) + Ns along x (S3, dim 1)
@@ -128,7 +133,9 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
     const int beta = t % BV, l = t / BV;
     const int i2 = l % N, i3 = l / N;
     int iy = ey * PDEG + i2, iz = ez * PDEG + i3;
-    bool live = (v0 + beta) < P.nvec;
+    const int ex = CELLS ? ex0 + beta / P.nvec : ex0;     // slot -> (cell, vector)
+    const int vv = CELLS ? beta % P.nvec : v0 + beta;
+    bool live = CELLS ? (ex < P.ncx && beta < (BV / P.nvec) * P.nvec) : (vv < P.nvec);
     if (P.dirichlet) {
       if (iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
     } else {
@@ -137,7 +144,7 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
     }
     double x[N], y[N];
     const long long row = (long long)P.ndx * ((long long)iy + (long long)P.ndy * iz);
-    const double* src = P.W + (row + (long long)ex * PDEG) * P.nvec + v0 + beta;
+    const double* src = P.W + (row + (long long)ex * PDEG) * P.nvec + vv;
 #pragma unroll
     for (int i = 0; i < N; ++i) {
       int ix = ex * PDEG + i;
@@ -217,8 +224,10 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
     double x[N], y[N];
     lds_line<N>(B + base + beta, stride, x);
     eo_apply<PDEG, EO_NST>(x, y);
+    const int ex = CELLS ? ex0 + beta / P.nvec : ex0;
+    const int vv = CELLS ? beta % P.nvec : v0 + beta;
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2;
-    bool live = (v0 + beta) < P.nvec;
+    bool live = CELLS ? (ex < P.ncx && beta < (BV / P.nvec) * P.nvec) : (vv < P.nvec);
     if (P.dirichlet) {
       if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1) live = false;
     } else {
@@ -227,7 +236,7 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
     }
     if (live) {
       const long long plane = (long long)P.ndx * P.ndy;
-      double* dst = P.Z + ((long long)ix + (long long)P.ndx * iy) * P.nvec + v0 + beta;
+      double* dst = P.Z + ((long long)ix + (long long)P.ndx * iy) * P.nvec + vv;
 #pragma unroll
       for (int i = 0; i < N; ++i) {
         int iz = ez * PDEG + i;

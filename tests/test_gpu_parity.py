@@ -164,6 +164,15 @@ def test_chebyshev_small_degrees_and_x_scratch(env, m):
     assert relerr(Xd.cpu().numpy(), Xprev) <= TOL           # X holds iterate m-1 (header contract)
 
 
+@pytest.mark.parametrize("nvec", [1, 2, 3])
+@pytest.mark.parametrize("p,bc,nc", [(7, inputs.BC_PERIODIC, (5, 2, 2)), (6, inputs.BC_DIRICHLET, (9, 2, 3)),
+                                     (4, inputs.BC_PERIODIC, (3, 3, 2)), (2, inputs.BC_DIRICHLET, (11, 2, 2))])
+def test_few_vectors_cells_as_slots(env, p, bc, nc, nvec):
+    """1-3 vectors on a Cartesian mesh: the tile slots hold several cells of an x-row (ragged last group of cells)."""
+    w = inputs.Workload(f"few_p{p}", p, nc, bc, inputs.GEOM_AFFINE, 0.6, (0.0, 0.0, 0.0), (2.5, 1.0, 1.5), nvec, 900 + p)
+    check_apply(env, w)
+
+
 def test_apply_host_path(env):
     torch, orc, binding = env
     for nvec in (3, 32):
