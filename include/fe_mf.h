@@ -139,9 +139,13 @@ int fe_probe_peaks(double *fp64_tflops, double *hbm_gbs, int cuda_device);
 /* Introspection used by bench.py / tests: vectors per thread block chosen for this nvec, the
  * number of kernel launches the last call enqueued, and the dominant kernel's name. */
 int fe_mf_batch_width(const fe_mf_ctx *ctx, int nvec);
+const char *fe_mf_kernel_name(const fe_mf_ctx *ctx, int nvec);   /* static string, never NULL */
 int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
 
-/* Select a kernel variant (0 = default).  For profiling/ablation only; returns EINVAL if unknown. */
+/* Select a kernel variant (0 = default: chosen from degree, geometry and nvec).  For profiling/ablation only:
+ * 1 general fallback kernel, 2 one-vector-per-thread Cartesian kernel (LDG/RED), 7 full-metric TMA kernel on a
+ * Cartesian mesh, 8 plane kernel (p = 6, 7), 10 / 11 line kernel with 16 / 8 vectors per block, 19 plane kernel
+ * that also initialises the output (one cooperative launch).  Returns EINVAL if unknown. */
 int fe_mf_set_variant(fe_mf_ctx *ctx, int variant);
 
 /* Message of the last failing call on ctx; with ctx == NULL, of the last failing fe_mf_create on

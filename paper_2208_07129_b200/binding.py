@@ -34,6 +34,7 @@ SYMBOLS = {
     "fe_fill_uniform": (C.c_int, [C.c_void_p, C.c_longlong, C.c_ulonglong, C.c_longlong, C.c_void_p]),
     "fe_probe_peaks": (C.c_int, [_PD, _PD, C.c_int]),
     "fe_mf_batch_width": (C.c_int, [C.c_void_p, C.c_int]),
+    "fe_mf_kernel_name": (C.c_char_p, [C.c_void_p, C.c_int]),
     "fe_mf_last_launch_count": (C.c_int, [C.c_void_p]),
     "fe_mf_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
     "fe_mf_last_error": (C.c_char_p, [C.c_void_p]),
@@ -145,6 +146,9 @@ class FeMf:
 
     def batch_width(self, nvec: int) -> int:
         return int(self._l.fe_mf_batch_width(self._ctx, int(nvec)))
+
+    def kernel_name(self, nvec: int) -> str:
+        return self._l.fe_mf_kernel_name(self._ctx, int(nvec)).decode()
 
     def last_launch_count(self) -> int:
         return int(self._l.fe_mf_last_launch_count(self._ctx))

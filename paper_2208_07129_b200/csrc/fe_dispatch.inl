@@ -375,14 +375,12 @@ int stream_grid(size_t count) {
 // Z <- beta*Z + gamma*W, stream-ordered (S1 / the axpby half of S9).
 int launch_init(fe_mf_ctx* c, double* Z, const double* W, double beta, double gamma, size_t count, cudaStream_t st) {
   if (beta == 0.0 && gamma == 0.0) {
-    FE_CUDA(c, cudaMemsetAsync(Z, 0, count * sizeof(double), st));
-  } else if (beta == 0.0) {
-    fe::fe_scale_copy_kernel<<<stream_grid(count), 256, 0, st>>>(Z, W, gamma, count);
-    FE_CUDA(c, cudaGetLastError());
-  } else {
-    fe::fe_axpby_kernel<<<stream_grid(count / 2 + 1), 256, 0, st>>>(Z, W, beta, gamma, count);
-    FE_CUDA(c, cudaGetLastError());
+    FE_CUDA(c, cudaMemsetAsync(Z, 0, count * sizeof(double), st));   // a driver memset: not counted as a kernel launch
+    return FE_MF_OK;
   }
+  if (beta == 0.0) fe::fe_scale_copy_kernel<<<stream_grid(count), 256, 0, st>>>(Z, W, gamma, count);
+  else fe::fe_axpby_kernel<<<stream_grid(count / 2 + 1), 256, 0, st>>>(Z, W, beta, gamma, count);
+  FE_CUDA(c, cudaGetLastError());
   c->last_launches += 1;
   return FE_MF_OK;
 }
@@ -533,6 +531,18 @@ extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
   if (!ctx || nvec < 1) return -1;
   const int kind = pick_kernel(ctx, nvec, nullptr, nullptr);
   return kernel_bv(ctx, kind, nvec);
+}
+
+extern "C" const char* fe_mf_kernel_name(const fe_mf_ctx* ctx, int nvec) {
+  if (!ctx || nvec < 1) return "";
+  switch (pick_kernel(ctx, nvec, nullptr, nullptr)) {
+    case 1: return "fe_apply_general";
+    case 2: return "fe_apply_cart";
+    case 3: return "fe_apply_cart<CELLS>";
+    case 6: return "fe_apply_gen_tma";
+    case 8: return "fe_apply_cart_plane";
+    default: return "fe_apply_cart_line";
+  }
 }
 
 extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx->last_launches : -1; }

@@ -258,10 +258,11 @@ def test_plane_kernel_many_layers(env, bc, variant):
     Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
     op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
-    assert op.last_launch_count() == (1 if variant == 19 else 2)
+    assert op.last_launch_count() == 1                      # the zero fill of variant 0 is a driver memset
     Zd = torch.from_numpy(Z0).cuda()
     op.apply_axpby(0.3, Xd, 0.5, -0.25, Zd, w.nvec); torch.cuda.synchronize()
     assert relerr(Zd.cpu().numpy(), 0.5 * Z0 - 0.25 * X + 0.3 * Yo) <= TOL
+    assert op.last_launch_count() == (1 if variant == 19 else 2)
     Zd = torch.from_numpy(Z0).cuda()
     op.apply_axpby(0.3, Xd, 0.0, -0.25, Zd, w.nvec); torch.cuda.synchronize()
     assert relerr(Zd.cpu().numpy(), -0.25 * X + 0.3 * Yo) <= TOL
