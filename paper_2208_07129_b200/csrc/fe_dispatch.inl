@@ -106,7 +106,7 @@ EncodeTiledFn encode_tiled_fn() {
 // Dirichlet meshes (Cartesian kernels): trim = 2 -> the map covers nodes 1 .. nd-2 in every direction, origin at
 // node (1,1,1), so that boundary nodes are out of bounds (zero on load; box coordinates shift by -1); trim = 1 ->
 // nodes 0 .. nd-2, origin unchanged (the last node is clipped on reduce).
-bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim = 0) {
+bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim = 0, int padx = 0) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
   if (trim && (c->ndx < 3 || c->ndy < 3 || c->ndz < 3)) return false;
@@ -114,7 +114,7 @@ bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int 
   const cuuint64_t strides[3] = {(cuuint64_t)nvec * 8, (cuuint64_t)nvec * 8 * c->ndx, (cuuint64_t)nvec * 8 * c->ndx * c->ndy};
   if (strides[2] >= ((cuuint64_t)1 << 40)) return false;
   if (trim == 2) base = (const char*)base + (strides[0] + strides[1] + strides[2]);
-  const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)c->n, (cuuint32_t)c->n, (cuuint32_t)c->n};
+  const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)(c->n + padx), (cuuint32_t)c->n, (cuuint32_t)c->n};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -227,13 +227,17 @@ int line_bv(const fe_mf_ctx* c, int nvec) {
   return 16;
 }
 
+// 8-vector blocks with an even number of nodes per direction: one pad node per x-row (see DenseTile)
+constexpr int line_padx(int p, int bv) { return (bv == 8 && (p + 1) % 2 == 0 && p >= 3) ? 1 : 0; }
+
 template <int PDEG, int CFG>
 cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                         cudaStream_t st) {
   using C = LineCfg<CFG>;
-  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  constexpr int PADX = line_padx(PDEG, C::BV);
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV, PADX>::PITCH + 64;
   static int bps = 0;
-  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB>;
+  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB, PADX>;
   const long long nitems = c->ncells * prm.nvb;
   long long grid = 0;
   cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
@@ -318,7 +322,8 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
   if (kind == 6 || kind == 8 || kind == 9) {
     // Cartesian kernels on Dirichlet meshes: boundary nodes are out of bounds of the maps (see make_tensor_map)
     const bool trim = (kind != 6) && (c->bc == FE_BC_DIRICHLET);
-    if (!make_tensor_map(&tw, c, W, nvec, bv, trim ? 2 : 0) || !make_tensor_map(&tz, c, Z, nvec, bv, trim ? 1 : 0))
+    const int padx = (kind == 9) ? line_padx(c->p, bv) : 0;
+    if (!make_tensor_map(&tw, c, W, nvec, bv, trim ? 2 : 0, padx) || !make_tensor_map(&tz, c, Z, nvec, bv, trim ? 1 : 0, padx))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
   }
   if (kind == 8 || kind == 9 || kind == 2 || kind == 3)

@@ -12,11 +12,11 @@
 
 namespace fe {
 
-template <int PDEG, int BV, int NT, int MINB>
+template <int PDEG, int BV, int NT, int MINB, int PADX>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                    const __grid_constant__ ApplyParams P, int nitems) {
-  using TL = DenseTile<PDEG, BV>;
+  using TL = DenseTile<PDEG, BV, PADX>;
   constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1, NL = N * N, TPL = BV / 2, TASKS = NL * TPL;
   constexpr int ROUNDS = (TASKS + NT - 1) / NT;
   constexpr bool ROTATE = (NT % 32 == 0) && (NT >= 128) && (TASKS % NT != 0);
@@ -34,6 +34,10 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
   if (tid == 0) {
     mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (PADX) {   // the pad node of every x-row of the result tile is reduced into Z too: it must stay zero
+    for (int e = tid; e < N * N * BV; e += NT) B[(e / BV) * TL::XP + N * BV + e % BV] = 0.0;
+    fence_async_smem();
   }
   __syncthreads();
   int item = blockIdx.x;
@@ -59,7 +63,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     mbar_wait(bar, parity);
     parity ^= 1u;
     if (special) {
-      plane_wrap_fixup<PDEG, BV, NT, false>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
+      plane_wrap_fixup<PDEG, BV, NT, false, PADX>(A, P, tid, ex, ey, ez, v0, wx, wy, wz);
       __syncthreads();
     }
     // ph0: Ns along x, in place in A
@@ -180,7 +184,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     }
     fence_async_smem();
     __syncthreads();
-    if (special) plane_wrap_fixup<PDEG, BV, NT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
+    if (special) plane_wrap_fixup<PDEG, BV, NT, true, PADX>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
     if (tid == 0) {
       tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
       tma_commit();

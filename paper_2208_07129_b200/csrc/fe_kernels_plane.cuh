@@ -122,7 +122,7 @@ __device__ __forceinline__ void eo_dtd(const T (&t)[PDEG + 1], T (&u2)[(PDEG + 1
 // the plane phases stay branch-free: only the (up to three) wrapped faces i_d = N-1 are visited.
 // IN (OUT = false): fetch the wrap-around nodes the TMA box could not reach (it zero-filled them).
 // OUT: RED the wrap-around nodes that the clipped TMA reduction will not store.
-template <int PDEG, int BV, int NT, bool OUT>
+template <int PDEG, int BV, int NT, bool OUT, int PADX = 0>
 __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams& P, int tid, int ex, int ey, int ez, int v0,
                                                  bool wx, bool wy, bool wz) {
   constexpr int N = PDEG + 1, HB = BV / 2, FACE = N * N * HB;
@@ -143,7 +143,7 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
       if (iy >= P.ndy) iy -= P.ndy;
       if (iz >= P.ndz) iz -= P.ndz;
       const long long g = ((long long)ix + (long long)P.ndx * ((long long)iy + (long long)P.ndy * iz)) * nvec + v0 + b2;
-      double2* s = reinterpret_cast<double2*>(tile + ((i3 * N + i2) * N + i1) * BV + b2);
+      double2* s = reinterpret_cast<double2*>(tile + ((i3 * N + i2) * (N + PADX) + i1) * BV + b2);
       if (!OUT) {
         *s = __ldg(reinterpret_cast<const double2*>(P.W + g));
       } else {

@@ -51,10 +51,14 @@ __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.w
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-template <int PDEG, int BV>
+// PADX = 1: the box carries one extra node per x-row (the first node of the next cell's interior, never used).
+// With 8 vectors per block a node is 64 bytes, and for even n all x-lines of a dense tile start a multiple of
+// 128 bytes apart, so the two lines that share a 128-byte wavefront always collide (measured at p = 7: a third of
+// all shared-memory wavefronts were conflict replays); the extra node makes the row pitch an odd multiple of 64.
+template <int PDEG, int BV, int PADX = 0>
 struct DenseTile {
   static constexpr int N = PDEG + 1;
-  static constexpr int XP = N * BV;                   // dense: the TMA box layout
+  static constexpr int XP = (N + PADX) * BV;          // dense: the TMA box layout
   static constexpr int SIZE = N * N * XP;             // doubles
   static constexpr int BYTES = SIZE * 8;
   static constexpr int PITCH = (BYTES + 127) / 128 * 128;   // placement of the second tile
