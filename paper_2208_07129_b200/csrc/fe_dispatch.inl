@@ -176,7 +176,7 @@ template <int PDEG, int IM>
 cudaError_t launch_plane_im(fe_mf_ctx* c, const fe::ApplyParams& prm, fe::InitParams init, const CUtensorMap& tw,
                             const CUtensorMap& tz, cudaStream_t st) {
   using C = PlaneCfg<PDEG>;
-  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
+  constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64 + fe::InitAhead<C::NT, IM>::STAGE_BYTES;
   static int bps = 0;
   auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IM>;
   long long grid = 0;

@@ -15,7 +15,7 @@
 // item that needs it finishes), but all blocks must be co-resident: the kernels are launched cooperatively.
 // The control words are zeroed on the stream before every launch.
 #pragma once
-#include "fe_kernels.cuh"
+#include "fe_kernels_tma.cuh"
 
 namespace fe {
 
@@ -28,13 +28,22 @@ struct InitParams {
   unsigned* done;                    // [ncz] warp-slices of chunk c completed (0 at launch)
 };
 
-// IM: 0 = no initialisation (everything compiles out), 1 = zero fill (stores only), 2 = scale / axpby (loads in
-// flight across a phase).  Slice and element counts are 32-bit (the host falls back to a separate pass when a
-// chunk has 2^31 or more double2 elements).
+// IM: 0 = no initialisation (everything compiles out), 1 = zero fill (stores only), 2 = scale / axpby: the old Z
+// and W slices are STAGED through shared memory by bulk copies (no registers, no load latency on the threads):
+// after each block barrier of the cell pipeline ("slot") the threads combine the sub-batch that landed in one
+// buffer and store it, and thread 0 starts the copies of the next sub-batch into the other buffer (all threads
+// finished reading that one before the barrier).  Slice and element counts are 32-bit (the host falls back to a
+// separate pass when a chunk has 2^31 or more double2 elements).
 template <int NT, int IM>
 struct InitAhead {
-  static constexpr int KB = 8;       // IM = 2: slices per batch (4*KB registers of loads in flight)
+  static constexpr int KB = 4;       // IM = 2, start-up only: slices per register batch
+  static constexpr int SB = 3;       // IM = 2: slices per staged sub-batch
+  static constexpr int STAGE_BYTES = (IM == 2) ? 2 * 2 * SB * NT * 16 + 16 : 0;   // two buffers x (Z, W) + two mbarriers
   static constexpr int NW = NT / 32;
+  double2* stage = nullptr; uint64_t* fbar = nullptr;
+  int cur = 0; uint32_t par0 = 0, par1 = 0;
+  // per buffer: chunk, slices (0 = empty), valid elements of the last slice, where its first slice goes in Z
+  int bc0 = 0, bc1 = 0; unsigned bn0 = 0, bn1 = 0, vl0 = 0, vl1 = 0; double2* gz0 = nullptr; double2* gz1 = nullptr;
   const InitParams& I;
   const int tid, last;               // last chunk index
   unsigned len_reg = 0, len_last = 0;   // double2 elements per regular / last chunk
@@ -164,35 +173,100 @@ struct InitAhead {
     asm volatile("atom.global.add.u32 %0, [%1], %2;" : "=r"(r) : "l"(I.slice_ctr + c), "r"((unsigned)per_item(c)) : "memory");
     return r;
   }
-  // all threads, once the reservation has been broadcast (s0 = first slice)
+  // thread 0, as soon as a reservation is known (most of an item before its slices are staged): pull them into L2,
+  // so that the staging copies, which are issued only one slot ahead, do not wait for DRAM
+  __device__ __forceinline__ void prefetch_l2(int c, unsigned s0) const {
+    if (IM != 2 || c > last) return;
+    const unsigned ns = nslices(c);
+    if (s0 >= ns) return;
+    const unsigned s1 = s0 + per_item(c) < ns ? s0 + per_item(c) : ns;
+    const unsigned n = len(c), e0 = s0 * NT, e1 = s1 * NT < n ? s1 * NT : n;
+    const uint32_t bytes = (e1 - e0) * 16u;
+    if (I.mode == INIT_AXPBY)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(Z2 + begin(c) + e0), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(W2 + begin(c) + e0), "r"(bytes) : "memory");
+  }
+  // all threads, once the reservation has been broadcast (s0 = first slice); right after a block barrier.
+  // IM = 2: the sub-batch in flight belongs to the previous hand-out and is finished first, so that a block never
+  // has more than one chunk waiting for publication.
   __device__ __forceinline__ void accept(int c, unsigned s0) {
     if (IM == 0) return;
+    if (IM == 2) { slot_process(); while (busy()) { slot_issue(); __syncthreads(); slot_process(); } }
     note(c > last ? -2 : c, 0u);   // the block has moved on: what it did for the previous chunk becomes publishable
     if (c > last) { c_cur = -1; s_cur = s_end = 0; return; }
     const unsigned ns = nslices(c);
     c_cur = c; s_cur = s0 < ns ? s0 : ns;
     s_end = s0 + per_item(c) < ns ? s0 + per_item(c) : ns;
   }
-  // next batch of the accepted slices: IM = 1 does all of them now; IM = 2 starts the loads of up to KB slices
+  // IM = 1: all accepted slices now (stores only)
   __device__ __forceinline__ void batch_begin() {
-    if (IM == 0 || s_cur >= s_end) { pend = 0; return; }
-    if (IM == 1) {
-      zero_slices(c_cur, s_cur, s_end, 1u);
-      note(c_cur, s_end - s_cur);
-      s_cur = s_end;
-    } else {
-      start_loads(c_cur, s_cur, s_end, 1u);
-    }
+    if (IM != 1 || s_cur >= s_end) return;
+    zero_slices(c_cur, s_cur, s_end, 1u);
+    note(c_cur, s_end - s_cur);
+    s_cur = s_end;
   }
-  __device__ __forceinline__ void batch_end() {
-    if (IM != 2 || pend == 0) return;
-    finish_loads(c_cur, s_cur, 1u);
-    note(c_cur, (unsigned)pend);
-    s_cur += pend; pend = 0;
-  }
-  __device__ __forceinline__ void drain() {   // whatever two batches did not cover
+  // IM = 2: shared-memory staging.  init_stage() once (thread 0 initialises the mbarriers; a block barrier follows).
+  __device__ __forceinline__ void init_stage(unsigned char* smem) {
     if (IM != 2) return;
-    while (s_cur < s_end) { batch_begin(); batch_end(); }
+    stage = reinterpret_cast<double2*>(smem);
+    fbar = reinterpret_cast<uint64_t*>(smem + 2 * 2 * SB * NT * 16);
+    if (tid == 0) { mbar_init(fbar, 1); mbar_init(fbar + 1, 1); }
+  }
+  __device__ __forceinline__ double2* zbuf(int b) const { return stage + (size_t)b * 2 * SB * NT; }
+  __device__ __forceinline__ double2* wbuf(int b) const { return zbuf(b) + SB * NT; }
+  // all threads, right AFTER a block barrier: combine + store the sub-batch that landed in buffer `cur`, start the
+  // copies of the next one into the other buffer, swap
+  __device__ __forceinline__ void slot() { slot_process(); slot_issue(); }
+  __device__ __forceinline__ void slot_process() {
+    if (IM != 2) return;
+    const unsigned bn = cur ? bn1 : bn0;
+    if (bn == 0) return;
+    mbar_wait(fbar + cur, cur ? par1 : par0);
+    if (cur) par1 ^= 1u; else par0 ^= 1u;
+    double2* z = (cur ? gz1 : gz0) + tid;                       // this thread's element of the first slice, in Z
+    const double2* zs = zbuf(cur) + tid; const double2* ws = wbuf(cur) + tid;
+    const unsigned vl = cur ? vl1 : vl0;                         // valid elements of the LAST slice (others are full)
+    const double be = I.beta, ga = I.gamma;
+    const bool axpby = (I.mode == INIT_AXPBY);
+#pragma unroll
+    for (int k = 0; k < SB; ++k) {
+      if ((unsigned)k >= bn) break;
+      if ((unsigned)k + 1 == bn && (unsigned)tid >= vl) break;
+      const double2 w = ws[k * NT];
+      double2 r;
+      if (axpby) { const double2 o = zs[k * NT]; r.x = fma(be, o.x, ga * w.x); r.y = fma(be, o.y, ga * w.y); }
+      else { r.x = ga * w.x; r.y = ga * w.y; }
+      z[k * NT] = r;
+    }
+    note(cur ? bc1 : bc0, bn);
+    if (cur) bn1 = 0; else bn0 = 0;
+  }
+  __device__ __forceinline__ void slot_issue() {
+    if (IM != 2) return;
+    const int nb = cur ^ 1;
+    if (s_cur < s_end) {
+      const unsigned cnt = (s_end - s_cur < (unsigned)SB) ? s_end - s_cur : (unsigned)SB;
+      const unsigned n = len(c_cur), e0 = s_cur * NT;
+      const unsigned e1 = (e0 + cnt * NT < n) ? e0 + cnt * NT : n;
+      double2* zg = Z2 + begin(c_cur) + e0;
+      if (tid == 0) {
+        const uint32_t bytes = (e1 - e0) * 16u;
+        fence_async_smem();
+        mbar_expect_tx(fbar + nb, I.mode == INIT_AXPBY ? 2u * bytes : bytes);
+        if (I.mode == INIT_AXPBY) bulk_load(zbuf(nb), zg, bytes, fbar + nb);
+        bulk_load(wbuf(nb), W2 + begin(c_cur) + e0, bytes, fbar + nb);
+      }
+      const unsigned vl = e1 - e0 - (cnt - 1) * NT;
+      if (nb) { bc1 = c_cur; gz1 = zg; vl1 = vl; bn1 = cnt; } else { bc0 = c_cur; gz0 = zg; vl0 = vl; bn0 = cnt; }
+      s_cur += cnt;
+    }
+    cur = nb;
+  }
+  __device__ __forceinline__ bool busy() const { return IM == 2 && (s_cur < s_end || bn0 || bn1); }
+  // whatever the slots of an item did not cover (rare), and at kernel end the sub-batches still in flight
+  __device__ __forceinline__ void drain() {
+    if (IM != 2) return;
+    while (busy()) { __syncthreads(); slot(); }
   }
   // acquire: chunks c-1 and c are complete (called by all threads; the caller has a block barrier after it)
   __device__ __forceinline__ void wait_ready(int c) {

@@ -185,6 +185,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   const int layer_items = P.ncx * P.ncy * P.nvb;
   InitAhead<NT, IM> ia(I, P, PDEG, tid, layer_items);
 
+  ia.init_stage(smem_raw + 2 * TL::PITCH + 64);
   if (tid == 0) {
     mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -251,7 +252,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     // P2: z-lines (i1, i2 = k): T = Ns_z A -> A ; R = gm T + 4 gzz (DtD T)/4 -> B
     // (init-ahead: the zero stores, or the loads of a first batch, are issued here and fly during P2)
     // (the slices were reserved during the block's PREVIOUS item, so that the atomic's latency is never waited for)
-    if (init) { ia.accept(s_next[2], (unsigned)s_next[1]); ia.batch_begin(); }
+    if (init) { ia.accept(s_next[2], (unsigned)s_next[1]); ia.batch_begin(); ia.slot_issue(); }
     if (active) {
       double xn[N];   // software pipeline: the next line is in flight while this one is computed
 #pragma unroll
@@ -282,51 +283,56 @@ FE_ZLOOP_PRAGMA
         if (N & 1) b[H * S3] = fma(g4z, m2, gm * tq[H]);
       }
     }
-    if (init) ia.batch_end();
     __syncthreads();
+    ia.slot();
 
     // P3: xy-plane i3 = k: R += Kx T (rows) ; R += Ky T, Ns^T along y (columns) ; Ns^T along x (rows)
-    if (active) {
+    {
       const double* a = A + k * S3 + beta;
       double* b = B + k * S3 + beta;
       double r[N][N];
+      if (active) {
 #pragma unroll
-      for (int j = 0; j < N; ++j)
+        for (int j = 0; j < N; ++j)
 #pragma unroll
-        for (int i = 0; i < N; ++i) r[j][i] = b[j * S2 + i * S1];
+          for (int i = 0; i < N; ++i) r[j][i] = b[j * S2 + i * S1];
 #pragma unroll
-      for (int j = 0; j < N; ++j) {
-        double t[N], u2[HH], v2[HH], m2;
+        for (int j = 0; j < N; ++j) {
+          double t[N], u2[HH], v2[HH], m2;
 #pragma unroll
-        for (int i = 0; i < N; ++i) t[i] = a[j * S2 + i * S1];
-        eo_dtd<PDEG>(t, u2, v2, m2);
+          for (int i = 0; i < N; ++i) t[i] = a[j * S2 + i * S1];
+          eo_dtd<PDEG>(t, u2, v2, m2);
 #pragma unroll
-        for (int q = 0; q < H; ++q) {
-          r[j][q] = fma(g2x, u2[q] + v2[q], r[j][q]);
-          r[j][N - 1 - q] = fma(g2x, v2[q] - u2[q], r[j][N - 1 - q]);
+          for (int q = 0; q < H; ++q) {
+            r[j][q] = fma(g2x, u2[q] + v2[q], r[j][q]);
+            r[j][N - 1 - q] = fma(g2x, v2[q] - u2[q], r[j][N - 1 - q]);
+          }
+          if (N & 1) r[j][H] = fma(g2x, m2, r[j][H]);
         }
-        if (N & 1) r[j][H] = fma(g2x, m2, r[j][H]);
       }
+      if (IM == 2) { __syncthreads(); ia.slot(); }   // an extra slot for the staged initialisation (no tile hazard here)
+      if (active) {
 #pragma unroll
-      for (int i = 0; i < N; ++i) {
-        double t[N], c[N], u2[HH], v2[HH], m2, rp[HH], rm[HH], u[HH], v[HH], m;
+        for (int i = 0; i < N; ++i) {
+          double t[N], c[N], u2[HH], v2[HH], m2, rp[HH], rm[HH], u[HH], v[HH], m;
 #pragma unroll
-        for (int j = 0; j < N; ++j) { t[j] = a[j * S2 + i * S1]; c[j] = r[j][i]; }
-        eo_dtd<PDEG>(t, u2, v2, m2);
-        eo_split<N>(c, rp, rm);
+          for (int j = 0; j < N; ++j) { t[j] = a[j * S2 + i * S1]; c[j] = r[j][i]; }
+          eo_dtd<PDEG>(t, u2, v2, m2);
+          eo_split<N>(c, rp, rm);
 #pragma unroll
-        for (int q = 0; q < H; ++q) { rp[q] = fma(g4y, v2[q], rp[q]); rm[q] = fma(g4y, u2[q], rm[q]); }
-        const double rc = (N & 1) ? fma(g2y, m2, c[H]) : 0.0;
-        eo_mult<PDEG, MAT_NS, true, false>(rp, rm, rc, u, v, m);
-        eo_combine<N, false>(u, v, m, c);
+          for (int q = 0; q < H; ++q) { rp[q] = fma(g4y, v2[q], rp[q]); rm[q] = fma(g4y, u2[q], rm[q]); }
+          const double rc = (N & 1) ? fma(g2y, m2, c[H]) : 0.0;
+          eo_mult<PDEG, MAT_NS, true, false>(rp, rm, rc, u, v, m);
+          eo_combine<N, false>(u, v, m, c);
 #pragma unroll
-        for (int j = 0; j < N; ++j) r[j][i] = c[j];
-      }
+          for (int j = 0; j < N; ++j) r[j][i] = c[j];
+        }
 #pragma unroll
-      for (int j = 0; j < N; ++j) {
-        eo_full<PDEG, MAT_NS, true>(r[j], r[j]);
+        for (int j = 0; j < N; ++j) {
+          eo_full<PDEG, MAT_NS, true>(r[j], r[j]);
 #pragma unroll
-        for (int i = 0; i < N; ++i) b[j * S2 + i * S1] = r[j][i];
+          for (int i = 0; i < N; ++i) b[j * S2 + i * S1] = r[j][i];
+        }
       }
     }
     __syncthreads();
@@ -334,7 +340,7 @@ FE_ZLOOP_PRAGMA
     if (tid == 0) {
       const int nxt = (int)(gridDim.x + nxt_raw);
       *s_next = nxt;
-      if (init) { s_next[1] = (int)sl0; s_next[2] = ez + LOOK; }
+      if (init) { s_next[1] = (int)sl0; s_next[2] = ez + LOOK; ia.prefetch_l2(ez + LOOK, sl0); }
       if (nxt < nitems) {
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
@@ -342,8 +348,8 @@ FE_ZLOOP_PRAGMA
         tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + org);
       }
     }
+    ia.slot();
     // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
-    if (init) ia.batch_begin();
     if (active) {
       double xn[N];
 #pragma unroll
@@ -369,14 +375,11 @@ FE_ZLOOP_PRAGMA
         for (int j = 0; j < N; ++j) b[j * S3] = x[j];
       }
     }
-    if (init) {
-      ia.batch_end();
-      ia.drain();
-      ia.wait_ready(ez + 1);   // the planes this cell adds into are initialised
-    }
+    ia.wait_ready(ez + 1);   // the planes this cell adds into are initialised
     fence_async_smem();
     __syncthreads();
     ia.publish_point();
+    ia.slot();
     if (special) plane_wrap_fixup<PDEG, BV, NT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
     if (tid == 0) {
       tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
@@ -385,8 +388,10 @@ FE_ZLOOP_PRAGMA
     item = *s_next;   // written before the barrier that ended P4
   }
   if (init) {   // the slices reserved during the last item
+    __syncthreads();
     ia.accept(s_next[2], (unsigned)s_next[1]);
-    ia.batch_begin(); ia.batch_end(); ia.drain();
+    ia.batch_begin();
+    ia.drain();
   }
   ia.finish();
   if (tid == 0) tma_wait_all0();
