@@ -91,14 +91,13 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
-      v2 x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u1[HH], v1[HH], m1, u2[HH], vv[HH], m2;
+      v2 x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u2[HH], vv[HH], m2;
       lds_line2<N>(A + base + b2, stride, x);
       eo_split<N>(x, xp, xm);
       eo_mult<PDEG, MAT_NS, false, false>(xp, xm, x[H], u, v, m);
       eo_combine<N, false>(u, v, m, tq);
       sts_line2<N>(A + base + b2, stride, tq);
-      eo_mult<PDEG, MAT_DS, false, true>(u, v, m, u1, v1, m1);
-      eo_mult<PDEG, MAT_DS, true, true>(v1, u1, m1, u2, vv, m2);
+      eo_dtd_eo<PDEG>(u, v, m, u2, vv, m2);
       v2 r[N];
 #pragma unroll
       for (int q = 0; q < H; ++q) {

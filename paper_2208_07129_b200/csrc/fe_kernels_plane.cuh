@@ -38,7 +38,7 @@ struct EoTab2 {
   double midm, midmh;       // M[mid][mid] and half of it
   double pad[2];
 };
-__constant__ EoTab2 c_eo2[KMAXN][2];   // [p][MAT_NS | MAT_DS]
+__constant__ EoTab2 c_eo2[KMAXN][3];   // [p][MAT_NS | MAT_DS | MAT_SH]
 
 // The primitives are generic in the value type T: double (one vector per thread, plane kernels) or v2 (two
 // vectors per thread, line kernels).
@@ -107,15 +107,26 @@ __device__ __forceinline__ void eo_full(const T (&x)[PDEG + 1], T (&y)[PDEG + 1]
   eo_combine<N, MAT == MAT_DS>(u, v, m, y);
 }
 
-// (u2, v2, m2) = HALF of the even/odd parts of Ds^T Ds t, from the line t.
+// (u2, v2, m2) = HALF of the even/odd parts of Ds^T Ds t, from the line t, in the convention of an
+// anti-symmetric-type product: y_q = 2 (u2_q + v2_q), y_{n-1-q} = 2 (v2_q - u2_q), y_mid = 2 m2.
+// On Cartesian cells the metric factor is constant along a line, so Ds^T g Ds = g (Ds^T Ds) and the 1D operator
+// S/2 = Ds^T Ds / 2 (host-precomputed like D = D~ N of PAPER.md:188; symmetric type) is applied as ONE contraction.
 template <int PDEG, typename T>
 __device__ __forceinline__ void eo_dtd(const T (&t)[PDEG + 1], T (&u2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
                                        T (&v2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], T& m2) {
   constexpr int N = PDEG + 1, HH = N / 2 > 0 ? N / 2 : 1;
-  T tp[HH], tm[HH], u1[HH], v1[HH], m1;
+  T tp[HH], tm[HH];
   eo_split<N>(t, tp, tm);
-  eo_mult<PDEG, MAT_DS, false, false>(tp, tm, t[N / 2], u1, v1, m1);
-  eo_mult<PDEG, MAT_DS, true, true>(v1, u1, m1, u2, v2, m2);
+  eo_mult<PDEG, MAT_SH, false, false>(tp, tm, t[N / 2], v2, u2, m2);   // (u, v) of a symmetric type swap roles
+}
+// The same from the even/odd parts (u, v, m) of t itself (as eo_mult leaves them: half of x+ / x-): QUARTER of
+// the even/odd parts of Ds^T Ds t.
+template <int PDEG, typename T>
+__device__ __forceinline__ void eo_dtd_eo(const T (&u)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                          const T (&v)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], T m,
+                                          T (&u2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1],
+                                          T (&v2)[(PDEG + 1) / 2 > 0 ? (PDEG + 1) / 2 : 1], T& m2) {
+  eo_mult<PDEG, MAT_SH, false, true>(u, v, m, v2, u2, m2);
 }
 
 // Periodic wrap fix-ups of the last cell in a direction, done cooperatively on the shared-memory tile so that
@@ -261,7 +272,7 @@ FE_ZLOOP_PRAGMA
       for (int i = 0; i < N; ++i) {
         double* a = A + k * S2 + i * S1 + beta;
         double* b = B + k * S2 + i * S1 + beta;
-        double x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u1[HH], v1[HH], m1, u2[HH], v2[HH], m2;
+        double x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u2[HH], v2[HH], m2;
 #pragma unroll
         for (int j = 0; j < N; ++j) x[j] = xn[j];
         if (i + 1 < N) {
@@ -273,8 +284,7 @@ FE_ZLOOP_PRAGMA
         eo_combine<N, false>(u, v, m, tq);
 #pragma unroll
         for (int j = 0; j < N; ++j) a[j * S3] = tq[j];
-        eo_mult<PDEG, MAT_DS, false, true>(u, v, m, u1, v1, m1);      // half of Ds T
-        eo_mult<PDEG, MAT_DS, true, true>(v1, u1, m1, u2, v2, m2);    // quarter of Ds^T Ds T
+        eo_dtd_eo<PDEG>(u, v, m, u2, v2, m2);                          // quarter of Ds^T Ds T
 #pragma unroll
         for (int q = 0; q < H; ++q) {
           b[q * S3] = fma(g4z, u2[q] + v2[q], gm * tq[q]);

@@ -65,9 +65,9 @@ struct DeviceGuard {
 
 // Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
 // 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
-void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4], fe::EoTab2 out2[2]) {
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4], fe::EoTab2 out2[3]) {
   const int n = t.n, h = n / 2, m = n / 2;
-  long double M[4][fe::MAXN * fe::MAXN];
+  long double M[5][fe::MAXN * fe::MAXN];
   for (int q = 0; q < n; ++q)
     for (int i = 0; i < n; ++i) {
       const long double sq = sqrtl(t.wl[q]), si = sqrtl(t.wl[i]);
@@ -76,23 +76,35 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4], fe::EoTab2 out2[2])
       M[0][q * n + i] = ns; M[1][i * n + q] = ns;
       M[2][q * n + i] = ds; M[3][i * n + q] = ds;
     }
-  for (int k = 0; k < 4; ++k) {
-    std::memset(&out[k], 0, sizeof(fe::EoTab));
+  // M[4] = Ds^T Ds / 2: the 1D stiffness operator at the quadrature points that the Cartesian kernels apply as ONE
+  // even-odd contraction (constant diagonal metric: Ds^T g Ds = g Ds^T Ds); symmetric and centro-symmetric
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) {
+      long double acc = 0.0L;
+      for (int q = 0; q < n; ++q) acc += M[2][q * n + i] * M[2][q * n + j];
+      M[4][i * n + j] = 0.5L * acc;
+    }
+  fe::EoTab tabs[5];
+  for (int k = 0; k < 5; ++k) {
+    std::memset(&tabs[k], 0, sizeof(fe::EoTab));
     for (int q = 0; q < h; ++q) {
       for (int i = 0; i < h; ++i) {
-        out[k].P[q * h + i] = (double)(0.5L * (M[k][q * n + i] + M[k][q * n + (n - 1 - i)]));
-        out[k].Mn[q * h + i] = (double)(0.5L * (M[k][q * n + i] - M[k][q * n + (n - 1 - i)]));
+        tabs[k].P[q * h + i] = (double)(0.5L * (M[k][q * n + i] + M[k][q * n + (n - 1 - i)]));
+        tabs[k].Mn[q * h + i] = (double)(0.5L * (M[k][q * n + i] - M[k][q * n + (n - 1 - i)]));
       }
-      if (n & 1) out[k].Pm[q] = (double)M[k][q * n + m];
+      if (n & 1) tabs[k].Pm[q] = (double)M[k][q * n + m];
     }
     if (n & 1) {
-      for (int i = 0; i < h; ++i) out[k].mid[i] = (double)M[k][m * n + i];
-      out[k].midm = (double)M[k][m * n + m];
+      for (int i = 0; i < h; ++i) tabs[k].mid[i] = (double)M[k][m * n + i];
+      tabs[k].midm = (double)M[k][m * n + m];
     }
   }
-  // the plane kernels' tables: Ns and Ds only (the transposes reuse them), plus the halved middle column / row
-  for (int k2 = 0; k2 < 2; ++k2) {
-    const fe::EoTab& s = out[2 * k2];
+  for (int k = 0; k < 4; ++k) out[k] = tabs[k];
+  // the plane / line kernels' tables: Ns, Ds (the transposes reuse them) and Ds^T Ds / 2, plus the halved middle
+  // column / row
+  const int src[3] = {0, 2, 4};
+  for (int k2 = 0; k2 < 3; ++k2) {
+    const fe::EoTab& s = tabs[src[k2]];
     fe::EoTab2& d = out2[k2];
     std::memset(&d, 0, sizeof(fe::EoTab2));
     for (int i = 0; i < 16; ++i) { d.P[i] = s.P[i]; d.Mn[i] = s.Mn[i]; }
@@ -161,10 +173,10 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
   if (e == cudaSuccess) {
     fe::EoTab eo[4];
-    fe::EoTab2 eo2[2];
+    fe::EoTab2 eo2[3];
     make_eo_tables(tab, eo, eo2);
     e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 4 * p);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 2 * p);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 3 * p);
   }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
 
