@@ -285,7 +285,9 @@ def run_ours(args):
     roof = {"bound": "alu", "achieved": achieved_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved_tf / fp64_peak,
             "traffic": traffic, "kernel": op.kernel_name(nvec), "kernel_ms": ms_kernel,
             "peak_source": "fe_probe_peaks: FP64 FMA chain measured live in this run (burst)",
-            "flop_convention": "2 x algorithmic FP64 instructions of the even-odd method (%.1f instr, %.1f flops per DoF*vec)" % (slots, flops),
+            "flop_convention": "2 x algorithmic FP64 instructions of the plain even-odd method (%.1f instr, %.1f flops per DoF*vec); the kernel may execute fewer (executed_fp64_instr_per_dof_vec, DESIGN.md section 5)" % (slots, flops),
+            "executed_fp64_instr_per_dof_vec": (roofline.executed_instr_per_dof_vec_cartesian(w.p)
+                                                if op.kernel_name(nvec) in ("fe_apply_cart_plane", "fe_apply_cart_line") else None),
             "t_roof_ms": t_roof * 1e3, "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
             "frac_of_t_roof": t_roof * 1e3 / ms_kernel,
             "hbm": {"achieved": count * roofline.bytes_per_dof_vec(w.p, w.geom == inputs.GEOM_QPOINT, bv) / (ms_kernel * 1e-3) / 1e9,

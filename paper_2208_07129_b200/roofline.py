@@ -41,6 +41,22 @@ def work_per_dof_vec(p: int, diagonal_metric: bool, even_odd: bool = True):
     return (fma + other) / p ** 3, (2 * fma + other) / p ** 3
 
 
+def executed_instr_per_dof_vec_cartesian(p: int) -> float:
+    """FP64 instructions the Cartesian plane / line kernels actually execute per DoF*vector:
+    even/odd operators chained without combine+split, Ds^T g Ds applied as the one precomputed 1D operator
+    g * (Ds^T Ds).  Per line of n points: split 2h, combine 2h, mult = h(h+odd) + h^2 + odd(1+h)."""
+    n = p + 1
+    h, odd = n // 2, n % 2
+    split = comb = 2 * h
+    mult = h * (h + odd) + h * h + odd * (1 + h)
+    full = split + mult + comb                                  # one complete even-odd contraction
+    pass_z = split + mult + comb + mult + 6 * h + 2 * odd       # N_z, T, R = gm T + g S T
+    kterm = split + mult + 4 * h + odd                          # R += g S T
+    cols = split + mult + split + (2 * h + odd) + mult + comb   # R += g S T accumulated in the even/odd basis, N^T
+    per_line = 2 * full + pass_z + kterm + cols + 2 * full
+    return per_line * n * n / p ** 3
+
+
 def bytes_per_dof_vec(p: int, per_qpoint_geometry: bool, bv: int, chebyshev: bool = False) -> float:
     n = p + 1
     b = 24.0 if chebyshev else 16.0
