@@ -146,7 +146,7 @@ template <> struct GenCfg<4> { static constexpr int BV = 8, NT = 128, MINB = 3; 
 template <> struct GenCfg<5> { static constexpr int BV = 8, NT = 160, MINB = 2; };
 template <> struct GenCfg<6> { static constexpr int BV = 8, NT = 128, MINB = 3; };
 template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 256, MINB = 1; };
-template <> struct GenCfg<8> { static constexpr int BV = 8, NT = 384, MINB = 1; };
+template <> struct GenCfg<8> { static constexpr int BV = 8, NT = 352, MINB = 1; };
 constexpr int kGenBv = 8;
 
 template <int PDEG>

@@ -27,13 +27,13 @@ struct EoTab {
   double midm;
   double pad[3];
 };
-enum { EO_NS = 0, EO_NST = 1, EO_DS = 2, EO_DST = 3 };
-__constant__ EoTab c_eo[KMAXN][4];
+enum { EO_NS = 0, EO_NST = 1, EO_DS = 2, EO_DST = 3, EO_SH = 4 };   // EO_SH: Ds^T Ds / 2 (symmetric type)
+__constant__ EoTab c_eo[KMAXN][5];
 
 template <int PDEG, int KIND>
 __device__ __forceinline__ void eo_apply(const double (&x)[PDEG + 1], double (&y)[PDEG + 1]) {
   constexpr int N = PDEG + 1, H = N / 2;
-  constexpr bool ODD = (N & 1) != 0, ANTI = (KIND >= 2);
+  constexpr bool ODD = (N & 1) != 0, ANTI = (KIND == EO_DS || KIND == EO_DST);
   const EoTab& t = c_eo[PDEG][KIND];
   double xp[H > 0 ? H : 1], xm[H > 0 ? H : 1];
 #pragma unroll
@@ -65,18 +65,17 @@ __device__ __forceinline__ void eo_apply(const double (&x)[PDEG + 1], double (&y
   }
 }
 
-// r += Ds^T (g * (Ds t)) : one direction of the stiffness term at the quadrature points (Alg. 2 l.2-9
-// restricted to a diagonal metric entry g, constant along the line).
+// r += Ds^T (g * (Ds t)) : one direction of the stiffness term at the quadrature points (Alg. 2 l.2-9 restricted to
+// a diagonal metric entry g that is constant along the line, so that Ds^T g Ds = 2g (Ds^T Ds / 2): ONE contraction
+// with the host-precomputed 1D operator, as in fe_kernels_plane.cuh).
 template <int PDEG>
 __device__ __forceinline__ void kterm(const double (&t)[PDEG + 1], double (&r)[PDEG + 1], double g) {
   constexpr int N = PDEG + 1;
-  double a[N], b[N];
-  eo_apply<PDEG, EO_DS>(t, a);
+  double b[N];
+  eo_apply<PDEG, EO_SH>(t, b);
+  const double g2 = 2.0 * g;
 #pragma unroll
-  for (int i = 0; i < N; ++i) a[i] *= g;
-  eo_apply<PDEG, EO_DST>(a, b);
-#pragma unroll
-  for (int i = 0; i < N; ++i) r[i] += b[i];
+  for (int i = 0; i < N; ++i) r[i] = fma(g2, b[i], r[i]);
 }
 
 // Shared-memory tile layout [i3][i2][i1][beta] with the x-line pitch padded by one node when n is even and

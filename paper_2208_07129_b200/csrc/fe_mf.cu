@@ -65,7 +65,7 @@ struct DeviceGuard {
 
 // Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
 // 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
-void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4], fe::EoTab2 out2[3]) {
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[3]) {
   const int n = t.n, h = n / 2, m = n / 2;
   long double M[5][fe::MAXN * fe::MAXN];
   for (int q = 0; q < n; ++q)
@@ -99,7 +99,7 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[4], fe::EoTab2 out2[3])
       tabs[k].midm = (double)M[k][m * n + m];
     }
   }
-  for (int k = 0; k < 4; ++k) out[k] = tabs[k];
+  for (int k = 0; k < 5; ++k) out[k] = tabs[k];
   // the plane / line kernels' tables: Ns, Ds (the transposes reuse them) and Ds^T Ds / 2, plus the halved middle
   // column / row
   const int src[3] = {0, 2, 4};
@@ -172,10 +172,10 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_D, tab.Dt, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
   if (e == cudaSuccess) {
-    fe::EoTab eo[4];
+    fe::EoTab eo[5];
     fe::EoTab2 eo2[3];
     make_eo_tables(tab, eo, eo2);
-    e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 4 * p);
+    e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 5 * p);
     if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 3 * p);
   }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
