@@ -173,6 +173,33 @@ def test_few_vectors_cells_as_slots(env, p, bc, nc, nvec):
     check_apply(env, w)
 
 
+def test_cuda_graph_capture(env):
+    """The entry points only enqueue work on the caller's stream (no host synchronisation, no allocation after the
+    first call): an apply and a filter can be captured in a CUDA graph and replayed (config 1 is launch-bound)."""
+    torch, orc, binding = env
+    w = inputs.configs()[1]
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    oo = orc.Operator(oracle_mesh(orc, w), w.sigma)
+    Yo = oo.apply(X)
+    Fo = orc.chebyshev_filter(oo.apply, X, 4, 50.0, 400.0, 0.0)
+    op = binding.FeMf.from_workload(w)
+    Xd = torch.from_numpy(X).cuda(); Yd = torch.empty_like(Xd); Xf = Xd.clone(); Yf = torch.empty_like(Xd)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        op.apply(Xd, Yd, w.nvec, stream=s); op.cheb_filter(Xf, Yf, w.nvec, 4, 50.0, 400.0, 0.0, stream=s)   # warm-up (function attributes)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        Xf.copy_(Xd)
+        with torch.cuda.graph(g, stream=s):
+            op.apply(Xd, Yd, w.nvec, stream=s)
+            op.cheb_filter(Xf, Yf, w.nvec, 4, 50.0, 400.0, 0.0, stream=s)
+        Yd.fill_(float("nan")); Yf.fill_(float("nan")); Xf.copy_(Xd)
+        g.replay()
+        s.synchronize()
+    assert relerr(Yd.cpu().numpy(), Yo) <= TOL
+    assert relerr(Yf.cpu().numpy(), Fo) <= TOL
+
+
 def test_apply_host_path(env):
     torch, orc, binding = env
     for nvec in (3, 32):
