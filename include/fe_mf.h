@@ -74,7 +74,9 @@ long long fe_mf_ndofs(const fe_mf_ctx *ctx);
  *   Y_dev  DEVICE, overwritten, same shape; must not alias X_dev.
  *   nvec   >= 1.
  *   cuda_stream  a cudaStream_t (NULL = default stream).  All work is enqueued on it; the call
- *                does not synchronise the host.
+ *                does not synchronise the host (it can be captured in a CUDA graph after a first call).
+ *                A context owns the work counters of its persistent kernels: calls on ONE context must be
+ *                stream-ordered (use one context per stream for concurrent applies).
  * Errors: EINVAL (null pointers, nvec < 1, aliasing), ECUDA.
  */
 int fe_mf_apply(fe_mf_ctx *ctx, const double *X_dev, double *Y_dev, int nvec, void *cuda_stream);
