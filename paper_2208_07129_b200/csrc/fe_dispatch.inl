@@ -172,13 +172,13 @@ template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 
 template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };   // spills; kept for comparison
 bool plane_ok(int p) { return p == 6 || p == 7; }
 
-template <int PDEG, int IM>
+template <int PDEG, int IM, bool IDENT = false>
 cudaError_t launch_plane_im(fe_mf_ctx* c, const fe::ApplyParams& prm, fe::InitParams init, const CUtensorMap& tw,
                             const CUtensorMap& tz, cudaStream_t st) {
   using C = PlaneCfg<PDEG>;
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64 + fe::InitAhead<C::NT, IM>::STAGE_BYTES;
   static int bps = 0;
-  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IM>;
+  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IM, IDENT>;
   long long grid = 0;
   int nitems = (int)(c->ncells * prm.nvb);
   cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
@@ -197,6 +197,7 @@ cudaError_t launch_plane_im(fe_mf_ctx* c, const fe::ApplyParams& prm, fe::InitPa
 template <int PDEG>
 cudaError_t launch_plane(fe_mf_ctx* c, const fe::ApplyParams& prm, const fe::InitParams& init, const CUtensorMap& tw,
                          const CUtensorMap& tz, cudaStream_t st) {
+  if (init.mode == fe::INIT_NONE && prm.idw != 0.0) return launch_plane_im<PDEG, 0, true>(c, prm, init, tw, tz, st);
   if (init.mode == fe::INIT_NONE) return launch_plane_im<PDEG, 0>(c, prm, init, tw, tz, st);
   if (init.mode == fe::INIT_ZERO) return launch_plane_im<PDEG, 1>(c, prm, init, tw, tz, st);
   return launch_plane_im<PDEG, 2>(c, prm, init, tw, tz, st);
@@ -292,6 +293,7 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.nsm = c->nsm;
   P.geom_stride = c->geom_stride;
   P.item_ctr = reinterpret_cast<int*>(c->ctrl);
+  P.idw = 0.0;
   return P;
 }
 
@@ -300,6 +302,10 @@ bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
   const long long chunk2 = (long long)(c->p + 1) * c->ndx * c->ndy * nvec / 2;   // double2 elements of the largest chunk
   return kind == 8 && c->coop && c->variant == 19 && chunk2 < (1LL << 31);
 }
+
+// Can this kernel add a multiple of W (identity term, partition-of-unity weights) in the same pass?  The p = 6 plane
+// kernel on periodic meshes: on a Dirichlet mesh the boundary nodes never enter a tile.
+bool kind_adds_identity(const fe_mf_ctx* c, int kind) { return kind == 8 && c->p == 6 && c->bc == FE_BC_PERIODIC && c->variant != 8; }
 
 #define FE_DISPATCH_P(CALL)                                           \
   switch (c->p) {                                                     \
@@ -311,11 +317,13 @@ bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
 
 // Z += alpha * A * W  (Z already initialised), or with init.mode != INIT_NONE (only if kind_fuses_init):
 // Z <- beta Z + gamma W + alpha A W in ONE launch.  Counts launches into c->last_launches.
+// idw != 0 (only if kind_adds_identity): Z += alpha A W + idw W in one launch.
 int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st,
-                      fe::InitParams init = fe::InitParams{fe::INIT_NONE, 0.0, 0.0, nullptr, nullptr}) {
+                      fe::InitParams init = fe::InitParams{fe::INIT_NONE, 0.0, 0.0, nullptr, nullptr}, double idw = 0.0) {
   const int kind = pick_kernel(c, nvec, W, Z);
   const int bv = kernel_bv(c, kind, nvec);
   fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
+  P.idw = idw;
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
   CUtensorMap tw, tz;
@@ -453,6 +461,45 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
   double alpha1 = sigma1 / e;
   double alpha2 = -c;
   double* X = X_dev; double* Y = Y_dev;
+  if (m <= 200 && c != 0.0 && kind_adds_identity(ctx, pick_kernel(ctx, nvec, X_dev, Y_dev))) {
+    // The same recurrence, X_1 = a_0 (A - cI) X_0, X_{k+1} = a_k (A - cI) X_k + b_k X_{k-1}  (a_0 = sigma_1/e,
+    // a_k = 2 sigma_2/e, b_k = -sigma sigma_2), in the scaled variables X_k = s_k U_k with s_0 = s_1 = 1,
+    // s_{k+1} = b_k s_{k-1}:   U_{k+1} = U_{k-1} + (a_k s_k / s_{k+1}) (A - cI) U_k.
+    // Every step is then ONE accumulate launch into the buffer of U_{k-1} (the plane kernel adds the -cI part with
+    // partition-of-unity weights): no axpby pass.  s_m and s_{m-1} are applied once at the end.  (|s_k| shrinks
+    // like |b|^(k/2); m <= 200 keeps it far from underflow.)
+    const fe::InitParams none{fe::INIT_NONE, 0.0, 0.0, nullptr, nullptr};
+    FE_CUDA(ctx, cudaMemsetAsync(Y, 0, count * sizeof(double), st));
+    ctx->last_launches = 0;
+    rc = launch_accumulate(ctx, alpha1, X, Y, nvec, st, none, -c * alpha1);
+    if (rc) return rc;
+    launches += ctx->last_launches;
+    double s_prev = 1.0, s_cur = 1.0;
+    double* Uprev = X; double* Ucur = Y;
+    for (int d = 2; d <= m; ++d) {
+      const double sigma2 = 1.0 / (gamma - sigma);
+      alpha1 = 2.0 * sigma2 / e;
+      alpha2 = -sigma * sigma2;
+      const double s_next = alpha2 * s_prev;
+      const double al = alpha1 * s_cur / s_next;
+      ctx->last_launches = 0;
+      rc = launch_accumulate(ctx, al, Ucur, Uprev, nvec, st, none, -c * al);
+      if (rc) return rc;
+      launches += ctx->last_launches;
+      double* t = Uprev; Uprev = Ucur; Ucur = t;
+      s_prev = s_cur; s_cur = s_next;
+      sigma = sigma2;
+    }
+    // Y_dev <- s_m U_m, X_dev <- s_{m-1} U_{m-1}
+    const int swap = (Ucur != Y_dev) ? 1 : 0;
+    if (swap || s_cur != 1.0 || s_prev != 1.0) {
+      fe::fe_scale2_kernel<<<stream_grid(count), 256, 0, st>>>(X_dev, Y_dev, s_prev, s_cur, swap, count);
+      FE_CUDA(ctx, cudaGetLastError());
+      launches += 1;
+    }
+    ctx->last_launches = launches;
+    return FE_MF_OK;
+  }
   // line 10: Y <- alpha1 A X + alpha1 alpha2 X
   rc = fe_mf_apply_axpby(ctx, alpha1, X, 0.0, alpha1 * alpha2, Y, nvec, cuda_stream);
   if (rc) return rc;

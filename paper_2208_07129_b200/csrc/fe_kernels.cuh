@@ -31,6 +31,7 @@ struct ApplyParams {
   int nsm;                        // SM count (persistent kernels)
   long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
   int* item_ctr;                  // persistent kernels: work counter (0 at launch); item = gridDim.x + atomicAdd after the first
+  double idw;                     // plane kernel with IDENT (periodic meshes): Z += alpha A W + idw W
 };
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.
@@ -184,6 +185,18 @@ __global__ void fe_scale_copy_kernel(double* __restrict__ Z, const double* __res
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t k = i; k < count; k += stride) Z[k] = gamma * W[k];
+}
+
+// A <- sa * A, B <- sb * B (swap = 0) or A <- sa * B_old, B <- sb * A_old (swap = 1): the end of the scaled
+// Chebyshev recurrence (fe_cheb_filter).
+__global__ void fe_scale2_kernel(double* __restrict__ A, double* __restrict__ B, double sa, double sb, int swap, size_t count) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t k = i; k < count; k += stride) {
+    const double a = A[k], b = B[k];
+    A[k] = sa * (swap ? b : a);
+    B[k] = sb * (swap ? a : b);
+  }
 }
 
 __global__ void fe_swap_kernel(double* __restrict__ A, double* __restrict__ B, size_t count) {

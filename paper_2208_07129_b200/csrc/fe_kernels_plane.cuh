@@ -168,7 +168,11 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
 // Z (+)= A W on uniform Cartesian cells (diagonal constant metric; alpha folded into P.ug).  One block = one
 // cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta.  With I.mode != INIT_NONE the
 // kernel also initialises Z (fe_init_ahead.cuh) and must be launched cooperatively.
-template <int PDEG, int BV, int NT, int MINB, int IM>
+// IDENT (periodic meshes): Z += alpha A W + idw W in the same pass.  The identity part is added cell by cell with
+// partition-of-unity weights (a node on a cell face in a direction is shared by two cells: weight 1/2 per
+// direction) in P4, on the nodal result, from the nodal values of W re-read through L2 (the tile that held them was
+// transformed in place).  The shifted operator A - cI of the Chebyshev recurrence then costs no separate pass.
+template <int PDEG, int BV, int NT, int MINB, int IM, bool IDENT>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                     const __grid_constant__ ApplyParams P, const __grid_constant__ InitParams I, int nitems) {
@@ -361,20 +365,40 @@ FE_ZLOOP_PRAGMA
     ia.slot();
     // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
     if (active) {
-      double xn[N];
+      double xn[N], wn[N];
 #pragma unroll
       for (int j = 0; j < N; ++j) xn[j] = B[k * S2 + beta + j * S3];
+      // IDENT: the z-line (i1, i2 = k) of W in global memory: node (ix, iy, ez p + j), periodic wrap
+      const bool wlive = IDENT && (v0 + beta) < P.nvec;
+      const long long zstep = (long long)P.ndx * P.ndy * P.nvec;
+      int iyw = ey * PDEG + k; if (iyw >= P.ndy) iyw -= P.ndy;
+      const double* wrow = P.W + ((long long)iyw * P.ndx + (long long)ez * PDEG * P.ndx * P.ndy) * P.nvec + v0 + beta;
+      const long long zwrap = wz ? (long long)P.ndz * zstep : 0;   // subtracted at j = N-1 in the last layer
+      const double wk = (k == 0 || k == N - 1) ? 0.5 * P.idw : P.idw;
+      auto load_w = [&](int i1, double (&w)[N]) {
+        int ixw = ex * PDEG + i1; if (ixw >= P.ndx) ixw -= P.ndx;
+        const double* q = wrow + (long long)ixw * P.nvec;
+#pragma unroll
+        for (int j = 0; j < N; ++j) w[j] = wlive ? __ldg(q + j * zstep - (j == N - 1 ? zwrap : 0)) : 0.0;
+      };
+      if (IDENT) load_w(0, wn);
 FE_ZLOOP_PRAGMA
       for (int i = 0; i < N; ++i) {
         double* b = B + k * S2 + i * S1 + beta;
-        double x[N];
+        double x[N], w[N];
 #pragma unroll
-        for (int j = 0; j < N; ++j) x[j] = xn[j];
+        for (int j = 0; j < N; ++j) { x[j] = xn[j]; if (IDENT) w[j] = wn[j]; }
         if (i + 1 < N) {
 #pragma unroll
           for (int j = 0; j < N; ++j) xn[j] = b[S1 + j * S3];
+          if (IDENT) load_w(i + 1, wn);
         }
         eo_full<PDEG, MAT_NS, true>(x, x);
+        if (IDENT) {
+          const double wi = (i == 0 || i == N - 1) ? 0.5 * wk : wk;
+#pragma unroll
+          for (int j = 0; j < N; ++j) x[j] = fma((j == 0 || j == N - 1) ? 0.5 * wi : wi, w[j], x[j]);
+        }
         if (dlow) {
           const bool zl = (ey == 0 && k == 0) || (ex == 0 && i == 0);
 #pragma unroll

@@ -147,6 +147,28 @@ def test_apply_axpby(env):
         assert np.array_equal(Wd.cpu().numpy(), W)
 
 
+@pytest.mark.parametrize("nvec", [16, 28])
+@pytest.mark.parametrize("m", [1, 2, 3, 8, 21])
+def test_chebyshev_scaled_recurrence_plane_kernel(env, m, nvec):
+    """p = 6, periodic (wrap in every direction), full and partial vector blocks: every filter step is one accumulate
+    launch of the plane kernel, which adds the -c I part itself (partition-of-unity weights), in the scaled
+    variables U_k = X_k / s_k."""
+    torch, orc, binding = env
+    w = inputs.Workload("cheb_plane", 6, (3, 2, 4), inputs.BC_PERIODIC, inputs.GEOM_AFFINE, 1.0, (0, 0, 0), (7.5, 5.0, 10.0),
+                        nvec, 77)
+    op_o = orc.Operator(oracle_mesh(orc, w), w.sigma)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    a, b, a0 = 1.0, 3.0, -0.05
+    Yo = orc.chebyshev_filter(op_o.apply, X, m, a, b, a0)
+    Xprev = orc.chebyshev_filter(op_o.apply, X, m - 1, a, b, a0) if m > 1 else X
+    op = binding.FeMf.from_workload(w)
+    Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
+    op.cheb_filter(Xd, Yd, w.nvec, m, a, b, a0); torch.cuda.synchronize()
+    assert relerr(Yd.cpu().numpy(), Yo) <= TOL
+    assert relerr(Xd.cpu().numpy(), Xprev) <= TOL           # X holds iterate m-1 (header contract)
+    assert op.last_launch_count() <= m + 1                  # m accumulate launches + one final scaling
+
+
 @pytest.mark.parametrize("m", [1, 2, 3, 6])
 def test_chebyshev_small_degrees_and_x_scratch(env, m):
     torch, orc, binding = env
