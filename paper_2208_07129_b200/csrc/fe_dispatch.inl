@@ -423,6 +423,17 @@ extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_d
     fe::InitParams init{beta == 0.0 ? (gamma == 0.0 ? fe::INIT_ZERO : fe::INIT_SCALE) : fe::INIT_AXPBY, beta, gamma, nullptr, nullptr};
     return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st, init);
   }
+  if (kind_adds_identity(ctx, kind) && gamma != 0.0) {
+    // the kernel adds gamma W itself (IDENT): the separate pass only has to scale Z (or zero it)
+    if (beta == 0.0) {
+      FE_CUDA(ctx, cudaMemsetAsync(Z_dev, 0, count * sizeof(double), st));
+    } else if (beta != 1.0) {
+      fe::fe_scale_kernel<<<stream_grid(count / 2 + 1), 256, 0, st>>>(Z_dev, beta, count);
+      FE_CUDA(ctx, cudaGetLastError());
+      ctx->last_launches += 1;
+    }
+    return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st, fe::InitParams{fe::INIT_NONE, 0.0, 0.0, nullptr, nullptr}, gamma);
+  }
   rc = launch_init(ctx, Z_dev, W_dev, beta, gamma, count, st);
   if (rc) return rc;
   return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st);

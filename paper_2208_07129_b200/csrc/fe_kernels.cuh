@@ -187,6 +187,14 @@ __global__ void fe_scale_copy_kernel(double* __restrict__ Z, const double* __res
   for (size_t k = i; k < count; k += stride) Z[k] = gamma * W[k];
 }
 
+__global__ void fe_scale_kernel(double* Z, double beta, size_t count) {   // Z <- beta Z
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  double2* Z2 = reinterpret_cast<double2*>(Z);
+  for (size_t k = i; k < count / 2; k += stride) { double2 z = Z2[k]; z.x *= beta; z.y *= beta; Z2[k] = z; }
+  if (i == 0 && (count & 1)) Z[count - 1] *= beta;
+}
+
 // A <- sa * A, B <- sb * B (swap = 0) or A <- sa * B_old, B <- sb * A_old (swap = 1): the end of the scaled
 // Chebyshev recurrence (fe_cheb_filter).
 __global__ void fe_scale2_kernel(double* __restrict__ A, double* __restrict__ B, double sa, double sb, int swap, size_t count) {
