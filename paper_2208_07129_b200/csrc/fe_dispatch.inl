@@ -231,14 +231,14 @@ int line_bv(const fe_mf_ctx* c, int nvec) {
 // 8-vector blocks with an even number of nodes per direction: one pad node per x-row (see DenseTile)
 constexpr int line_padx(int p, int bv) { return (bv == 8 && (p + 1) % 2 == 0 && p >= 3) ? 1 : 0; }
 
-template <int PDEG, int CFG>
-cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+template <int PDEG, int CFG, bool IDENT = false>
+cudaError_t launch_line_id(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                         cudaStream_t st) {
   using C = LineCfg<CFG>;
   constexpr int PADX = line_padx(PDEG, C::BV);
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV, PADX>::PITCH + 64;
   static int bps = 0;
-  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB, PADX>;
+  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB, PADX, IDENT>;
   const long long nitems = c->ncells * prm.nvb;
   long long grid = 0;
   cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
@@ -246,6 +246,12 @@ cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CU
   if (e != cudaSuccess) return e;
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
+}
+
+template <int PDEG, int CFG>
+cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                        cudaStream_t st) {
+  return prm.idw != 0.0 ? launch_line_id<PDEG, CFG, true>(c, prm, tw, tz, st) : launch_line_id<PDEG, CFG, false>(c, prm, tw, tz, st);
 }
 
 // ---- which kernel serves (ctx, nvec, pointers)
@@ -303,9 +309,10 @@ bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
   return kind == 8 && c->coop && c->variant == 19 && chunk2 < (1LL << 31);
 }
 
-// Can this kernel add a multiple of W (identity term, partition-of-unity weights) in the same pass?  The p = 6 plane
-// kernel on periodic meshes: on a Dirichlet mesh the boundary nodes never enter a tile.
-bool kind_adds_identity(const fe_mf_ctx* c, int kind) { return kind == 8 && c->p == 6 && c->bc == FE_BC_PERIODIC && c->variant != 8; }
+// Can this kernel add a multiple of W (identity term, partition-of-unity weights) in the same pass?  The Cartesian
+// plane and line kernels, at every node they write: all nodes on periodic meshes, the interior nodes on Dirichlet
+// meshes (the boundary nodes never enter a tile: callers treat them separately).
+bool kind_adds_identity(const fe_mf_ctx* c, int kind) { return (kind == 8 && c->p == 6) || kind == 9; }
 
 #define FE_DISPATCH_P(CALL)                                           \
   switch (c->p) {                                                     \
@@ -423,7 +430,7 @@ extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_d
     fe::InitParams init{beta == 0.0 ? (gamma == 0.0 ? fe::INIT_ZERO : fe::INIT_SCALE) : fe::INIT_AXPBY, beta, gamma, nullptr, nullptr};
     return launch_accumulate(ctx, alpha, W_dev, Z_dev, nvec, st, init);
   }
-  if (kind_adds_identity(ctx, kind) && gamma != 0.0) {
+  if (kind_adds_identity(ctx, kind) && gamma != 0.0 && ctx->bc == FE_BC_PERIODIC) {
     // the kernel adds gamma W itself (IDENT): the separate pass only has to scale Z (or zero it)
     if (beta == 0.0) {
       FE_CUDA(ctx, cudaMemsetAsync(Z_dev, 0, count * sizeof(double), st));
@@ -478,7 +485,9 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
     // s_{k+1} = b_k s_{k-1}:   U_{k+1} = U_{k-1} + (a_k s_k / s_{k+1}) (A - cI) U_k.
     // Every step is then ONE accumulate launch into the buffer of U_{k-1} (the plane kernel adds the -cI part with
     // partition-of-unity weights): no axpby pass.  s_m and s_{m-1} are applied once at the end.  (|s_k| shrinks
-    // like |b|^(k/2); m <= 200 keeps it far from underflow.)
+    // like |b|^(k/2); m <= 200 keeps it far from underflow.)  Dirichlet meshes: the kernels neither read nor write
+    // the boundary nodes, whose entries obey the scalar recurrence with A = 0 (q_k); X_dev keeps the input there
+    // until the final kernel writes q_m x0 and q_{m-1} x0.
     const fe::InitParams none{fe::INIT_NONE, 0.0, 0.0, nullptr, nullptr};
     FE_CUDA(ctx, cudaMemsetAsync(Y, 0, count * sizeof(double), st));
     ctx->last_launches = 0;
@@ -486,6 +495,7 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
     if (rc) return rc;
     launches += ctx->last_launches;
     double s_prev = 1.0, s_cur = 1.0;
+    double q_prev = 1.0, q_cur = -c * alpha1;   // the same recurrence at a boundary node of a Dirichlet mesh: (A X) = 0 there
     double* Uprev = X; double* Ucur = Y;
     for (int d = 2; d <= m; ++d) {
       const double sigma2 = 1.0 / (gamma - sigma);
@@ -493,6 +503,8 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
       alpha2 = -sigma * sigma2;
       const double s_next = alpha2 * s_prev;
       const double al = alpha1 * s_cur / s_next;
+      const double q_next = -c * alpha1 * q_cur + alpha2 * q_prev;
+      q_prev = q_cur; q_cur = q_next;
       ctx->last_launches = 0;
       rc = launch_accumulate(ctx, al, Ucur, Uprev, nvec, st, none, -c * al);
       if (rc) return rc;
@@ -503,8 +515,10 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
     }
     // Y_dev <- s_m U_m, X_dev <- s_{m-1} U_{m-1}
     const int swap = (Ucur != Y_dev) ? 1 : 0;
-    if (swap || s_cur != 1.0 || s_prev != 1.0) {
-      fe::fe_scale2_kernel<<<stream_grid(count), 256, 0, st>>>(X_dev, Y_dev, s_prev, s_cur, swap, count);
+    const int bnd = (ctx->bc == FE_BC_DIRICHLET) ? 1 : 0;
+    if (swap || bnd || s_cur != 1.0 || s_prev != 1.0) {
+      fe::fe_scale2_kernel<<<stream_grid(count), 256, 0, st>>>(X_dev, Y_dev, s_prev, s_cur, swap, count, bnd, q_prev, q_cur,
+                                                               ctx->ndx, ctx->ndy, ctx->ndz, nvec);
       FE_CUDA(ctx, cudaGetLastError());
       launches += 1;
     }

@@ -195,13 +195,23 @@ __global__ void fe_scale_kernel(double* Z, double beta, size_t count) {   // Z <
   if (i == 0 && (count & 1)) Z[count - 1] *= beta;
 }
 
-// A <- sa * A, B <- sb * B (swap = 0) or A <- sa * B_old, B <- sb * A_old (swap = 1): the end of the scaled
-// Chebyshev recurrence (fe_cheb_filter).
-__global__ void fe_scale2_kernel(double* __restrict__ A, double* __restrict__ B, double sa, double sb, int swap, size_t count) {
+// The end of the scaled Chebyshev recurrence (fe_cheb_filter): A <- sa * A, B <- sb * B (swap = 0) or
+// A <- sa * B_old, B <- sb * A_old (swap = 1).  On a Dirichlet mesh (bnd = 1) the kernels never touch the boundary
+// nodes, whose entries follow the scalar recurrence: there A still holds the input x0, and A <- qa x0, B <- qb x0.
+__global__ void fe_scale2_kernel(double* __restrict__ A, double* __restrict__ B, double sa, double sb, int swap, size_t count,
+                                 int bnd, double qa, double qb, int ndx, int ndy, int ndz, int nvec) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t k = i; k < count; k += stride) {
     const double a = A[k], b = B[k];
+    if (bnd) {
+      const size_t node = k / (size_t)nvec;
+      const int ix = (int)(node % ndx), iy = (int)((node / ndx) % ndy), iz = (int)(node / ((size_t)ndx * ndy));
+      if (ix == 0 || ix == ndx - 1 || iy == 0 || iy == ndy - 1 || iz == 0 || iz == ndz - 1) {
+        A[k] = qa * a; B[k] = qb * a;
+        continue;
+      }
+    }
     A[k] = sa * (swap ? b : a);
     B[k] = sb * (swap ? a : b);
   }

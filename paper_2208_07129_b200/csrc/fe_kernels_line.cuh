@@ -12,7 +12,9 @@
 
 namespace fe {
 
-template <int PDEG, int BV, int NT, int MINB, int PADX>
+// IDENT: Z += alpha A W + idw W in the same pass (see fe_apply_cart_plane): the identity part is added in ph6 on
+// the nodal result, with partition-of-unity weights, from the nodal values of W re-read through L2.
+template <int PDEG, int BV, int NT, int MINB, int PADX, bool IDENT>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                    const __grid_constant__ ApplyParams P, int nitems) {
@@ -168,9 +170,33 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
-      v2 x[N];
+      v2 x[N], wv[N];
+      if (IDENT) {   // the z-line (i1, i2) of W in global memory (issued first: in flight during the contraction)
+        const int i1 = l % N, i2 = l / N;
+        int ixw = ex * PDEG + i1, iyw = ey * PDEG + i2;
+        if (ixw >= P.ndx) ixw -= P.ndx;
+        if (iyw >= P.ndy) iyw -= P.ndy;
+        const bool wlive = (v0 + b2) < P.nvec;
+        const long long zstep = (long long)P.ndx * P.ndy * P.nvec;
+        const double* q = P.W + ((long long)ixw + (long long)P.ndx * ((long long)iyw + (long long)P.ndy * ez * PDEG)) * P.nvec + v0 + b2;
+        const long long zwrap = wz ? (long long)P.ndz * zstep : 0;
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+          double2 d = make_double2(0.0, 0.0);
+          if (wlive) d = __ldg(reinterpret_cast<const double2*>(q + j * zstep - (j == N - 1 ? zwrap : 0)));
+          wv[j] = {d.x, d.y};
+        }
+      }
       lds_line2<N>(B + base + b2, stride, x);
       eo_full<PDEG, MAT_NS, true>(x, x);
+      if (IDENT) {
+        const int i1 = l % N, i2 = l / N;
+        double wl = P.idw;
+        if (i1 == 0 || i1 == N - 1) wl *= 0.5;
+        if (i2 == 0 || i2 == N - 1) wl *= 0.5;
+#pragma unroll
+        for (int j = 0; j < N; ++j) x[j] = vfma((j == 0 || j == N - 1) ? 0.5 * wl : wl, wv[j], x[j]);
+      }
       if (dlow) {
         const int i1 = l % N, i2 = l / N;
         if ((ex == 0 && i1 == 0) || (ey == 0 && i2 == 0)) {

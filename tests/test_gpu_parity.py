@@ -147,6 +147,28 @@ def test_apply_axpby(env):
         assert np.array_equal(Wd.cpu().numpy(), W)
 
 
+@pytest.mark.parametrize("p,bc,nc,nvec", [(7, inputs.BC_PERIODIC, (2, 3, 2), 12), (7, inputs.BC_DIRICHLET, (3, 2, 2), 8),
+                                          (6, inputs.BC_DIRICHLET, (2, 2, 4), 16), (4, inputs.BC_DIRICHLET, (3, 3, 3), 6),
+                                          (5, inputs.BC_PERIODIC, (2, 2, 3), 20), (8, inputs.BC_DIRICHLET, (2, 2, 2), 4)])
+@pytest.mark.parametrize("m", [1, 2, 7])
+def test_chebyshev_scaled_recurrence_all_cartesian_kernels(env, m, p, bc, nc, nvec):
+    """The one-launch-per-step filter on the line kernels (even and odd n, 8- and 16-vector blocks, pad-node tiles)
+    and on Dirichlet meshes, where the boundary entries follow the scalar recurrence (closed form at the end)."""
+    torch, orc, binding = env
+    w = inputs.Workload("cheb_line", p, nc, bc, inputs.GEOM_AFFINE, 0.8, (0, 0, 0), (4.0, 6.0, 5.0), nvec, 500 + p)
+    op_o = orc.Operator(oracle_mesh(orc, w), w.sigma)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    a, b, a0 = 1.5, 12.0, -0.2
+    Yo = orc.chebyshev_filter(op_o.apply, X, m, a, b, a0)
+    Xprev = orc.chebyshev_filter(op_o.apply, X, m - 1, a, b, a0) if m > 1 else X
+    op = binding.FeMf.from_workload(w)
+    Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
+    op.cheb_filter(Xd, Yd, w.nvec, m, a, b, a0); torch.cuda.synchronize()
+    assert relerr(Yd.cpu().numpy(), Yo) <= TOL
+    assert relerr(Xd.cpu().numpy(), Xprev) <= TOL
+    assert op.last_launch_count() <= m + 1
+
+
 @pytest.mark.parametrize("nvec", [16, 28])
 @pytest.mark.parametrize("m", [1, 2, 3, 8, 21])
 def test_chebyshev_scaled_recurrence_plane_kernel(env, m, nvec):
