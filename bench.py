@@ -37,6 +37,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cheb", action="store_true", help="skip the Chebyshev-filter leg (config 5, 1024 vectors, m = 20)")
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other degrees (configs 3 and 4)")
     return ap.parse_args()
 
 
@@ -261,6 +262,39 @@ def run_ours(args):
         except Exception as exc:   # e.g. not enough free memory on a shared device
             cheb = {"error": str(exc)[:200]}
 
+    # ---- the other degrees of the metric ("per degree p"): configs 3 (p = 8, per-q-point) and 4 (p = 7), short runs;
+    #      context only -- the bench line is config 2
+    others = None
+    if rank == 0 and world == 1 and not args.no_others and args.config == 2:
+        others = []
+        for cfg_o, nv_o in ((3, 16), (4, 32), (4, 1)):
+            try:
+                wo = inputs.configs()[cfg_o]
+                opo = binding.FeMf.from_workload(wo, device=local)
+                no = wo.ndof * nv_o
+                Xo = torch.empty(no, dtype=torch.float64, device="cuda"); Yo_ = torch.empty_like(Xo)
+                binding.fill_uniform(Xo, wo.seed)
+                for _ in range(3):
+                    opo.apply(Xo, Yo_, nv_o)
+                ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                ev[0].record(stream)
+                for _ in range(10):
+                    opo.apply(Xo, Yo_, nv_o)
+                ev[1].record(stream)
+                for _ in range(10):
+                    opo.accumulate(1.0, Xo, Yo_, nv_o)
+                ev[2].record(stream)
+                torch.cuda.synchronize()
+                t_apply, t_kern = ev[0].elapsed_time(ev[1]) / 10, ev[1].elapsed_time(ev[2]) / 10
+                so, _ = roofline.work_per_dof_vec(wo.p, wo.geom == inputs.GEOM_AFFINE)
+                others.append({"workload": wo.name, "p": wo.p, "nvec": nv_o, "kernel": opo.kernel_name(nv_o),
+                               "value": no / (t_apply * 1e-3) / 1e9, "kernel_only": no / (t_kern * 1e-3) / 1e9,
+                               "kernel_ms": t_kern, "frac": no * so * 2.0 / (t_kern * 1e-3) / 1e12 / fp64_peak})
+                del Xo, Yo_, opo
+                torch.cuda.empty_cache()
+            except Exception as exc:
+                others.append({"config": cfg_o, "error": str(exc)[:200]})
+
     # ---- roofline of the dominant kernel
     diag = (w.geom == inputs.GEOM_AFFINE)
     bv = op.batch_width(nvec)
@@ -324,7 +358,7 @@ def run_ours(args):
                "data": "synthetic", "config": config_dict(w, nvec, {"bv": bv, "variant": args.variant,
                                                                      "sharding": "vector columns, no collective"}),
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roof,
-               "cpu_baseline": cpu, "chebyshev": cheb}
+               "cpu_baseline": cpu, "chebyshev": cheb, "other_configs": others}
         print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
