@@ -146,7 +146,7 @@ template <> struct GenCfg<4> { static constexpr int BV = 8, NT = 128, MINB = 3; 
 template <> struct GenCfg<5> { static constexpr int BV = 8, NT = 160, MINB = 2; };
 template <> struct GenCfg<6> { static constexpr int BV = 8, NT = 128, MINB = 3; };
 template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 256, MINB = 1; };
-template <> struct GenCfg<8> { static constexpr int BV = 8, NT = 352, MINB = 1; };
+template <> struct GenCfg<8> { static constexpr int BV = 4, NT = 192, MINB = 2; };
 constexpr int kGenBv = 8;
 
 template <int PDEG>
@@ -280,7 +280,7 @@ int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
     case 1: return general_bv(c->p, nvec);
     case 2: return 8;
     case 3: return nvec;
-    case 6: return kGenBv;
+    case 6: return c->p == 8 ? 4 : kGenBv;
     case 8: return 16;
     default: return line_bv(c, nvec);
   }
