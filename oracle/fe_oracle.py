@@ -19,6 +19,12 @@ element matrices, exactly integrated Kronecker closed form on Cartesian meshes, 
 K*1 = 0, 1^T M 1 = |Omega|, exact polynomial energies, patch test on the perturbed mesh,
 long-double brute force on a single cell, Chebyshev closed form T_m, Lanczos bound >= lambda_max,
 the paper's printed DoF counts.  Nothing here is "parity unpinned".
+
+SURVEY.md §8(f) NEXT-1 pieces (pins in tests/test_oracle_mass_scaled.py): kappa given at the quadrature points
+(`Operator(kappa=...)`), the GLL-lumped mass diagonal (`lumped_mass_diagonal`) and
+H~ = M^-1/2 (K + M^kappa) M^-1/2 (`Operator.apply_mass_scaled`, Eq. B.1).  Pinned by
+printed Lobatto weights, the rule's exactness, sum M_ii = |Omega|, lumped = row sums of the consistent mass,
+closed-form moments of a bilinear kappa, the p = 1 Fourier closed form and the Laplacian spectrum on a periodic cube.
 """
 from __future__ import annotations
 
@@ -68,6 +74,14 @@ def gll_nodes(p: int) -> np.ndarray:
     # enforce exact anti-symmetry of the node set
     x = (x - x[::-1]) / LD(2)
     return x
+
+
+def gll_weights(p: int) -> np.ndarray:
+    """Weights of the (p+1)-point Gauss-Lobatto-Legendre rule: w_i = 2 / (p (p+1) P_p(xi_i)^2) (long double)."""
+    x = gll_nodes(p)
+    pn, _ = _legendre(p, x)
+    w = LD(2) / (LD(p) * LD(p + 1) * pn * pn)
+    return (w + w[::-1]) / LD(2)
 
 
 def gauss_legendre(n: int):
@@ -192,8 +206,9 @@ def trilinear_map(verts8: np.ndarray, pts: np.ndarray):
     return x, J
 
 
-def geometric_factors(verts8: np.ndarray, qpts: np.ndarray, W: np.ndarray, sigma: float):
-    """G[s][d][Q] = (J^-1 J^-T)_sd det J w_Q (mu = 1) and g[Q] = sigma det J w_Q."""
+def geometric_factors(verts8: np.ndarray, qpts: np.ndarray, W: np.ndarray, sigma):
+    """G[s][d][Q] = (J^-1 J^-T)_sd det J w_Q (mu = 1) and g[Q] = kappa_Q det J w_Q (Eq. 22
+    PAPER.md:336-341): sigma is the constant kappa of the Helmholtz operator or an array kappa_Q of n_q^3 values."""
     _, J = trilinear_map(verts8, qpts)
     det = np.linalg.det(J)
     if np.any(det <= 0.0):
@@ -292,24 +307,65 @@ class Mesh:
         return out
 
 
+def quadrature_point_coordinates(mesh: Mesh) -> np.ndarray:
+    """(ncells, n_q^3, 3) physical coordinates x_Q^(e) of the quadrature points, cells in
+    lexicographic order (x fastest), Q = q1 + n q2 + n^2 q3."""
+    qp, _ = reference_points_3d(mesh.p)
+    ncx, ncy, ncz = mesh.ncells
+    out = np.zeros((ncx * ncy * ncz, mesh.n ** 3, 3))
+    for ez in range(ncz):
+        for ey in range(ncy):
+            for ex in range(ncx):
+                out[ex + ncx * (ey + ncy * ez)], _ = trilinear_map(mesh.cell_vertices(ex, ey, ez), qp)
+    return out
+
+
+def lumped_mass_diagonal(mesh: Mesh) -> np.ndarray:
+    """diag(M) with the overlap integrals evaluated by the GLL rule on the nodes themselves:
+    M_ii = sum over the cells that contain node i of det J(xi_i) w_i1 w_i2 w_i3.  Dirichlet boundary nodes keep
+    their entry (they are masked by the operator anyway)."""
+    w1 = gll_weights(mesh.p).astype(np.float64)
+    n = mesh.n
+    I = np.arange(n ** 3)
+    w3 = w1[I % n] * w1[(I // n) % n] * w1[I // (n * n)]
+    _, gl = reference_points_3d(mesh.p)
+    M = np.zeros(mesh.ndof)
+    for ez in range(mesh.ncells[2]):
+        for ey in range(mesh.ncells[1]):
+            for ex in range(mesh.ncells[0]):
+                idx, _ = mesh.cell_dofs(ex, ey, ez)
+                _, J = trilinear_map(mesh.cell_vertices(ex, ey, ez), gl)
+                np.add.at(M, idx, np.linalg.det(J) * w3)
+    return M
+
+
 class Operator:
     """A = K + sigma*M on a Mesh by the cell-matrix method (PAPER.md:134-143 steps 1-4).
 
     split=(ck, cm) scales the stiffness and mass parts (pins use (1,0) and (0,1)); the default is
     K + sigma M."""
 
-    def __init__(self, mesh: Mesh, sigma: float, ck: float = 1.0, cm: float = 1.0, form_matrices: bool = False):
+    def __init__(self, mesh: Mesh, sigma: float, ck: float = 1.0, cm: float = 1.0, form_matrices: bool = False,
+                 kappa=None):
+        """kappa: None (constant sigma) or an array [ncells][n_q^3] of values at the quadrature points of every cell
+        (cells in lexicographic order, x fastest; Eq. 22, the "precomputed potential" of
+        PAPER.md:796), which then replaces sigma."""
         self.mesh, self.sigma, self.ck, self.cm = mesh, float(sigma), float(ck), float(cm)
+        self.kappa = None if kappa is None else np.asarray(kappa, dtype=np.float64).reshape(
+            mesh.ncells[0] * mesh.ncells[1] * mesh.ncells[2], (mesh.p + 1) ** 3)
         self.Nf, self.Df, self.W = tables_3d(mesh.p)
         self.qpts, _ = reference_points_3d(mesh.p)
         self.form_matrices = form_matrices
         self._Ae_uniform = None
-        if mesh.vertices is None:
+        if mesh.vertices is None and self.kappa is None:
             # every cell of a uniform Cartesian mesh has the same A_e: a property of the input
             self._Ae_uniform = self.cell_matrix(0, 0, 0)
 
     def _factors(self, ex, ey, ez):
-        G, g = geometric_factors(self.mesh.cell_vertices(ex, ey, ez), self.qpts, self.W, self.sigma)
+        kap = self.sigma
+        if self.kappa is not None:
+            kap = self.kappa[ex + self.mesh.ncells[0] * (ey + self.mesh.ncells[1] * ez)]
+        G, g = geometric_factors(self.mesh.cell_vertices(ex, ey, ez), self.qpts, self.W, kap)
         return self.ck * G, self.cm * g
 
     def cell_matrix(self, ex, ey, ez) -> np.ndarray:
@@ -347,6 +403,14 @@ class Operator:
                         V[mask] = 0.0                            # C^T: boundary rows dropped
                     Y[idx] += V                                  # Q^(e)T: assembly (idx unique per cell)
         return Y
+
+    def apply_mass_scaled(self, X: np.ndarray, d: np.ndarray) -> np.ndarray:
+        """H~ X = M^-1/2 (K + M^kappa) M^-1/2 X with d = diag(M)^-1/2 of the GLL-lumped mass matrix
+        (Eq. 26; Eq. B.1 PAPER.md:1171 with a = 1, b = c = 0)."""
+        X = np.asarray(X, dtype=np.float64)
+        if X.ndim == 1:
+            return d * self.apply(d * X)
+        return d[:, None] * self.apply(d[:, None] * X)
 
     def apply_at_nodes(self, x_rows, nodes) -> np.ndarray:
         """Rows `nodes` of Y = A X without forming X: x_rows(idx) must return X[idx] (len(idx), nvec).
