@@ -131,6 +131,27 @@ int fe_fill_uniform(double *out_dev, long long count, unsigned long long seed, l
                     void *cuda_stream);
 
 /*
+ * the operator of the paper's eigenproblem benchmark:
+ *   H = K + M^kappa with kappa(x) given at the quadrature points, and H~ = M^-1/2 H M^-1/2 with M the mass matrix
+ *   evaluated by the (p+1)-point Gauss-Lobatto-Legendre rule on the nodes, hence diagonal.
+ *
+ * fe_mf_set_kappa: kappa_host is a HOST array [ncells][n^3] (cells x fastest, point Q = q1 + n q2 + n^2 q3 at the
+ *   Gauss points of the cell: kappa_Q = kappa(x_Q)), copied; it replaces sigma in every later call
+ *   (G_QQ = kappa_Q det J w_Q).  NULL restores the constant sigma.  The context must have been created
+ *   with FE_GEOM_QPOINT (the mesh may still be the uniform box), else EINVAL.
+ * fe_mf_set_mass_scaling: on != 0 makes fe_mf_apply / fe_mf_apply_axpby / fe_cheb_filter / fe_mf_apply_host act
+ *   with H~ instead of H: Z = alpha M^-1/2 H M^-1/2 W + beta Z + gamma W (Eq. B.1); the diagonal
+ *   scaling is done inside the kernel at extraction and assembly, not in extra passes.  Runs on
+ *   the full-metric kernels.  Dirichlet boundary entries of M are computed like all others and never used.
+ * fe_mf_mass_diagonal: writes diag(M) (HOST array of fe_mf_ndofs doubles, node order of the multivector rows) so
+ *   that the caller can map U = M^-1/2 U~.
+ * All three synchronise the device (they are setup calls, not stream-ordered) and return FE_MF_* codes.
+ */
+int fe_mf_set_kappa(fe_mf_ctx *ctx, const double *kappa_host);
+int fe_mf_set_mass_scaling(fe_mf_ctx *ctx, int on);
+int fe_mf_mass_diagonal(fe_mf_ctx *ctx, double *out_host);
+
+/*
  * fe_probe_peaks -- box peaks for the roofline (BASELINE.json north_star: "peaks measured on the box
  * by a stream/DGEMM microbenchmark"): FP64 FMA-chain rate in TFLOP/s (2 flops per DFMA) and FP64
  * stream-copy bandwidth in GB/s (read + write bytes), best of 5 after one warm-up, on cuda_device's

@@ -37,6 +37,9 @@ SYMBOLS = {
     "fe_mf_kernel_name": (C.c_char_p, [C.c_void_p, C.c_int]),
     "fe_mf_last_launch_count": (C.c_int, [C.c_void_p]),
     "fe_mf_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
+    "fe_mf_set_kappa": (C.c_int, [C.c_void_p, _PD]),
+    "fe_mf_set_mass_scaling": (C.c_int, [C.c_void_p, C.c_int]),
+    "fe_mf_mass_diagonal": (C.c_int, [C.c_void_p, _PD]),
     "fe_mf_last_error": (C.c_char_p, [C.c_void_p]),
     "fe_mf_destroy": (None, [C.c_void_p]),
 }
@@ -105,6 +108,7 @@ class FeMf:
             raise FeMfError(rc, self._l.fe_mf_last_error(None).decode())
         self.ndofs = int(self._l.fe_mf_ndofs(self._ctx))
         self.p, self.device = int(p), int(device)
+        self.ncells = tuple(int(c) for c in ncells)
 
     @classmethod
     def from_workload(cls, w, device: int = 0) -> "FeMf":
@@ -155,6 +159,25 @@ class FeMf:
 
     def set_variant(self, variant: int):
         self._raise(self._l.fe_mf_set_variant(self._ctx, int(variant)))
+
+    def set_kappa(self, kappa):
+        """kappa at the quadrature points, host array [ncells][n^3] (or None: back to the constant sigma)."""
+        if kappa is None:
+            self._raise(self._l.fe_mf_set_kappa(self._ctx, None))
+            return
+        k = np.ascontiguousarray(kappa, dtype=np.float64)
+        n3 = (self.p + 1) ** 3
+        if k.size != self.ncells[0] * self.ncells[1] * self.ncells[2] * n3:
+            raise ValueError("kappa must have ncells * (p+1)^3 entries")
+        self._raise(self._l.fe_mf_set_kappa(self._ctx, k.ctypes.data_as(_PD)))
+
+    def set_mass_scaling(self, on: bool):
+        self._raise(self._l.fe_mf_set_mass_scaling(self._ctx, 1 if on else 0))
+
+    def mass_diagonal(self) -> np.ndarray:
+        out = np.empty(self.ndofs, dtype=np.float64)
+        self._raise(self._l.fe_mf_mass_diagonal(self._ctx, out.ctypes.data_as(_PD)))
+        return out
 
     def destroy(self):
         if getattr(self, "_ctx", None) and self._ctx.value:

@@ -149,14 +149,14 @@ template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 256, MINB = 1; 
 template <> struct GenCfg<8> { static constexpr int BV = 4, NT = 192, MINB = 2; };
 constexpr int kGenBv = 8;
 
-template <int PDEG>
+template <int PDEG, bool MSC = false>
 cudaError_t launch_gen(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                        cudaStream_t st) {
   using C = GenCfg<PDEG>;
   constexpr int NN = (PDEG + 1) * (PDEG + 1) * (PDEG + 1);
   constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, C::BV>::PITCH + ((size_t)7 * NN * 8 + 15) / 16 * 16 + 64;
   static int bps = 0;
-  auto kern = fe::fe_apply_gen_tma<PDEG, C::BV, C::NT, C::MINB>;
+  auto kern = fe::fe_apply_gen_tma<PDEG, C::BV, C::NT, C::MINB, MSC>;
   const long long nitems = c->ncells * prm.nvb;
   long long grid = 0;
   cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
@@ -257,7 +257,8 @@ cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CU
 // ---- which kernel serves (ctx, nvec, pointers)
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 1) return 1;
-  const bool diag = (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
+  const bool msc = c->mass_scaled;   // only the full-metric kernels (kinds 1, 6) apply M^-1/2
+  const bool diag = !msc && (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
   const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
   const bool tma_ok = !(nvec & 1) && aligned && encode_tiled_fn() &&
                       (unsigned long long)nvec * 8ULL * c->ndx * c->ndy < (1ULL << 40) &&
@@ -300,6 +301,7 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.geom_stride = c->geom_stride;
   P.item_ctr = reinterpret_cast<int*>(c->ctrl);
   P.idw = 0.0;
+  P.dscale = c->mass_scaled ? c->dscale_dev : nullptr;
   return P;
 }
 
@@ -343,7 +345,11 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
   }
   if (kind == 8 || kind == 9 || kind == 2 || kind == 3)
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // Cartesian kernels: the result is linear in the metric constants
-  if (kind == 6) {
+  if (kind == 6 && P.dscale) {
+#define FE_CALL(p_) launch_gen<p_, true>(c, P, tw, tz, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
+  } else if (kind == 6) {
 #define FE_CALL(p_) launch_gen<p_>(c, P, tw, tz, st)
     FE_DISPATCH_P(FE_CALL)
 #undef FE_CALL

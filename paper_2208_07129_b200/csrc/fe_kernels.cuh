@@ -32,6 +32,8 @@ struct ApplyParams {
   long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
   int* item_ctr;                  // persistent kernels: work counter (0 at launch); item = gridDim.x + atomicAdd after the first
   double idw;                     // plane kernel with IDENT (periodic meshes): Z += alpha A W + idw W
+  const double* dscale;           // nullptr, or d = diag(M)^-1/2 [ndof] of the GLL-lumped mass matrix: Z += alpha d.(A (d.W))
+                                  // (Eq. B.1; kernels of kinds 1 and 6 only)
 };
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.
@@ -100,7 +102,9 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
       if (iy >= P.ndy) iy -= P.ndy;
       if (iz >= P.ndz) iz -= P.ndz;
     }
-    T0[t] = live ? P.W[global_node(P, ix, iy, iz) * P.nvec + v0 + beta] : 0.0;
+    double xv = live ? P.W[global_node(P, ix, iy, iz) * P.nvec + v0 + beta] : 0.0;
+    if (P.dscale && live) xv *= __ldg(P.dscale + global_node(P, ix, iy, iz));   // M^-1/2 at extraction
+    T0[t] = xv;
   }
   __syncthreads();
   // S3 interpolate (Alg. 1)
@@ -159,7 +163,10 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
       if (iy >= P.ndy) iy -= P.ndy;
       if (iz >= P.ndz) iz -= P.ndz;
     }
-    if (live) atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], P.alpha * T0[t]);
+    if (live) {
+      const double dv = P.dscale ? __ldg(P.dscale + global_node(P, ix, iy, iz)) : 1.0;   // M^-1/2 at assembly
+      atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], P.alpha * (dv * T0[t]));
+    }
   }
 }
 

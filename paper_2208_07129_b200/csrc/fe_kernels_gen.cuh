@@ -20,7 +20,27 @@
 
 namespace fe {
 
-template <int PDEG, int BV, int NT, int MINB>
+// d at the N nodes of x-line l = i2 + N i3 of cell (ex,ey,ez), periodic indices wrapped
+template <int PDEG>
+__device__ __forceinline__ void load_dscale(const ApplyParams& P, int ex, int ey, int ez, int l, double* dn) {
+  constexpr int N = PDEG + 1;
+  int iy = ey * PDEG + l % N, iz = ez * PDEG + l / N;
+  if (iy >= P.ndy) iy -= P.ndy;
+  if (iz >= P.ndz) iz -= P.ndz;
+  const double* src = P.dscale + (long long)P.ndx * ((long long)iy + (long long)P.ndy * iz);
+  const int x0 = ex * PDEG;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    int ix = x0 + i;
+    if (ix >= P.ndx) ix -= P.ndx;
+    dn[i] = __ldg(src + ix);
+  }
+}
+
+// MSC: the mass-scaled operator Z += alpha d.(A (d.W)), d = diag(M)^-1/2 of the GLL-lumped mass matrix
+// (PAPER.md:925-929), applied where the paper applies it -- at extraction and assembly: ph0 scales
+// the x-lines it reads, ph8 the x-lines it writes; d is read through L2 (one value per node, shared by all vectors).
+template <int PDEG, int BV, int NT, int MINB, bool MSC>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                  const __grid_constant__ ApplyParams P, int nitems) {
@@ -115,6 +135,12 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
             x[N - 1] = {d.x, d.y};
           }
         }
+      }
+      if (MSC) {
+        double dn[N];
+        load_dscale<PDEG>(P, ex, ey, ez, l, dn);
+#pragma unroll
+        for (int i = 0; i < N; ++i) x[i] = vmul(dn[i], x[i]);
       }
       eo2<PDEG, MAT_NS, false>(x, y);
       sts_line2<N>(A + base + b2, stride, y);
@@ -254,8 +280,14 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N], y[N];
+      double dn[N];
+      if (MSC) load_dscale<PDEG>(P, ex, ey, ez, l, dn);
       lds_line2<N>(A + base + b2, stride, x);
       eo2<PDEG, MAT_NS, true>(x, y);
+      if (MSC) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) y[i] = vmul(dn[i], y[i]);
+      }
       if (special) {
         const int i2 = l % N, i3 = l / N;
         int iy = ey * PDEG + i2, iz = ez * PDEG + i3;

@@ -4,6 +4,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <string>
@@ -34,6 +35,13 @@ struct fe_mf_ctx {
   unsigned* ctrl = nullptr;
   size_t ctrl_bytes = 0;
   bool coop = false;           // cooperative launches supported
+  // kappa at the quadrature points and the mass-scaled operator
+  std::vector<double> verts;   // copy of vertices_host (empty: uniform box)
+  double lo[3] = {0, 0, 0}, h[3] = {1, 1, 1};
+  std::vector<double> detq;    // geom_mode 2: det J at the quadrature points [cell][n^3]
+  double* dscale_dev = nullptr;   // diag(M)^-1/2 of the GLL-lumped mass matrix [ndof]
+  std::vector<double> mass_diag;  // diag(M) [ndof] (host copy, filled with dscale_dev)
+  bool mass_scaled = false;
   int variant = 0;
   int last_launches = 0;
   // fe_mf_apply_host workspace
@@ -186,6 +194,11 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
     const int nc[3] = {ncx, ncy, ncz};
     for (int d = 0; d < 3; ++d) { lo[d] = box_lo[d]; h[d] = (box_hi[d] - box_lo[d]) / nc[d]; }
   }
+  for (int d = 0; d < 3; ++d) { c->lo[d] = lo[d]; c->h[d] = h[d]; }
+  if (vertices_host) {
+    try { c->verts.assign(vertices_host, vertices_host + 3 * (size_t)(ncx + 1) * (ncy + 1) * (ncz + 1)); }
+    catch (...) { delete c; return fail(nullptr, FE_MF_ENOMEM, "out of host memory (vertices)"); }
+  }
   const double centre[3] = {0.0, 0.0, 0.0};
   if (!vertices_host && geom == FE_GEOM_AFFINE) {
     c->geom_mode = 0;
@@ -203,7 +216,8 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
     const size_t per_cell = perq ? (((size_t)7 * nn + 1) & ~(size_t)1) : 7;   // even: 16-byte bulk copies
     c->geom_stride = (long long)per_cell;
     std::vector<double> G;
-    try { G.resize(per_cell * (size_t)c->ncells); } catch (...) { delete c; return fail(nullptr, FE_MF_ENOMEM, "out of host memory (geometry)"); }
+    try { G.resize(per_cell * (size_t)c->ncells); if (perq) c->detq.resize((size_t)nn * c->ncells); }
+    catch (...) { delete c; return fail(nullptr, FE_MF_ENOMEM, "out of host memory (geometry)"); }
     bool bad = false;
     for (int ez = 0; ez < ncz; ++ez)
       for (int ey = 0; ey < ncy; ++ey)
@@ -227,6 +241,7 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
                   const int Q = q1 + n * (q2 + n * q3);
                   for (int k = 0; k < 6; ++k) g[(size_t)k * nn + Q] = m[k];
                   g[(size_t)6 * nn + Q] = sigma * m[6];
+                  c->detq[cell * nn + Q] = m[6];
                 }
           }
         }
@@ -252,10 +267,103 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
   DeviceGuard guard(ctx->device);
   if (ctx->geom_dev) cudaFree(ctx->geom_dev);
   if (ctx->ctrl) cudaFree(ctx->ctrl);
+  if (ctx->dscale_dev) cudaFree(ctx->dscale_dev);
   if (ctx->ws_x) cudaFree(ctx->ws_x);
   if (ctx->ws_y) cudaFree(ctx->ws_y);
   for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
   delete ctx;
+}
+
+// ---- kappa(x) at the quadrature points, GLL-lumped mass scaling ---------------------------
+
+extern "C" int fe_mf_set_kappa(fe_mf_ctx* ctx, const double* kappa_host) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (ctx->geom_mode != 2) return fail(ctx, FE_MF_EINVAL, "fe_mf_set_kappa needs a context created with FE_GEOM_QPOINT");
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
+  const size_t nn = (size_t)ctx->n * ctx->n * ctx->n, total = nn * (size_t)ctx->ncells;
+  std::vector<double> g;
+  try { g.resize(total); } catch (...) { return fail(ctx, FE_MF_ENOMEM, "out of host memory (kappa)"); }
+  // G_QQ = kappa_Q det J; the weight w_Q lives in the sqrt(w)-scaled 1D tables
+  for (size_t i = 0; i < total; ++i) g[i] = (kappa_host ? kappa_host[i] : ctx->sigma) * ctx->detq[i];
+  FE_CUDA(ctx, cudaDeviceSynchronize());
+  FE_CUDA(ctx, cudaMemcpy2D(ctx->geom_dev + 6 * nn, (size_t)ctx->geom_stride * sizeof(double), g.data(), nn * sizeof(double),
+                            nn * sizeof(double), (size_t)ctx->ncells, cudaMemcpyHostToDevice));
+  return FE_MF_OK;
+}
+
+namespace {
+
+// diag(M) by the (p+1)-point Gauss-Lobatto-Legendre rule on the nodes:
+// M_ii = sum over cells containing node i of det J(xi_i) w_i1 w_i2 w_i3, w = 2 / (p (p+1) P_p(xi)^2)
+int build_mass_diagonal(fe_mf_ctx* c) {
+  const int p = c->p, n = c->n;
+  long double xl[fe::MAXN], wl[fe::MAXN];
+  fe::gll_nodes(p, xl);
+  for (int i = 0; i < n; ++i) {
+    long double pn, pm;
+    fe::legendre(p, xl[i], pn, pm);
+    wl[i] = 2.0L / ((long double)p * (p + 1) * pn * pn);
+  }
+  double w[fe::MAXN], x[fe::MAXN];
+  for (int i = 0; i < n; ++i) { w[i] = (double)(0.5L * (wl[i] + wl[n - 1 - i])); x[i] = (double)xl[i]; }
+  try { c->mass_diag.assign((size_t)c->ndof, 0.0); } catch (...) { return fail(c, FE_MF_ENOMEM, "out of host memory (mass diagonal)"); }
+  const double* verts = c->verts.empty() ? nullptr : c->verts.data();
+  for (int ez = 0; ez < c->ncz; ++ez)
+    for (int ey = 0; ey < c->ncy; ++ey)
+      for (int ex = 0; ex < c->ncx; ++ex) {
+        double v[8][3], J[3][3], m[7];
+        cell_vertices(c, verts, c->lo, c->h, ex, ey, ez, v);
+        for (int i3 = 0; i3 < n; ++i3)
+          for (int i2 = 0; i2 < n; ++i2)
+            for (int i1 = 0; i1 < n; ++i1) {
+              const double xi[3] = {x[i1], x[i2], x[i3]};
+              fe::trilinear_jacobian(v, xi, J);
+              if (!fe::metric_from_jacobian(J, m)) return fail(c, FE_MF_EINVAL, "non-positive det J at a node");
+              int ix = ex * p + i1, iy = ey * p + i2, iz = ez * p + i3;
+              if (ix >= c->ndx) ix -= c->ndx;
+              if (iy >= c->ndy) iy -= c->ndy;
+              if (iz >= c->ndz) iz -= c->ndz;
+              c->mass_diag[(size_t)ix + (size_t)c->ndx * ((size_t)iy + (size_t)c->ndy * iz)] += m[6] * (w[i1] * w[i2] * w[i3]);
+            }
+      }
+  std::vector<double> d;
+  try { d.resize((size_t)c->ndof); } catch (...) { return fail(c, FE_MF_ENOMEM, "out of host memory (mass diagonal)"); }
+  for (size_t i = 0; i < d.size(); ++i) d[i] = 1.0 / std::sqrt(c->mass_diag[i]);
+  if (cudaMalloc(&c->dscale_dev, d.size() * sizeof(double)) != cudaSuccess) {
+    c->dscale_dev = nullptr; c->mass_diag.clear();
+    return fail(c, FE_MF_ENOMEM, "cudaMalloc (mass scaling) failed");
+  }
+  FE_CUDA(c, cudaMemcpy(c->dscale_dev, d.data(), d.size() * sizeof(double), cudaMemcpyHostToDevice));
+  return FE_MF_OK;
+}
+
+}  // namespace
+
+extern "C" int fe_mf_set_mass_scaling(fe_mf_ctx* ctx, int on) {
+  if (!ctx) return FE_MF_EINVAL;
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
+  FE_CUDA(ctx, cudaDeviceSynchronize());
+  if (on && !ctx->dscale_dev) {
+    const int rc = build_mass_diagonal(ctx);
+    if (rc != FE_MF_OK) return rc;
+  }
+  ctx->mass_scaled = on != 0;
+  return FE_MF_OK;
+}
+
+extern "C" int fe_mf_mass_diagonal(fe_mf_ctx* ctx, double* out_host) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (!out_host) return fail(ctx, FE_MF_EINVAL, "out_host is NULL");
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
+  if (!ctx->dscale_dev) {
+    const int rc = build_mass_diagonal(ctx);
+    if (rc != FE_MF_OK) return rc;
+  }
+  std::memcpy(out_host, ctx->mass_diag.data(), sizeof(double) * (size_t)ctx->ndof);
+  return FE_MF_OK;
 }
 
 #include "fe_dispatch.inl"

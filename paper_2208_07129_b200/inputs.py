@@ -145,3 +145,11 @@ def workload_vertices(w: Workload) -> Optional[np.ndarray]:
     if w.geom == GEOM_QPOINT:
         return perturbed_vertices(w.ncells, w.box_lo, w.box_hi, w.perturb, w.seed + 100)
     return None
+
+
+def kappa_points(seed: int, ncells: int, n3: int, lo: float = -1.0, hi: float = 3.0) -> np.ndarray:
+    """Synthetic stand-in for the 'precomputed potential' kappa of PAPER.md:796: one value per quadrature point,
+    [ncells][n3], independent draws in [lo, hi] from the counter generator (the kernels' cost does not depend on the
+    values; smooth potentials are built in the tests from the oracle's quadrature-point coordinates)."""
+    u = uniform_pm1(seed, 0, ncells * n3).reshape(ncells, n3)
+    return lo + (hi - lo) * 0.5 * (u + 1.0)
