@@ -172,13 +172,13 @@ template <> struct PlaneCfg<6> { static constexpr int BV = 16, NT = 128, MINB = 
 template <> struct PlaneCfg<7> { static constexpr int BV = 16, NT = 128, MINB = 1; };   // spills; kept for comparison
 bool plane_ok(int p) { return p == 6 || p == 7; }
 
-template <int PDEG, int IM, bool IDENT = false>
+template <int PDEG, int IM, bool IDENT = false, bool EIG = false>
 cudaError_t launch_plane_im(fe_mf_ctx* c, const fe::ApplyParams& prm, fe::InitParams init, const CUtensorMap& tw,
                             const CUtensorMap& tz, cudaStream_t st) {
   using C = PlaneCfg<PDEG>;
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64 + fe::InitAhead<C::NT, IM>::STAGE_BYTES;
   static int bps = 0;
-  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IM, IDENT>;
+  auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IM, IDENT, EIG>;
   long long grid = 0;
   int nitems = (int)(c->ncells * prm.nvb);
   cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
@@ -197,6 +197,11 @@ cudaError_t launch_plane_im(fe_mf_ctx* c, const fe::ApplyParams& prm, fe::InitPa
 template <int PDEG>
 cudaError_t launch_plane(fe_mf_ctx* c, const fe::ApplyParams& prm, const fe::InitParams& init, const CUtensorMap& tw,
                          const CUtensorMap& tz, cudaStream_t st) {
+  if (prm.kappa) {   // eigenproblem operator (EIG): never combined with the fused initialisation
+    if (init.mode != fe::INIT_NONE) return cudaErrorInvalidValue;
+    return prm.idw != 0.0 ? launch_plane_im<PDEG, 0, true, true>(c, prm, init, tw, tz, st)
+                          : launch_plane_im<PDEG, 0, false, true>(c, prm, init, tw, tz, st);
+  }
   if (init.mode == fe::INIT_NONE && prm.idw != 0.0) return launch_plane_im<PDEG, 0, true>(c, prm, init, tw, tz, st);
   if (init.mode == fe::INIT_NONE) return launch_plane_im<PDEG, 0>(c, prm, init, tw, tz, st);
   if (init.mode == fe::INIT_ZERO) return launch_plane_im<PDEG, 1>(c, prm, init, tw, tz, st);
@@ -231,14 +236,14 @@ int line_bv(const fe_mf_ctx* c, int nvec) {
 // 8-vector blocks with an even number of nodes per direction: one pad node per x-row (see DenseTile)
 constexpr int line_padx(int p, int bv) { return (bv == 8 && (p + 1) % 2 == 0 && p >= 3) ? 1 : 0; }
 
-template <int PDEG, int CFG, bool IDENT = false>
+template <int PDEG, int CFG, bool IDENT = false, bool EIG = false>
 cudaError_t launch_line_id(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                         cudaStream_t st) {
   using C = LineCfg<CFG>;
   constexpr int PADX = line_padx(PDEG, C::BV);
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV, PADX>::PITCH + 64;
   static int bps = 0;
-  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB, PADX, IDENT>;
+  auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB, PADX, IDENT, EIG>;
   const long long nitems = c->ncells * prm.nvb;
   long long grid = 0;
   cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
@@ -251,24 +256,36 @@ cudaError_t launch_line_id(const fe_mf_ctx* c, const fe::ApplyParams& prm, const
 template <int PDEG, int CFG>
 cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
                         cudaStream_t st) {
+  if (prm.kappa)
+    return prm.idw != 0.0 ? launch_line_id<PDEG, CFG, true, true>(c, prm, tw, tz, st)
+                          : launch_line_id<PDEG, CFG, false, true>(c, prm, tw, tz, st);
   return prm.idw != 0.0 ? launch_line_id<PDEG, CFG, true>(c, prm, tw, tz, st) : launch_line_id<PDEG, CFG, false>(c, prm, tw, tz, st);
 }
 
 // ---- which kernel serves (ctx, nvec, pointers)
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 1) return 1;
-  const bool msc = c->mass_scaled;   // only the full-metric kernels (kinds 1, 6) apply M^-1/2
-  const bool diag = !msc && (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
+  // NEXT-1 operator: a uniform box with mass scaling runs on the Cartesian TMA kernels instantiated with EIG (kappa per
+  // point, M^-1/2 inside the interpolation tables); kappa without mass scaling on such a context only on the general
+  // kernel; every other mesh on the full-metric kernels (kinds 6, 1), which read d = diag(M)^-1/2 from memory
+  const bool msc = c->mass_scaled;
+  const bool eig = msc && c->geom_mode == 0;
+  if (c->kappa_dev && !msc) return 1;
+  const bool diag = (!msc || eig) && (c->geom_mode == 0) && c->ug[1] == 0.0 && c->ug[2] == 0.0 && c->ug[4] == 0.0;
   const bool aligned = ((((uintptr_t)W) | ((uintptr_t)Z)) & 15) == 0;
   const bool tma_ok = !(nvec & 1) && aligned && encode_tiled_fn() &&
                       (unsigned long long)nvec * 8ULL * c->ndx * c->ndy < (1ULL << 40) &&
                       c->ncells * ((nvec + 7) / 8) < (1LL << 31);
-  if ((!diag || c->variant == 7) && tma_ok) return 6;
-  if (!diag) return 1;
-  if (nvec < 4) return 3;
-  if (!tma_ok || c->variant == 2) return 2;
   const bool trim_ok = (c->bc != FE_BC_DIRICHLET) || (c->ndx >= 3 && c->ndy >= 3 && c->ndz >= 3);
-  if (!trim_ok) return 2;
+  if (eig) {   // kinds 8 / 9 or the general kernel (which then reads d and kappa from memory)
+    if (!tma_ok || !trim_ok || nvec < 4 || c->variant == 2 || c->variant == 7) return 1;
+  } else {
+    if ((!diag || c->variant == 7) && tma_ok) return 6;
+    if (!diag) return 1;
+    if (nvec < 4) return 3;
+    if (!tma_ok || c->variant == 2) return 2;
+    if (!trim_ok) return 2;
+  }
   if (c->variant == 10 || c->variant == 11) return 9;
   if ((c->variant == 8 || c->variant == 19) && plane_ok(c->p)) return 8;
   // plane kernel: 16 vectors per block; worth it when the last block of vectors is mostly full
@@ -302,13 +319,15 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.item_ctr = reinterpret_cast<int*>(c->ctrl);
   P.idw = 0.0;
   P.dscale = c->mass_scaled ? c->dscale_dev : nullptr;
+  P.kappa = c->kappa_dev;
+  if (P.kappa) P.ug[6] = c->detj0;   // mass factor = det J * kappa_Q
   return P;
 }
 
 // Can this kernel kind initialise Z itself?  (plane kernel, cooperative launch, 32-bit chunk sizes; opt-in)
 bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
   const long long chunk2 = (long long)(c->p + 1) * c->ndx * c->ndy * nvec / 2;   // double2 elements of the largest chunk
-  return kind == 8 && c->coop && c->variant == 19 && chunk2 < (1LL << 31);
+  return kind == 8 && c->coop && c->variant == 19 && chunk2 < (1LL << 31) && !c->kappa_dev;
 }
 
 // Can this kernel add a multiple of W (identity term, partition-of-unity weights) in the same pass?  The Cartesian
@@ -345,6 +364,11 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
   }
   if (kind == 8 || kind == 9 || kind == 2 || kind == 3)
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // Cartesian kernels: the result is linear in the metric constants
+  if ((kind == 8 || kind == 9) && c->mass_scaled) {
+    // EIG kernels: diag(M)^-1/2 = (det J)^-1/2 kron diag(w~)^-1/2; the tables carry the second factor (both sides)
+    for (int k = 0; k < 7; ++k) P.ug[k] /= c->detj0;
+    P.dscale = nullptr;
+  }
   if (kind == 6 && P.dscale) {
 #define FE_CALL(p_) launch_gen<p_, true>(c, P, tw, tz, st)
     FE_DISPATCH_P(FE_CALL)

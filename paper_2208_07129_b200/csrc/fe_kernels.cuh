@@ -34,6 +34,9 @@ struct ApplyParams {
   double idw;                     // plane kernel with IDENT (periodic meshes): Z += alpha A W + idw W
   const double* dscale;           // nullptr, or d = diag(M)^-1/2 [ndof] of the GLL-lumped mass matrix: Z += alpha d.(A (d.W))
                                   // (Eq. B.1; kernels of kinds 1 and 6 only)
+  const double* kappa;            // nullptr, or kappa at the quadrature points [cell][n^3] of a uniform box (geom_mode 0):
+                                  // the mass factor is ug[6] * kappa_Q, ug[6] then holding det J without sigma
+                                  // (kind 1, and the Cartesian kernels instantiated with EIG)
 };
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.
@@ -133,6 +136,7 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
       } else {
 #pragma unroll
         for (int k = 0; k < 7; ++k) g[k] = P.ug[k] * wq;
+        if (P.kappa) g[6] *= __ldg(P.kappa + (size_t)cell * NN + Q);
       }
     }
     const double a = T0[t], b = T1[t], c = T2[t];

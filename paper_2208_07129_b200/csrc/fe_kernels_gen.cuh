@@ -96,6 +96,10 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     const bool special = dirichlet ? (ex == 0 || ex == P.ncx - 1 || ey == 0 || ey == P.ncy - 1 || ez == 0 || ez == P.ncz - 1)
                                    : (wx || wy || wz);
     if (!perq && tid < 7) GS[tid] = __ldg(P.geom + (P.geom_mode == 1 ? (size_t)cell * 7 : 0) + tid);   // visible after the barriers below
+    // MSC: the first round's d values are requested before the waits that precede their use (L2 latency)
+    const int t_first = (ROUNDS > 1 || !ROTATE) ? tid : rot_tid;
+    double dpre[N];
+    if (MSC && t_first < TASKS) load_dscale<PDEG>(P, ex, ey, ez, t_first / TPL, dpre);
     mbar_wait(bar, parity);
     parity ^= 1u;
 
@@ -138,7 +142,12 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       }
       if (MSC) {
         double dn[N];
-        load_dscale<PDEG>(P, ex, ey, ez, l, dn);
+        if (r_ == 0) {
+#pragma unroll
+          for (int i = 0; i < N; ++i) dn[i] = dpre[i];
+        } else {
+          load_dscale<PDEG>(P, ex, ey, ez, l, dn);
+        }
 #pragma unroll
         for (int i = 0; i < N; ++i) x[i] = vmul(dn[i], x[i]);
       }
@@ -266,6 +275,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     }
     __syncthreads();
     // ph7: Ns^T along y, in place
+    if (MSC && t_first < TASKS) load_dscale<PDEG>(P, ex, ey, ez, t_first / TPL, dpre);   // for ph8
     FE_FOR_TASKS(t) {
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<1>(l, base, stride);
@@ -281,7 +291,14 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N], y[N];
       double dn[N];
-      if (MSC) load_dscale<PDEG>(P, ex, ey, ez, l, dn);
+      if (MSC) {
+        if (r_ == 0) {
+#pragma unroll
+          for (int i = 0; i < N; ++i) dn[i] = dpre[i];
+        } else {
+          load_dscale<PDEG>(P, ex, ey, ez, l, dn);
+        }
+      }
       lds_line2<N>(A + base + b2, stride, x);
       eo2<PDEG, MAT_NS, true>(x, y);
       if (MSC) {

@@ -14,13 +14,15 @@ namespace fe {
 
 // IDENT: Z += alpha A W + idw W in the same pass (see fe_apply_cart_plane): the identity part is added in ph6 on
 // the nodal result, with partition-of-unity weights, from the nodal values of W re-read through L2.
-template <int PDEG, int BV, int NT, int MINB, int PADX, bool IDENT>
+// EIG: see fe_apply_cart_plane (kappa per quadrature point, mass-scaled interpolation tables).
+template <int PDEG, int BV, int NT, int MINB, int PADX, bool IDENT, bool EIG = false>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                    const __grid_constant__ ApplyParams P, int nitems) {
   using TL = DenseTile<PDEG, BV, PADX>;
   constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1, NL = N * N, TPL = BV / 2, TASKS = NL * TPL;
   constexpr int ROUNDS = (TASKS + NT - 1) / NT;
+  constexpr int NSM = EIG ? MAT_NSS : MAT_NS;
   constexpr bool ROTATE = (NT % 32 == 0) && (NT >= 128) && (TASKS % NT != 0);
   constexpr int NW = NT / 32;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -74,7 +76,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N];
       lds_line2<N>(A + base + b2, stride, x);
-      eo_full<PDEG, MAT_NS, false>(x, x);
+      eo_full<PDEG, NSM, false>(x, x);
       sts_line2<N>(A + base + b2, stride, x);
     }
     __syncthreads();
@@ -84,7 +86,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       int base, stride; TL::template line<1>(l, base, stride);
       v2 x[N];
       lds_line2<N>(A + base + b2, stride, x);
-      eo_full<PDEG, MAT_NS, false>(x, x);
+      eo_full<PDEG, NSM, false>(x, x);
       sts_line2<N>(A + base + b2, stride, x);
     }
     if (tid == 0) tma_wait_read0();     // the previous item's reduction has finished reading tile B
@@ -94,19 +96,25 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       const int b2 = (t % TPL) * 2, l = t / TPL;
       int base, stride; TL::template line<2>(l, base, stride);
       v2 x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u2[HH], vv[HH], m2;
+      double gq[N];   // gm kappa_Q along the z-line l = i1 + N i2
+      if (EIG) {
+        const double* kp = P.kappa + (size_t)cell * (N * N * N) + l;
+#pragma unroll
+        for (int q = 0; q < N; ++q) gq[q] = gm * __ldg(kp + q * N * N);
+      }
       lds_line2<N>(A + base + b2, stride, x);
       eo_split<N>(x, xp, xm);
-      eo_mult<PDEG, MAT_NS, false, false>(xp, xm, x[H], u, v, m);
+      eo_mult<PDEG, NSM, false, false>(xp, xm, x[H], u, v, m);
       eo_combine<N, false>(u, v, m, tq);
       sts_line2<N>(A + base + b2, stride, tq);
       eo_dtd_eo<PDEG>(u, v, m, u2, vv, m2);
       v2 r[N];
 #pragma unroll
       for (int q = 0; q < H; ++q) {
-        r[q] = vfma(g4z, u2[q] + vv[q], vmul(gm, tq[q]));
-        r[N - 1 - q] = vfma(g4z, vv[q] - u2[q], vmul(gm, tq[N - 1 - q]));
+        r[q] = vfma(g4z, u2[q] + vv[q], vmul(EIG ? gq[q] : gm, tq[q]));
+        r[N - 1 - q] = vfma(g4z, vv[q] - u2[q], vmul(EIG ? gq[N - 1 - q] : gm, tq[N - 1 - q]));
       }
-      if (N & 1) r[H] = vfma(g4z, m2, vmul(gm, tq[H]));
+      if (N & 1) r[H] = vfma(g4z, m2, vmul(EIG ? gq[H] : gm, tq[H]));
       sts_line2<N>(B + base + b2, stride, r);
     }
     __syncthreads();
@@ -140,7 +148,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       for (int q = 0; q < H; ++q) { rp[q] = vfma(g4y, vv[q], rp[q]); rm[q] = vfma(g4y, u2[q], rm[q]); }
       vzero(rc);
       if (N & 1) rc = vfma(g2y, m2, c[H]);
-      eo_mult<PDEG, MAT_NS, true, false>(rp, rm, rc, u, v, m);
+      eo_mult<PDEG, NSM, true, false>(rp, rm, rc, u, v, m);
       eo_combine<N, false>(u, v, m, c);
       sts_line2<N>(B + base + b2, stride, c);
     }
@@ -162,7 +170,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       int base, stride; TL::template line<0>(l, base, stride);
       v2 x[N];
       lds_line2<N>(B + base + b2, stride, x);
-      eo_full<PDEG, MAT_NS, true>(x, x);
+      eo_full<PDEG, NSM, true>(x, x);
       sts_line2<N>(B + base + b2, stride, x);
     }
     __syncthreads();
@@ -188,7 +196,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
         }
       }
       lds_line2<N>(B + base + b2, stride, x);
-      eo_full<PDEG, MAT_NS, true>(x, x);
+      eo_full<PDEG, NSM, true>(x, x);
       if (IDENT) {
         const int i1 = l % N, i2 = l / N;
         double wl = P.idw;

@@ -38,7 +38,7 @@ struct EoTab2 {
   double midm, midmh;       // M[mid][mid] and half of it
   double pad[2];
 };
-__constant__ EoTab2 c_eo2[KMAXN][3];   // [p][MAT_NS | MAT_DS | MAT_SH]
+__constant__ EoTab2 c_eo2[KMAXN][4];   // [p][MAT_NS | MAT_DS | MAT_SH | MAT_NSS]
 
 // The primitives are generic in the value type T: double (one vector per thread, plane kernels) or v2 (two
 // vectors per thread, line kernels).
@@ -172,13 +172,17 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
 // partition-of-unity weights (a node on a cell face in a direction is shared by two cells: weight 1/2 per
 // direction) in P4, on the nodal result, from the nodal values of W re-read through L2 (the tile that held them was
 // transformed in place).  The shifted operator A - cI of the Chebyshev recurrence then costs no separate pass.
-template <int PDEG, int BV, int NT, int MINB, int IM, bool IDENT>
+// EIG: the operator of the paper's eigenproblem on a uniform box, H~ = M^-1/2 (K + M^kappa) M^-1/2:
+// kappa is read per quadrature point (P.kappa [cell][n^3]) and the interpolation passes use the
+// mass-scaled tables MAT_NSS (the constant (1/det J) of M^-1 is folded into the metric constants by the host).
+template <int PDEG, int BV, int NT, int MINB, int IM, bool IDENT, bool EIG = false>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
                     const __grid_constant__ ApplyParams P, const __grid_constant__ InitParams I, int nitems) {
   using TL = DenseTile<PDEG, BV>;
   constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1;
   constexpr int S1 = BV, S2 = N * BV, S3 = N * N * BV;   // element strides along x, y, z
+  constexpr int NSM = EIG ? MAT_NSS : MAT_NS;
   static_assert(N * BV <= NT && NT % 128 == 0, "one plane task per thread; whole warps on every sub-partition");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* A = reinterpret_cast<double*>(smem_raw);
@@ -248,13 +252,13 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
 #pragma unroll
         for (int i = 0; i < N; ++i) r[j][i] = a[j * S2 + i * S1];
 #pragma unroll
-      for (int j = 0; j < N; ++j) eo_full<PDEG, MAT_NS, false>(r[j], r[j]);
+      for (int j = 0; j < N; ++j) eo_full<PDEG, NSM, false>(r[j], r[j]);
 #pragma unroll
       for (int i = 0; i < N; ++i) {
         double c[N];
 #pragma unroll
         for (int j = 0; j < N; ++j) c[j] = r[j][i];
-        eo_full<PDEG, MAT_NS, false>(c, c);
+        eo_full<PDEG, NSM, false>(c, c);
 #pragma unroll
         for (int j = 0; j < N; ++j) a[j * S2 + i * S1] = c[j];
       }
@@ -277,6 +281,12 @@ FE_ZLOOP_PRAGMA
         double* a = A + k * S2 + i * S1 + beta;
         double* b = B + k * S2 + i * S1 + beta;
         double x[N], tq[N], xp[HH], xm[HH], u[HH], v[HH], m, u2[HH], v2[HH], m2;
+        double gq[N];   // gm kappa_Q along the z-line (i, k, .): shared by the block's vectors, L1-resident
+        if (EIG) {
+          const double* kp = P.kappa + (size_t)cell * (N * N * N) + i + N * k;
+#pragma unroll
+          for (int q = 0; q < N; ++q) gq[q] = __ldg(kp + q * N * N);
+        }
 #pragma unroll
         for (int j = 0; j < N; ++j) x[j] = xn[j];
         if (i + 1 < N) {
@@ -284,17 +294,17 @@ FE_ZLOOP_PRAGMA
           for (int j = 0; j < N; ++j) xn[j] = a[S1 + j * S3];
         }
         eo_split<N>(x, xp, xm);
-        eo_mult<PDEG, MAT_NS, false, false>(xp, xm, x[H], u, v, m);
+        eo_mult<PDEG, NSM, false, false>(xp, xm, x[H], u, v, m);
         eo_combine<N, false>(u, v, m, tq);
 #pragma unroll
         for (int j = 0; j < N; ++j) a[j * S3] = tq[j];
         eo_dtd_eo<PDEG>(u, v, m, u2, v2, m2);                          // quarter of Ds^T Ds T
 #pragma unroll
         for (int q = 0; q < H; ++q) {
-          b[q * S3] = fma(g4z, u2[q] + v2[q], gm * tq[q]);
-          b[(N - 1 - q) * S3] = fma(g4z, v2[q] - u2[q], gm * tq[N - 1 - q]);
+          b[q * S3] = fma(g4z, u2[q] + v2[q], (EIG ? gm * gq[q] : gm) * tq[q]);
+          b[(N - 1 - q) * S3] = fma(g4z, v2[q] - u2[q], (EIG ? gm * gq[N - 1 - q] : gm) * tq[N - 1 - q]);
         }
-        if (N & 1) b[H * S3] = fma(g4z, m2, gm * tq[H]);
+        if (N & 1) b[H * S3] = fma(g4z, m2, (EIG ? gm * gq[H] : gm) * tq[H]);
       }
     }
     __syncthreads();
@@ -336,14 +346,14 @@ FE_ZLOOP_PRAGMA
 #pragma unroll
           for (int q = 0; q < H; ++q) { rp[q] = fma(g4y, v2[q], rp[q]); rm[q] = fma(g4y, u2[q], rm[q]); }
           const double rc = (N & 1) ? fma(g2y, m2, c[H]) : 0.0;
-          eo_mult<PDEG, MAT_NS, true, false>(rp, rm, rc, u, v, m);
+          eo_mult<PDEG, NSM, true, false>(rp, rm, rc, u, v, m);
           eo_combine<N, false>(u, v, m, c);
 #pragma unroll
           for (int j = 0; j < N; ++j) r[j][i] = c[j];
         }
 #pragma unroll
         for (int j = 0; j < N; ++j) {
-          eo_full<PDEG, MAT_NS, true>(r[j], r[j]);
+          eo_full<PDEG, NSM, true>(r[j], r[j]);
 #pragma unroll
           for (int i = 0; i < N; ++i) b[j * S2 + i * S1] = r[j][i];
         }
@@ -393,7 +403,7 @@ FE_ZLOOP_PRAGMA
           for (int j = 0; j < N; ++j) xn[j] = b[S1 + j * S3];
           if (IDENT) load_w(i + 1, wn);
         }
-        eo_full<PDEG, MAT_NS, true>(x, x);
+        eo_full<PDEG, NSM, true>(x, x);
         if (IDENT) {
           const double wi = (i == 0 || i == N - 1) ? 0.5 * wk : wk;
 #pragma unroll

@@ -42,6 +42,10 @@ struct fe_mf_ctx {
   double* dscale_dev = nullptr;   // diag(M)^-1/2 of the GLL-lumped mass matrix [ndof]
   std::vector<double> mass_diag;  // diag(M) [ndof] (host copy, filled with dscale_dev)
   bool mass_scaled = false;
+  double* kappa_dev = nullptr;    // geom_mode 0: kappa at the quadrature points [cell][n^3] (set_kappa, or sigma everywhere
+                                  // once mass scaling is on: the EIG kernels always read it)
+  bool kappa_user = false;
+  double detj0 = 1.0;             // geom_mode 0: det J of every cell
   int variant = 0;
   int last_launches = 0;
   // fe_mf_apply_host workspace
@@ -74,9 +78,9 @@ struct DeviceGuard {
 
 // Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
 // 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
-void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[3]) {
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[4]) {
   const int n = t.n, h = n / 2, m = n / 2;
-  long double M[5][fe::MAXN * fe::MAXN];
+  long double M[6][fe::MAXN * fe::MAXN];
   for (int q = 0; q < n; ++q)
     for (int i = 0; i < n; ++i) {
       const long double sq = sqrtl(t.wl[q]), si = sqrtl(t.wl[i]);
@@ -93,8 +97,24 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[3])
       for (int q = 0; q < n; ++q) acc += M[2][q * n + i] * M[2][q * n + j];
       M[4][i * n + j] = 0.5L * acc;
     }
-  fe::EoTab tabs[5];
-  for (int k = 0; k < 5; ++k) {
+  // M[5] = Ns diag(w~)^-1/2, w~ = the (p+1)-point Gauss-Lobatto weights with the two end weights doubled (a face
+  // node of a uniform mesh belongs to two cells per direction): on a uniform box diag(M)^-1/2 of the GLL-lumped mass
+  // matrix is (1/det J)^1/2 times the Kronecker product of diag(w~)^-1/2, so that the mass scaling of
+  // H~ = M^-1/2 H M^-1/2 is absorbed by the interpolation tables and costs nothing in the kernels
+  {
+    long double xl[fe::MAXN];
+    fe::gll_nodes(t.p, xl);
+    for (int i = 0; i < n; ++i) {
+      long double pn, pm;
+      fe::legendre(t.p, xl[i], pn, pm);
+      long double wg = 2.0L / ((long double)t.p * (t.p + 1) * pn * pn);
+      if (i == 0 || i == n - 1) wg *= 2.0L;
+      const long double si = 1.0L / sqrtl(wg);
+      for (int q = 0; q < n; ++q) M[5][q * n + i] = M[0][q * n + i] * si;
+    }
+  }
+  fe::EoTab tabs[6];
+  for (int k = 0; k < 6; ++k) {
     std::memset(&tabs[k], 0, sizeof(fe::EoTab));
     for (int q = 0; q < h; ++q) {
       for (int i = 0; i < h; ++i) {
@@ -111,8 +131,8 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[3])
   for (int k = 0; k < 5; ++k) out[k] = tabs[k];
   // the plane / line kernels' tables: Ns, Ds (the transposes reuse them) and Ds^T Ds / 2, plus the halved middle
   // column / row
-  const int src[3] = {0, 2, 4};
-  for (int k2 = 0; k2 < 3; ++k2) {
+  const int src[4] = {0, 2, 4, 5};
+  for (int k2 = 0; k2 < 4; ++k2) {
     const fe::EoTab& s = tabs[src[k2]];
     fe::EoTab2& d = out2[k2];
     std::memset(&d, 0, sizeof(fe::EoTab2));
@@ -182,10 +202,10 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
   if (e == cudaSuccess) {
     fe::EoTab eo[5];
-    fe::EoTab2 eo2[3];
+    fe::EoTab2 eo2[4];
     make_eo_tables(tab, eo, eo2);
     e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 5 * p);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 3 * p);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 4 * p);
   }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
 
@@ -206,6 +226,7 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
     cell_vertices(c, nullptr, lo, h, 0, 0, 0, v);
     fe::trilinear_jacobian(v, centre, J);
     if (!fe::metric_from_jacobian(J, c->ug)) { delete c; return fail(nullptr, FE_MF_EINVAL, "non-positive det J"); }
+    c->detj0 = c->ug[6];
     c->ug[6] *= sigma;
     e = cudaMalloc(&c->geom_dev, 7 * sizeof(double));   // the general TMA kernel reads the uniform metric from memory
     if (e == cudaSuccess) e = cudaMemcpy(c->geom_dev, c->ug, 7 * sizeof(double), cudaMemcpyHostToDevice);
@@ -268,6 +289,7 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
   if (ctx->geom_dev) cudaFree(ctx->geom_dev);
   if (ctx->ctrl) cudaFree(ctx->ctrl);
   if (ctx->dscale_dev) cudaFree(ctx->dscale_dev);
+  if (ctx->kappa_dev) cudaFree(ctx->kappa_dev);
   if (ctx->ws_x) cudaFree(ctx->ws_x);
   if (ctx->ws_y) cudaFree(ctx->ws_y);
   for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
@@ -278,10 +300,32 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
 
 extern "C" int fe_mf_set_kappa(fe_mf_ctx* ctx, const double* kappa_host) {
   if (!ctx) return FE_MF_EINVAL;
-  if (ctx->geom_mode != 2) return fail(ctx, FE_MF_EINVAL, "fe_mf_set_kappa needs a context created with FE_GEOM_QPOINT");
+  if (ctx->geom_mode == 1)
+    return fail(ctx, FE_MF_EINVAL, "fe_mf_set_kappa needs a uniform box or a context created with FE_GEOM_QPOINT");
   DeviceGuard guard(ctx->device);
   if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
   const size_t nn = (size_t)ctx->n * ctx->n * ctx->n, total = nn * (size_t)ctx->ncells;
+  if (ctx->geom_mode == 0) {   // uniform box: the raw kappa array, read by the EIG kernels and the general kernel
+    FE_CUDA(ctx, cudaDeviceSynchronize());
+    ctx->kappa_user = kappa_host != nullptr;
+    if (!kappa_host && !ctx->mass_scaled) {
+      if (ctx->kappa_dev) cudaFree(ctx->kappa_dev);
+      ctx->kappa_dev = nullptr;
+      return FE_MF_OK;
+    }
+    if (!ctx->kappa_dev && cudaMalloc(&ctx->kappa_dev, total * sizeof(double)) != cudaSuccess) {
+      ctx->kappa_dev = nullptr;
+      return fail(ctx, FE_MF_ENOMEM, "cudaMalloc (kappa) failed");
+    }
+    if (kappa_host) {
+      FE_CUDA(ctx, cudaMemcpy(ctx->kappa_dev, kappa_host, total * sizeof(double), cudaMemcpyHostToDevice));
+    } else {
+      std::vector<double> k0;
+      try { k0.assign(total, ctx->sigma); } catch (...) { return fail(ctx, FE_MF_ENOMEM, "out of host memory (kappa)"); }
+      FE_CUDA(ctx, cudaMemcpy(ctx->kappa_dev, k0.data(), total * sizeof(double), cudaMemcpyHostToDevice));
+    }
+    return FE_MF_OK;
+  }
   std::vector<double> g;
   try { g.resize(total); } catch (...) { return fail(ctx, FE_MF_ENOMEM, "out of host memory (kappa)"); }
   // G_QQ = kappa_Q det J; the weight w_Q lives in the sqrt(w)-scaled 1D tables
@@ -350,6 +394,11 @@ extern "C" int fe_mf_set_mass_scaling(fe_mf_ctx* ctx, int on) {
     if (rc != FE_MF_OK) return rc;
   }
   ctx->mass_scaled = on != 0;
+  if (ctx->geom_mode == 0) {
+    // the EIG kernels read kappa per point: constant sigma becomes an array while the scaling is on
+    if (on && !ctx->kappa_dev) return fe_mf_set_kappa(ctx, nullptr);
+    if (!on && ctx->kappa_dev && !ctx->kappa_user) { cudaFree(ctx->kappa_dev); ctx->kappa_dev = nullptr; }
+  }
   return FE_MF_OK;
 }
 

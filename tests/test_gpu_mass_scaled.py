@@ -71,12 +71,31 @@ def test_kappa_at_quadrature_points(env, p, bc, nvec):
     assert relerr(Yd.cpu().numpy(), orc.Operator(mesh, 0.7).apply(X)) <= TOL
 
 
-def test_kappa_needs_qpoint_context(env):
+def test_kappa_rejected_on_per_cell_metric_context(env):
     torch, orc, binding = env
-    op, mesh = make_pair(env, 3, inputs.BC_PERIODIC, "uniform")
+    verts = inputs.uniform_vertices((3, 2, 3), (0, 0, 0), (1, 1, 1))
+    op = binding.FeMf((3, 2, 3), 3, 1.0, inputs.BC_PERIODIC, binding.FE_GEOM_AFFINE, vertices=verts)
     with pytest.raises(binding.FeMfError) as e:
         op.set_kappa(np.zeros((18, 64)))
     assert e.value.code == binding.FE_MF_EINVAL
+
+
+@pytest.mark.parametrize("p", [2, 6, 7])
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+def test_kappa_on_uniform_box_context(env, p, bc):
+    """kappa without mass scaling on an affine (uniform box) context: served by the general kernel."""
+    torch, orc, binding = env
+    op, mesh = make_pair(env, p, bc, "uniform")
+    kap = inputs.kappa_points(5 + p, 18, (p + 1) ** 3)
+    op.set_kappa(kap)
+    X = inputs.multivector(31, mesh.ndof, 8)
+    Xd = torch.from_numpy(X).cuda()
+    Yd = torch.full_like(Xd, float("nan"))
+    op.apply(Xd, Yd, 8)
+    assert relerr(Yd.cpu().numpy(), orc.Operator(mesh, 0.0, kappa=kap).apply(X)) <= TOL
+    op.set_kappa(None)
+    op.apply(Xd, Yd, 8)
+    assert relerr(Yd.cpu().numpy(), orc.Operator(mesh, 0.7).apply(X)) <= TOL
 
 
 def smooth_potential(orc, mesh):
@@ -86,13 +105,14 @@ def smooth_potential(orc, mesh):
     return -8.0 * np.exp(-((xq - c1) ** 2).sum(-1) / 0.3) - 5.0 * np.exp(-((xq - c2) ** 2).sum(-1) / 0.5)
 
 
-@pytest.mark.parametrize("p", [1, 3, 4, 6, 7, 8])
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
-@pytest.mark.parametrize("kind", ["uniform", "uniform_q", "perturbed_q"])
+@pytest.mark.parametrize("kind", ["uniform", "uniform_k", "uniform_q", "perturbed_q"])
 def test_mass_scaled_apply(env, p, bc, kind):
-    """Y = M^-1/2 (K + M^kappa) M^-1/2 X."""
+    """Y = M^-1/2 (K + M^kappa) M^-1/2 X.  'uniform' / 'uniform_k' (affine context, constant sigma /
+    kappa per point) run on the Cartesian kernels with the mass-scaled tables, the others on the full-metric kernel."""
     torch, orc, binding = env
-    op, mesh = make_pair(env, p, bc, kind)
+    op, mesh = make_pair(env, p, bc, "uniform" if kind == "uniform_k" else kind)
     kap = None
     if kind != "uniform":
         kap = smooth_potential(orc, mesh)
@@ -100,7 +120,7 @@ def test_mass_scaled_apply(env, p, bc, kind):
     op.set_mass_scaling(True)
     oo = orc.Operator(mesh, 0.7, kappa=kap)
     d = 1.0 / np.sqrt(orc.lumped_mass_diagonal(mesh))
-    for nvec in (8, 3):
+    for nvec in (8, 3, 16, 28):
         X = inputs.multivector(37, mesh.ndof, nvec)
         Xd = torch.from_numpy(X).cuda()
         Yd = torch.full_like(Xd, float("nan"))
@@ -108,15 +128,16 @@ def test_mass_scaled_apply(env, p, bc, kind):
         assert relerr(Yd.cpu().numpy(), oo.apply_mass_scaled(X, d)) <= TOL, (nvec, op.kernel_name(nvec))
     # switching the scaling off restores H
     op.set_mass_scaling(False)
-    op.apply(Xd, Yd, 3)
+    op.apply(Xd, Yd, nvec)
     assert relerr(Yd.cpu().numpy(), oo.apply(X)) <= TOL
 
 
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
-def test_mass_scaled_axpby_eq_b1(env, bc):
+@pytest.mark.parametrize("kind,p", [("perturbed_q", 5), ("uniform", 6), ("uniform", 7), ("uniform", 3)])
+def test_mass_scaled_axpby_eq_b1(env, bc, kind, p):
     """Y = a H~ X + b X + c Y (Eq. B.1)."""
     torch, orc, binding = env
-    op, mesh = make_pair(env, 5, bc, "perturbed_q")
+    op, mesh = make_pair(env, p, bc, kind)
     kap = smooth_potential(orc, mesh)
     op.set_kappa(kap)
     op.set_mass_scaling(True)
@@ -133,17 +154,19 @@ def test_mass_scaled_axpby_eq_b1(env, bc):
 
 
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
-@pytest.mark.parametrize("p", [4, 6])
-def test_mass_scaled_chebyshev_filter(env, p, bc):
-    """Algorithm 6 lines 2-17 on H~ with mu = 1 and a smooth potential."""
+@pytest.mark.parametrize("p", [4, 6, 7, 8])
+@pytest.mark.parametrize("kind", ["uniform", "uniform_q"])
+def test_mass_scaled_chebyshev_filter(env, p, bc, kind):
+    """Algorithm 6 lines 2-17 on H~ with mu = 1 and a smooth potential; on the affine context the
+    one-launch-per-step recurrence of the Cartesian kernels (identity term added in the kernel)."""
     torch, orc, binding = env
-    op, mesh = make_pair(env, p, bc, "uniform_q", ncells=(3, 3, 2))
+    op, mesh = make_pair(env, p, bc, kind, ncells=(3, 3, 2))
     kap = smooth_potential(orc, mesh)
     op.set_kappa(kap)
     op.set_mass_scaling(True)
     oo = orc.Operator(mesh, 0.0, kappa=kap)
     d = 1.0 / np.sqrt(orc.lumped_mass_diagonal(mesh))
-    nvec = 8
+    nvec = 16
     X = inputs.multivector(47, mesh.ndof, nvec)
     app = lambda V: oo.apply_mass_scaled(V, d)
     b = orc.lanczos_upper_bound(app, X[:, 0].copy(), 12)
@@ -155,3 +178,5 @@ def test_mass_scaled_chebyshev_filter(env, p, bc):
     Yd = torch.full_like(Xd, float("nan"))
     op.cheb_filter(Xd, Yd, nvec, m, a, b, a0)
     assert relerr(Yd.cpu().numpy(), Yo) <= 1e-11
+    if kind == "uniform":
+        assert op.last_launch_count() <= m + 1
