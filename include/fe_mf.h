@@ -137,12 +137,15 @@ int fe_fill_uniform(double *out_dev, long long count, unsigned long long seed, l
  *
  * fe_mf_set_kappa: kappa_host is a HOST array [ncells][n^3] (cells x fastest, point Q = q1 + n q2 + n^2 q3 at the
  *   Gauss points of the cell: kappa_Q = kappa(x_Q)), copied; it replaces sigma in every later call
- *   (G_QQ = kappa_Q det J w_Q).  NULL restores the constant sigma.  The context must have been created
- *   with FE_GEOM_QPOINT (the mesh may still be the uniform box), else EINVAL.
+ *   (G_QQ = kappa_Q det J w_Q).  NULL restores the constant sigma.  The context must be a uniform box
+ *   (FE_GEOM_AFFINE without vertices) or have been created with FE_GEOM_QPOINT, else EINVAL (one metric per cell of a
+ *   vertex array has no per-point storage).  On a uniform box the fast path is kappa TOGETHER with mass scaling (the
+ *   eigenproblem operator, served by the Cartesian kernels); kappa alone runs there on the general fallback kernel.
  * fe_mf_set_mass_scaling: on != 0 makes fe_mf_apply / fe_mf_apply_axpby / fe_cheb_filter / fe_mf_apply_host act
  *   with H~ instead of H: Z = alpha M^-1/2 H M^-1/2 W + beta Z + gamma W (Eq. B.1); the diagonal
- *   scaling is done inside the kernel at extraction and assembly, not in extra passes.  Runs on
- *   the full-metric kernels.  Dirichlet boundary entries of M are computed like all others and never used.
+ *   scaling is done inside the kernel, not in extra passes: on a uniform box M^-1/2 is a Kronecker product and is
+ *   absorbed by the 1D interpolation tables (no cost); on other meshes it is applied at extraction and assembly
+ *    by the full-metric kernels from a vector of n_dof doubles.  Dirichlet boundary entries of M are computed like all others and never used.
  * fe_mf_mass_diagonal: writes diag(M) (HOST array of fe_mf_ndofs doubles, node order of the multivector rows) so
  *   that the caller can map U = M^-1/2 U~.
  * All three synchronise the device (they are setup calls, not stream-ordered) and return FE_MF_* codes.
