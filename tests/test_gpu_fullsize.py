@@ -95,3 +95,57 @@ def test_cfg5_full_chebyshev(env):
     Yo = orc.chebyshev_filter(oo.apply, Xc, w.cheb_m, w.cheb_a, b, w.cheb_a0)
     err = float(np.abs(Yg - Yo).max() / np.abs(Yo).max())
     assert err <= TOL, err
+
+
+# ---------------------------------------------------------------- SURVEY.md 8(f) NEXT-1 at full size
+def run_full_eigen_operator(env, w, nvec, nsamples=12):
+    """H~ = M^-1/2 (K + M^kappa) M^-1/2 with a seeded kappa per quadrature point, whole multivector on the GPU,
+    sampled rows from the oracle: (H~ X)[J] = d_J (H (d.X))[J]."""
+    torch, orc, binding = env
+    op = binding.FeMf.from_workload(w)
+    ncell = w.ncells[0] * w.ncells[1] * w.ncells[2]
+    kap = inputs.kappa_points(w.seed + 300, ncell, (w.p + 1) ** 3)
+    op.set_kappa(kap)
+    op.set_mass_scaling(True)
+    X = torch.empty(w.ndof * nvec, dtype=torch.float64, device="cuda")
+    Y = torch.full_like(X, float("nan"))
+    binding.fill_uniform(X, w.seed)
+    op.apply(X, Y, nvec)
+    torch.cuda.synchronize()
+    Yv = Y.view(w.ndof, nvec)
+    scale = float(Yv.abs().max().item())
+    assert np.isfinite(scale) and scale > 0
+    bc = "periodic" if w.bc == inputs.BC_PERIODIC else "dirichlet"
+    mesh = orc.Mesh(w.ncells, w.p, bc, w.box_lo, w.box_hi, vertices=inputs.workload_vertices(w))
+    oo = orc.Operator(mesh, 0.0, kappa=kap)
+    Mo = orc.lumped_mass_diagonal(mesh)
+    # det J comes from differences of vertex coordinates: rounding is amplified by |x| / h (<= cells per direction)
+    assert (np.abs(op.mass_diagonal() - Mo) / Mo).max() <= 16 * np.finfo(float).eps * max(w.ncells)
+    d = 1.0 / np.sqrt(Mo)
+    nodes = sample_nodes(w, nsamples, 23)
+    rows = lambda idx: d[idx, None] * inputs.multivector(w.seed, w.ndof, nvec, rows=idx)
+    Yo = d[nodes, None] * oo.apply_at_nodes(rows, nodes)
+    Yg = Yv[torch.from_numpy(nodes).cuda()].cpu().numpy()
+    err = float(np.abs(Yg - Yo).max() / scale)
+    assert err <= TOL, (w.name, nvec, op.kernel_name(nvec), err)
+    V = torch.empty_like(X); AV = torch.empty_like(X)
+    binding.fill_uniform(V, w.seed + 1000)
+    op.apply(V, AV, nvec); torch.cuda.synchronize()
+    a = float((X * AV).sum().item()); b = float((V * Y).sum().item())
+    assert abs(a - b) <= 1e-10 * max(abs(a), abs(b), 1.0)
+    return op.kernel_name(nvec)
+
+
+def test_cfg2_full_eigen_operator(env):
+    w = inputs.configs()[2]
+    assert run_full_eigen_operator(env, w, w.nvec) == "fe_apply_cart_plane"
+
+
+def test_cfg4_full_eigen_operator(env):
+    w = inputs.configs()[4]
+    assert run_full_eigen_operator(env, w, 16) == "fe_apply_cart_line"
+
+
+def test_cfg3_full_eigen_operator(env):
+    w = inputs.configs()[3]
+    assert run_full_eigen_operator(env, w, w.nvec, nsamples=10) == "fe_apply_gen_tma"
