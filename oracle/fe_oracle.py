@@ -496,3 +496,50 @@ def lanczos_upper_bound(apply, v0: np.ndarray, k: int = 10) -> float:
         v_prev, v = v, w / beta
     T = np.diag(alphas) + np.diag(betas[:-1], 1) + np.diag(betas[:-1], -1)
     return float(np.linalg.eigvalsh(T)[-1] + betas[-1])
+
+
+# --------------------------------------------------------------------------------------
+# Chebyshev filtered subspace iteration (Alg. 6)
+# --------------------------------------------------------------------------------------
+
+def chfsi_iterate(apply, U: np.ndarray, m: int, lam_max: float, lam_u: float, lam_min: float, free=None):
+    """One pass of Alg. 6 lines 2-20: filter U with degree m damping [lam_u, lam_max] (lines 2-17), orthogonalise the
+    filtered block (line 18; any orthonormal basis of its span: Householder QR here), solve the projected problem
+    Xo^T H Xo Q = Q Lambda (line 19) and rotate U = Xo Q (line 20).  Returns (U, Lambda ascending, residual norms
+    ||H u_j - lambda_j u_j||_2 of line 1).
+
+    free: boolean mask of the unconstrained rows (None: all).  With C^T A C (reading 7) every constrained DoF is a
+    null vector of H~, i.e. an eigenvalue 0 inside the wanted interval; the eigenproblem is posed on the unconstrained
+    DoFs, so the subspace must keep exact zeros in the constrained rows.  The filter and the rotation do; a Householder
+    QR of the whole block would not (it mixes rows at rounding level, which later passes amplify), hence the
+    orthogonalisation acts on the free rows."""
+    Y = chebyshev_filter(apply, U, m, lam_u, lam_max, lam_min)
+    if free is None:
+        Xo, _ = np.linalg.qr(Y)
+    else:
+        Xo = np.zeros_like(Y)
+        Xo[free], _ = np.linalg.qr(Y[free])
+    HX = apply(Xo)
+    T = Xo.T @ HX
+    lam, Q = np.linalg.eigh((T + T.T) / 2.0)
+    Un = Xo @ Q
+    R = apply(Un) - Un * lam[None, :]
+    return Un, lam, np.linalg.norm(R, axis=0)
+
+
+def chfsi_solve(apply, U0: np.ndarray, n_wanted: int, m: int, lam_max: float, lam_u: float, lam_min: float,
+                tau: float, max_iter: int = 50, free=None):
+    """Alg. 6 line 1 loop: repeat chfsi_iterate until the n_wanted lowest pairs have residual <= tau.  The paper takes
+    the bounds as data and is silent on how they follow the iteration; reading (Zhou-Saad [37]): after
+    each pass lam_min <- lowest Ritz value, lam_u <- highest Ritz value of the subspace (the vectors beyond n_wanted
+    are the buffer).  Returns (U, Lambda, residuals, passes)."""
+    U = np.array(U0, dtype=np.float64)
+    if free is not None:
+        U[~free] = 0.0
+    lam = res = None
+    for it in range(1, max_iter + 1):
+        U, lam, res = chfsi_iterate(apply, U, m, lam_max, lam_u, lam_min, free)
+        if res[:n_wanted].max() <= tau:
+            return U, lam, res, it
+        lam_min, lam_u = float(lam[0]), float(lam[-1])
+    return U, lam, res, max_iter
