@@ -165,6 +165,8 @@ int fe_probe_peaks(double *fp64_tflops, double *hbm_gbs, int cuda_device);
 /* Introspection used by bench.py / tests: vectors per thread block chosen for this nvec, the
  * number of kernel launches the last call enqueued, and the dominant kernel's name. */
 int fe_mf_batch_width(const fe_mf_ctx *ctx, int nvec);
+/* Nodes per direction nd[3] (HOST), boundary condition FE_BC_* and the CUDA device of the context. */
+int fe_mf_shape(const fe_mf_ctx *ctx, int nd[3], int *bc, int *cuda_device);
 const char *fe_mf_kernel_name(const fe_mf_ctx *ctx, int nvec);   /* static string, never NULL */
 int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
 

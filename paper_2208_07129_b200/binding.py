@@ -34,6 +34,7 @@ SYMBOLS = {
     "fe_fill_uniform": (C.c_int, [C.c_void_p, C.c_longlong, C.c_ulonglong, C.c_longlong, C.c_void_p]),
     "fe_probe_peaks": (C.c_int, [_PD, _PD, C.c_int]),
     "fe_mf_batch_width": (C.c_int, [C.c_void_p, C.c_int]),
+    "fe_mf_shape": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "fe_mf_kernel_name": (C.c_char_p, [C.c_void_p, C.c_int]),
     "fe_mf_last_launch_count": (C.c_int, [C.c_void_p]),
     "fe_mf_set_variant": (C.c_int, [C.c_void_p, C.c_int]),

@@ -2,7 +2,8 @@
 
     python -m paper_2208_07129_b200.build [--force] [--verbose]
 
-Produces paper_2208_07129_b200/csrc/libfe_mf.so (git-ignored; it travels with gpurun snapshots).
+Produces paper_2208_07129_b200/csrc/libfe_mf.so (git-ignored; it travels with gpurun snapshots) and, beside it,
+libfe_chfsi.so (include/fe_chfsi.h: the subspace iteration around the operator; links libfe_mf.so, cuBLAS, cuSOLVER).
 """
 from __future__ import annotations
 
@@ -26,6 +27,11 @@ NVCC_FLAGS = [
 ]
 
 
+LIB_CHFSI = os.path.join(CSRC, "libfe_chfsi.so")
+CHFSI_SOURCES = ["fe_chfsi.cu"]
+CHFSI_DEPS = [os.path.join("..", "..", "include", "fe_chfsi.h"), os.path.join("..", "..", "include", "fe_mf.h")]
+
+
 def nvcc_path() -> str:
     for cand in (os.environ.get("NVCC"), shutil.which("nvcc"), "/usr/local/cuda/bin/nvcc"):
         if cand and os.path.exists(cand):
@@ -44,6 +50,31 @@ def needs_build() -> bool:
     return False
 
 
+def _stale(lib: str, files) -> bool:
+    if not os.path.exists(lib):
+        return True
+    t = os.path.getmtime(lib)
+    return any(os.path.exists(os.path.join(CSRC, f)) and os.path.getmtime(os.path.join(CSRC, f)) > t for f in files)
+
+
+def build_chfsi(force: bool = False, verbose: bool = False) -> str:
+    """libfe_chfsi.so; a separate library so that libfe_mf.so itself depends on nothing but the CUDA runtime."""
+    build(force=False, verbose=verbose)
+    if not force and not _stale(LIB_CHFSI, CHFSI_SOURCES + CHFSI_DEPS) and os.path.getmtime(LIB_CHFSI) >= os.path.getmtime(LIB):
+        return LIB_CHFSI
+    nvcc = nvcc_path()
+    cuda_lib = os.path.join(os.path.dirname(os.path.dirname(os.path.realpath(nvcc))), "lib64")
+    cmd = [nvcc] + NVCC_FLAGS + [os.path.join(CSRC, s) for s in CHFSI_SOURCES] + \
+          ["-o", LIB_CHFSI, "-L" + CSRC, "-lfe_mf", "-lcublas", "-lcusolver",
+           "-Xlinker", "-rpath=$ORIGIN", "-Xlinker", "-rpath=" + cuda_lib]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or res.returncode != 0:
+        sys.stderr.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed building libfe_chfsi.so")
+    return LIB_CHFSI
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
@@ -59,3 +90,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build_chfsi(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -281,6 +281,14 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
 
 extern "C" long long fe_mf_ndofs(const fe_mf_ctx* ctx) { return ctx ? ctx->ndof : -1; }
 
+extern "C" int fe_mf_shape(const fe_mf_ctx* ctx, int nd[3], int* bc, int* cuda_device) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (nd) { nd[0] = ctx->ndx; nd[1] = ctx->ndy; nd[2] = ctx->ndz; }
+  if (bc) *bc = ctx->bc;
+  if (cuda_device) *cuda_device = ctx->device;
+  return FE_MF_OK;
+}
+
 extern "C" const char* fe_mf_last_error(const fe_mf_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {

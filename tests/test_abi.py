@@ -11,8 +11,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def header_symbols():
-    src = open(os.path.join(ROOT, "include", "fe_mf.h")).read()
+def header_symbols(header="fe_mf.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(fe_[a-z0-9_]+)\s*\(", src)))
 
@@ -39,6 +39,22 @@ def test_binding_table_matches_header(built_lib):
     from paper_2208_07129_b200 import binding
     assert sorted(binding.SYMBOLS) == header_symbols()
     binding.lib()
+
+
+def test_chfsi_library_exports_every_declared_symbol(built_lib):
+    """include/fe_chfsi.h (SURVEY.md 8(f) NEXT-3): libfe_chfsi.so builds, loads and exports what the header declares;
+    the binding's table matches."""
+    from paper_2208_07129_b200 import build, chfsi
+    path = build.build_chfsi()
+    ctypes.CDLL(built_lib, mode=ctypes.RTLD_GLOBAL)
+    lib = ctypes.CDLL(path)
+    syms = [s for s in header_symbols("fe_chfsi.h") if s.startswith("fe_chfsi_")]
+    assert "fe_chfsi_solve" in syms and "fe_chfsi_iterate" in syms
+    for name in syms:
+        assert hasattr(lib, name), name
+    assert sorted(chfsi.SYMBOLS) == syms
+    from paper_2208_07129_b200 import binding
+    assert chfsi.lib().fe_chfsi_solve(None, None, 1, 1, 1.0, 0.5, 0.0, 1e-3, 1, None, None, None, None) == binding.FE_MF_EINVAL
 
 
 def test_no_cpu_fallback(built_lib):
