@@ -5,9 +5,13 @@
  *   line 1       while ||H U - U Lambda|| > tau                  fe_chfsi_solve
  *   lines 2-17   Chebyshev filter                                fe_cheb_filter (fe_mf.h, hand-written kernels)
  *   line 18      Xo <- orthogonalize(X)                          Cholesky QR, twice: S = X^T X (cuBLAS DSYRK),
- *                                                                S = L L^T (cuSOLVER DPOTRF), X <- X L^-T (DTRSM)
+ *                                                                S = L L^T (cuSOLVER DPOTRF), X <- X L^-T (DGEMM with
+ *                                                                the explicit n x n inverse)
  *   line 19      Xo^T H Xo Q = Q Lambda                          fe_mf_apply, DGEMM, cuSOLVER DSYEVD
  *   line 20      U <- Xo Q                                       DGEMM
+ *                In fe_chfsi_iterate / fe_chfsi_solve the second Cholesky-QR round is folded into lines 19-20 as the
+ *                generalised problem (X1^T H X1) Z = (X1^T X1) Z Lambda, U = X1 Z (cuSOLVER DSYGVD): same U, one tall
+ *                DGEMM less.
  *   line 1       r_j = ||H u_j - lambda_j u_j||_2                fe_mf_apply + a column-norm kernel
  *
  * The operator is whatever the fe_mf context applies (H~ = M^-1/2 (K + M^kappa) M^-1/2 once fe_mf_set_kappa /

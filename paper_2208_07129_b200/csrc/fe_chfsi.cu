@@ -9,6 +9,8 @@
 #include <cusolverDn.h>
 
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -26,6 +28,7 @@ struct fe_chfsi {
   double* work = nullptr; int lwork = 0; int* info = nullptr;
   double* lv = nullptr;                     // 3 Lanczos vectors, allocated on first use
   cudaEvent_t ev[8] = {};
+  cudaEvent_t ev_end = nullptr;
   double ms[6] = {0, 0, 0, 0, 0, 0};
   std::string err;
 };
@@ -128,8 +131,16 @@ int zero_constrained(fe_chfsi* h, double* U, int nvec, cudaStream_t st) {
   return FE_MF_OK;
 }
 
-// Cholesky QR, one round: S = X^T X, S = L L^T, X <- X L^-T  (X row-major [ndof][nvec] = column-major nvec x ndof)
-int cholqr_round(fe_chfsi* h, double* X, cudaStream_t st) {
+__global__ void set_identity(double* __restrict__ A, int n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < (long long)n * n) A[i] = (i / n == i % n) ? 1.0 : 0.0;
+}
+
+// Cholesky QR, one round (X row-major [ndof][nvec] = column-major nvec x ndof): S = X^T X, S = L L^T,
+// dst <- X L^-T (dst != X).  The triangular solve of the tall block is done as a DGEMM with the explicit n x n
+// inverse L^-1 (measured on the B200, n = 1024, n_dof = 884736: DTRSM 95 ms, DGEMM 53 ms; the second round removes
+// what the explicit inverse loses).  h->T holds L^-1 afterwards.
+int cholqr_round(fe_chfsi* h, const double* X, double* dst, cudaStream_t st) {
   const int n = h->nvec, k = (int)h->ndof;
   const double one = 1.0, zero = 0.0;
   CH_BLAS(h, cublasDsyrk(h->blas, CUBLAS_FILL_MODE_LOWER, CUBLAS_OP_N, n, k, &one, X, n, &zero, h->S, n));
@@ -140,8 +151,11 @@ int cholqr_round(fe_chfsi* h, double* X, cudaStream_t st) {
   if (info != 0)
     return fail(h, FE_MF_EINVAL, "orthonormalisation: X^T X is not positive definite (block numerically rank deficient, potrf info " +
                                      std::to_string(info) + ")");
-  CH_BLAS(h, cublasDtrsm(h->blas, CUBLAS_SIDE_LEFT, CUBLAS_FILL_MODE_LOWER, CUBLAS_OP_N, CUBLAS_DIAG_NON_UNIT, n, k, &one,
-                         h->S, n, X, n));
+  set_identity<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, st>>>(h->T, n);
+  CH_CUDA(h, cudaGetLastError());
+  CH_BLAS(h, cublasDtrsm(h->blas, CUBLAS_SIDE_LEFT, CUBLAS_FILL_MODE_LOWER, CUBLAS_OP_N, CUBLAS_DIAG_NON_UNIT, n, n, &one,
+                         h->S, n, h->T, n));                                                     // T = L^-1
+  CH_BLAS(h, cublasDgemm(h->blas, CUBLAS_OP_N, CUBLAS_OP_N, n, k, n, &one, h->T, n, X, n, &zero, dst, n));
   return FE_MF_OK;
 }
 
@@ -152,10 +166,23 @@ int set_stream(fe_chfsi* h, cudaStream_t st) {
 }
 
 int orthonormalize_impl(fe_chfsi* h, double* X, cudaStream_t st) {
-  // twice: the first round leaves ||X^T X - I|| ~ eps cond(X)^2, the second brings it to eps
-  int rc = cholqr_round(h, X, st);
-  if (rc == FE_MF_OK) rc = cholqr_round(h, X, st);
+  // twice: the first round leaves ||X^T X - I|| ~ eps cond(X)^2, the second brings it to eps  (X -> W -> X)
+  int rc = cholqr_round(h, X, h->W, st);
+  if (rc == FE_MF_OK) rc = cholqr_round(h, h->W, X, st);
   return rc;
+}
+
+// h->res[c] = || HU[:,c] - lam[c] U[:,c] ||^2  (device)
+int residual_norms(fe_chfsi* h, const double* HU, const double* U, cudaStream_t st) {
+  const int n = h->nvec;
+  CH_CUDA(h, cudaMemsetAsync(h->res, 0, sizeof(double) * n, st));
+  int cw = 1;
+  while (cw * 2 <= n && cw < 256) cw *= 2;
+  const long long blocks = 148LL * 8;
+  const long long rpb = (h->ndof + blocks - 1) / blocks;
+  residual_sq_kernel<<<(unsigned)((h->ndof + rpb - 1) / rpb), 256, 0, st>>>(HU, U, h->lam, h->res, h->ndof, n, cw, rpb);
+  CH_CUDA(h, cudaGetLastError());
+  return FE_MF_OK;
 }
 
 int rayleigh_ritz_impl(fe_chfsi* h, const double* X, double* U, double* evals_host, double* resid_host, cudaStream_t st) {
@@ -177,13 +204,10 @@ int rayleigh_ritz_impl(fe_chfsi* h, const double* X, double* U, double* evals_ho
   CH_CUDA(h, cudaEventRecord(h->ev[6], st));
   CH_OP(h, fe_mf_apply(h->op, U, h->W, n, st));                                                   // W = H U
   CH_CUDA(h, cudaEventRecord(h->ev[7], st));
-  CH_CUDA(h, cudaMemsetAsync(h->res, 0, sizeof(double) * n, st));
-  int cw = 1;
-  while (cw * 2 <= n && cw < 256) cw *= 2;
-  const long long blocks = 148LL * 8;
-  const long long rpb = (h->ndof + blocks - 1) / blocks;
-  residual_sq_kernel<<<(unsigned)((h->ndof + rpb - 1) / rpb), 256, 0, st>>>(h->W, U, h->lam, h->res, h->ndof, n, cw, rpb);
-  CH_CUDA(h, cudaGetLastError());
+  {
+    const int rc = residual_norms(h, h->W, U, st);
+    if (rc != FE_MF_OK) return rc;
+  }
   CH_CUDA(h, cudaEventRecord(h->ev[0], st));   // reused as the end mark
   std::vector<double> r(n);
   if (evals_host) CH_CUDA(h, cudaMemcpyAsync(evals_host, h->lam, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
@@ -229,11 +253,16 @@ extern "C" int fe_chfsi_create(fe_chfsi** out, fe_mf_ctx* op, int nvec) {
     ok = cusolverDnDpotrf_bufferSize(h->sol, CUBLAS_FILL_MODE_LOWER, nvec, h->S, nvec, &l1) == CUSOLVER_STATUS_SUCCESS &&
          cusolverDnDsyevd_bufferSize(h->sol, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, nvec, h->T, nvec, h->lam, &l2) ==
              CUSOLVER_STATUS_SUCCESS;
+    int l3 = 0;
+    ok = ok && cusolverDnDsygvd_bufferSize(h->sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, nvec,
+                                           h->T, nvec, h->S, nvec, h->lam, &l3) == CUSOLVER_STATUS_SUCCESS;
     h->lwork = l1 > l2 ? l1 : l2;
+    if (l3 > h->lwork) h->lwork = l3;
     if (h->lwork < 1) h->lwork = 1;
     ok = ok && cudaMalloc(&h->work, (size_t)h->lwork * sizeof(double)) == cudaSuccess;
   }
   for (int i = 0; ok && i < 8; ++i) ok = cudaEventCreate(&h->ev[i]) == cudaSuccess;
+  ok = ok && cudaEventCreate(&h->ev_end) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
     fe_chfsi_destroy(h);
@@ -252,6 +281,7 @@ extern "C" void fe_chfsi_destroy(fe_chfsi* h) {
   for (double* b : bufs) if (b) cudaFree(b);
   if (h->info) cudaFree(h->info);
   for (int i = 0; i < 8; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  if (h->ev_end) cudaEventDestroy(h->ev_end);
   delete h;
 }
 
@@ -335,19 +365,52 @@ extern "C" int fe_chfsi_iterate(fe_chfsi* h, double* U_dev, int m, double lam_ma
   if (rc != FE_MF_OK) return rc;
   rc = zero_constrained(h, U_dev, h->nvec, st);
   if (rc != FE_MF_OK) return rc;
+  const int n = h->nvec, k = (int)h->ndof;
+  const double one = 1.0, zero = 0.0;
   CH_CUDA(h, cudaEventRecord(h->ev[0], st));
-  CH_OP(h, fe_cheb_filter(h->op, U_dev, h->Y, h->nvec, m, lam_u, lam_max, lam_min, st));        // lines 2-17
+  CH_OP(h, fe_cheb_filter(h->op, U_dev, h->Y, n, m, lam_u, lam_max, lam_min, st));              // lines 2-17: Y
   CH_CUDA(h, cudaEventRecord(h->ev[1], st));
-  rc = orthonormalize_impl(h, h->Y, st);                                                          // line 18
+  // line 18, first Cholesky-QR round: X1 = Y L1^-T -> W.  The second round is folded into lines 19-20: with
+  // S2 = X1^T X1 = L2 L2^T (= I up to eps cond(Y)^2) the orthonormal block is Xo = X1 L2^-T, and
+  // Xo^T H Xo Q = Q Lambda, U = Xo Q  <=>  (X1^T H X1) Z = S2 Z Lambda, Z^T S2 Z = I, U = X1 Z  (Z = L2^-T Q),
+  // which DSYGVD solves: one tall DGEMM and the DTRSM of the second round are saved.
+  rc = cholqr_round(h, h->Y, h->W, st);
   if (rc != FE_MF_OK) return rc;
+  CH_BLAS(h, cublasDsyrk(h->blas, CUBLAS_FILL_MODE_LOWER, CUBLAS_OP_N, n, k, &one, h->W, n, &zero, h->S, n));   // S2
   CH_CUDA(h, cudaEventRecord(h->ev[2], st));
+  CH_OP(h, fe_mf_apply(h->op, h->W, h->Y, n, st));                                                // Y = H X1
+  CH_CUDA(h, cudaEventRecord(h->ev[3], st));
+  CH_BLAS(h, cublasDgemm(h->blas, CUBLAS_OP_N, CUBLAS_OP_T, n, n, k, &one, h->W, n, h->Y, n, &zero, h->T, n));   // X1^T H X1
+  CH_CUDA(h, cudaEventRecord(h->ev[4], st));
+  CH_SOL(h, cusolverDnDsygvd(h->sol, CUSOLVER_EIG_TYPE_1, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, h->T, n,
+                             h->S, n, h->lam, h->work, h->lwork, h->info));                       // line 19
+  int info = 0;
+  CH_CUDA(h, cudaMemcpyAsync(&info, h->info, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CH_CUDA(h, cudaEventRecord(h->ev[5], st));
+  CH_BLAS(h, cublasDgemm(h->blas, CUBLAS_OP_T, CUBLAS_OP_N, n, k, n, &one, h->T, n, h->W, n, &zero, U_dev, n));  // line 20
+  CH_CUDA(h, cudaEventRecord(h->ev[6], st));
+  CH_OP(h, fe_mf_apply(h->op, U_dev, h->Y, n, st));                                               // Y = H U
+  CH_CUDA(h, cudaEventRecord(h->ev[7], st));
+  rc = residual_norms(h, h->Y, U_dev, st);                                                        // line 1
+  if (rc != FE_MF_OK) return rc;
+  cudaEvent_t end = h->ev_end;
+  CH_CUDA(h, cudaEventRecord(end, st));
+  std::vector<double> r(n);
+  if (evals_host) CH_CUDA(h, cudaMemcpyAsync(evals_host, h->lam, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+  CH_CUDA(h, cudaMemcpyAsync(r.data(), h->res, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
   CH_CUDA(h, cudaStreamSynchronize(st));
-  float t0 = 0.f, t1 = 0.f;
-  cudaEventElapsedTime(&t0, h->ev[0], h->ev[1]);
-  cudaEventElapsedTime(&t1, h->ev[1], h->ev[2]);
-  rc = rayleigh_ritz_impl(h, h->Y, U_dev, evals_host, resid_host, st);                            // lines 19-20, 1
-  h->ms[0] = t0; h->ms[1] = t1;
-  return rc;
+  if (info != 0)
+    return fail(h, info > n ? FE_MF_EINVAL : FE_MF_ECUDA,
+                info > n ? "orthonormalisation: second-round Gram matrix not positive definite" : "cusolverDnDsygvd did not converge");
+  if (resid_host) for (int j = 0; j < n; ++j) resid_host[j] = std::sqrt(r[j]);
+  auto el = [](cudaEvent_t a, cudaEvent_t b) { float t = 0.f; cudaEventElapsedTime(&t, a, b); return (double)t; };
+  h->ms[0] = el(h->ev[0], h->ev[1]);
+  h->ms[1] = el(h->ev[1], h->ev[2]);
+  h->ms[2] = el(h->ev[2], h->ev[3]) + el(h->ev[6], h->ev[7]);
+  h->ms[3] = el(h->ev[3], h->ev[4]) + el(h->ev[5], h->ev[6]);
+  h->ms[4] = el(h->ev[4], h->ev[5]);
+  h->ms[5] = el(h->ev[7], end);
+  return FE_MF_OK;
 }
 
 extern "C" int fe_chfsi_solve(fe_chfsi* h, double* U_dev, int n_wanted, int m, double lam_max, double lam_u,
