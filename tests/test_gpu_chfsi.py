@@ -130,3 +130,35 @@ def test_orthonormalize_and_rayleigh_ritz_entry_points(env):
     X[:, 3] = X[:, 1]
     with pytest.raises(binding.FeMfError):
         h.orthonormalize(torch.from_numpy(X).cuda())
+
+
+@pytest.mark.parametrize("nvec", [2, 5])
+def test_small_and_odd_blocks(env, nvec):
+    """Odd nvec (the operator falls back to its general kernel) and the smallest block the solve loop accepts."""
+    torch, orc, binding, chfsi = env
+    op, mesh, app, free = setup(env, 2, inputs.BC_DIRICHLET, ncells=(3, 3, 3))
+    H = app(np.eye(mesh.ndof))
+    ref = np.linalg.eigvalsh(H[np.ix_(free, free)])
+    U0 = inputs.multivector(99, mesh.ndof, nvec)
+    h = chfsi.Chfsi(op, nvec)
+    b = h.lanczos_bound(torch.from_numpy(U0[:, 0].copy()).cuda(), 12)
+    Ud = torch.from_numpy(U0).cuda()
+    lam, res, it = h.solve(Ud, 1, 16, b, ref[0] + 0.3 * (b - ref[0]), ref[0] - 1.0, 1e-9, 200)
+    assert res[0] <= 1e-9 and abs(lam[0] - ref[0]) <= 1e-9 * np.abs(ref).max()
+
+
+def test_argument_errors(env):
+    torch, orc, binding, chfsi = env
+    op, mesh, app, free = setup(env, 2, inputs.BC_PERIODIC, ncells=(2, 2, 2))
+    with pytest.raises(binding.FeMfError):
+        chfsi.Chfsi(op, 0)
+    h = chfsi.Chfsi(op, 4)
+    U = torch.from_numpy(inputs.multivector(1, mesh.ndof, 4)).cuda()
+    with pytest.raises(binding.FeMfError) as e:
+        h.solve(U, 5, 8, 10.0, 5.0, 0.0, 1e-6)            # n_wanted > nvec
+    assert e.value.code == binding.FE_MF_EINVAL
+    with pytest.raises(binding.FeMfError) as e:
+        h.iterate(U, 8, 10.0, 12.0, 0.0)                   # inverted filter interval: fe_cheb_filter refuses
+    assert e.value.code == binding.FE_MF_EINVAL
+    with pytest.raises(binding.FeMfError):
+        h.rayleigh_ritz(U, U)
