@@ -172,7 +172,8 @@ int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
 
 /* Select a kernel variant (0 = default: chosen from degree, geometry and nvec).  For profiling/ablation only:
  * 1 general fallback kernel, 2 one-vector-per-thread Cartesian kernel (LDG/RED), 7 full-metric TMA kernel on a
- * Cartesian mesh, 8 plane kernel (p = 6, 7), 10 / 11 line kernel with 16 / 8 vectors per block, 19 plane kernel
+ * Cartesian mesh, 8 plane kernel (p = 6, 7), 10 / 11 line kernel with 16 / 8 vectors per block, 12 Kronecker-product kernel (uniform box, constant
+ * kappa; fe_kernels_kron.cuh), 19 plane kernel
  * that also initialises the output (one cooperative launch).  Returns EINVAL if unknown. */
 int fe_mf_set_variant(fe_mf_ctx *ctx, int variant);
 

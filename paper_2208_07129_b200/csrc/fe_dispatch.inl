@@ -234,7 +234,7 @@ int line_bv(const fe_mf_ctx* c, int nvec) {
 }
 
 // 8-vector blocks with an even number of nodes per direction: one pad node per x-row (see DenseTile)
-constexpr int line_padx(int p, int bv) { return (bv == 8 && (p + 1) % 2 == 0 && p >= 3) ? 1 : 0; }
+constexpr int line_padx(int p, int bv) { return ((bv == 8 || bv == 4) && (p + 1) % 2 == 0 && p >= 3) ? 1 : 0; }
 
 template <int PDEG, int CFG, bool IDENT = false, bool EIG = false>
 cudaError_t launch_line_id(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
@@ -262,6 +262,45 @@ cudaError_t launch_line(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CU
   return prm.idw != 0.0 ? launch_line_id<PDEG, CFG, true>(c, prm, tw, tz, st) : launch_line_id<PDEG, CFG, false>(c, prm, tw, tz, st);
 }
 
+// ---- kind 10: Kronecker kernel (uniform box, constant kappa): three tiles.  Variant 12 only: measured on the B200 it
+// is no faster than the plane / line kernels (p = 6: 146 vs 144, p = 7: 121 vs 129 GDoF*vec/s; one vector per thread
+// with twice the warps: 134 / 114) -- 25 % fewer FP64 instructions, but the same 10 tile accesses per point as the
+// plane kernel and three short phases per item
+template <int PDEG> struct KronCfg;
+template <> struct KronCfg<1> { static constexpr int BV = 8, NT = 32, MINB = 4, VPT = 2; };
+template <> struct KronCfg<2> { static constexpr int BV = 8, NT = 64, MINB = 4, VPT = 2; };
+template <> struct KronCfg<3> { static constexpr int BV = 8, NT = 64, MINB = 4, VPT = 2; };
+template <> struct KronCfg<4> { static constexpr int BV = 8, NT = 128, MINB = 4, VPT = 2; };
+template <> struct KronCfg<5> { static constexpr int BV = 8, NT = 160, MINB = 4, VPT = 2; };
+template <> struct KronCfg<6> { static constexpr int BV = 8, NT = 224, MINB = 2, VPT = 2; };
+// p = 7, 8: the y-pass holds two lines and three products of two vectors (~150-160 registers): 4-vector blocks keep
+// three / two blocks per SM resident without spills
+template <> struct KronCfg<7> { static constexpr int BV = 4, NT = 128, MINB = 3, VPT = 2; };
+template <> struct KronCfg<8> { static constexpr int BV = 4, NT = 192, MINB = 2, VPT = 2; };
+int kron_bv(int p) { return p >= 7 ? 4 : 8; }
+
+template <int PDEG, bool IDENT>
+cudaError_t launch_kron_id(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                           cudaStream_t st) {
+  using C = KronCfg<PDEG>;
+  constexpr int BV = C::BV, PADX = line_padx(PDEG, BV);
+  constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, BV, PADX>::PITCH + 64;
+  static int bps = 0;
+  auto kern = fe::fe_apply_cart_kron<PDEG, BV, C::NT, C::MINB, PADX, IDENT, C::VPT>;
+  const long long nitems = c->ncells * prm.nvb;
+  long long grid = 0;
+  cudaError_t e = persistent_grid(kern, C::NT, SMEM, bps, c, nitems, grid);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->ctrl, 0, 16, st);
+  if (e != cudaSuccess) return e;
+  kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
+  return cudaGetLastError();
+}
+template <int PDEG>
+cudaError_t launch_kron(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
+                        cudaStream_t st) {
+  return prm.idw != 0.0 ? launch_kron_id<PDEG, true>(c, prm, tw, tz, st) : launch_kron_id<PDEG, false>(c, prm, tw, tz, st);
+}
+
 // ---- which kernel serves (ctx, nvec, pointers)
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
   if (c->variant == 1) return 1;
@@ -286,6 +325,7 @@ int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
     if (!tma_ok || c->variant == 2) return 2;
     if (!trim_ok) return 2;
   }
+  if (c->variant == 12 && !eig) return 10;
   if (c->variant == 10 || c->variant == 11) return 9;
   if ((c->variant == 8 || c->variant == 19) && plane_ok(c->p)) return 8;
   // plane kernel: 16 vectors per block; worth it when the last block of vectors is mostly full
@@ -300,6 +340,7 @@ int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
     case 3: return nvec;
     case 6: return c->p == 8 ? 4 : kGenBv;
     case 8: return 16;
+    case 10: return kron_bv(c->p);
     default: return line_bv(c, nvec);
   }
 }
@@ -333,7 +374,7 @@ bool kind_fuses_init(const fe_mf_ctx* c, int kind, int nvec) {
 // Can this kernel add a multiple of W (identity term, partition-of-unity weights) in the same pass?  The Cartesian
 // plane and line kernels, at every node they write: all nodes on periodic meshes, the interior nodes on Dirichlet
 // meshes (the boundary nodes never enter a tile: callers treat them separately).
-bool kind_adds_identity(const fe_mf_ctx* c, int kind) { return (kind == 8 && c->p == 6) || kind == 9; }
+bool kind_adds_identity(const fe_mf_ctx* c, int kind) { return (kind == 8 && c->p == 6) || kind == 9 || kind == 10; }
 
 #define FE_DISPATCH_P(CALL)                                           \
   switch (c->p) {                                                     \
@@ -355,14 +396,14 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
   CUtensorMap tw, tz;
-  if (kind == 6 || kind == 8 || kind == 9) {
+  if (kind == 6 || kind == 8 || kind == 9 || kind == 10) {
     // Cartesian kernels on Dirichlet meshes: boundary nodes are out of bounds of the maps (see make_tensor_map)
     const bool trim = (kind != 6) && (c->bc == FE_BC_DIRICHLET);
-    const int padx = (kind == 9) ? line_padx(c->p, bv) : 0;
+    const int padx = (kind == 9 || kind == 10) ? line_padx(c->p, bv) : 0;
     if (!make_tensor_map(&tw, c, W, nvec, bv, trim ? 2 : 0, padx) || !make_tensor_map(&tz, c, Z, nvec, bv, trim ? 1 : 0, padx))
       return fail(c, FE_MF_ECUDA, "cuTensorMapEncodeTiled failed");
   }
-  if (kind == 8 || kind == 9 || kind == 2 || kind == 3)
+  if (kind == 8 || kind == 9 || kind == 10 || kind == 2 || kind == 3)
     for (int k = 0; k < 7; ++k) P.ug[k] *= alpha;   // Cartesian kernels: the result is linear in the metric constants
   if ((kind == 8 || kind == 9) && c->mass_scaled) {
     // EIG kernels: diag(M)^-1/2 = (det J)^-1/2 kron diag(w~)^-1/2; the tables carry the second factor (both sides)
@@ -375,6 +416,10 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
 #undef FE_CALL
   } else if (kind == 6) {
 #define FE_CALL(p_) launch_gen<p_>(c, P, tw, tz, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
+  } else if (kind == 10) {
+#define FE_CALL(p_) launch_kron<p_>(c, P, tw, tz, st)
     FE_DISPATCH_P(FE_CALL)
 #undef FE_CALL
   } else if (kind == 8) {
@@ -650,6 +695,7 @@ extern "C" const char* fe_mf_kernel_name(const fe_mf_ctx* ctx, int nvec) {
     case 3: return "fe_apply_cart<CELLS>";
     case 6: return "fe_apply_gen_tma";
     case 8: return "fe_apply_cart_plane";
+    case 10: return "fe_apply_cart_kron";
     default: return "fe_apply_cart_line";
   }
 }
@@ -659,7 +705,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
   const bool known = variant == 0 || variant == 1 || variant == 2 || variant == 7 || variant == 8 || variant == 10 ||
-                     variant == 11 || variant == 19;
+                     variant == 11 || variant == 12 || variant == 19;
   if (!known) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;

@@ -38,7 +38,7 @@ struct EoTab2 {
   double midm, midmh;       // M[mid][mid] and half of it
   double pad[2];
 };
-__constant__ EoTab2 c_eo2[KMAXN][4];   // [p][MAT_NS | MAT_DS | MAT_SH | MAT_NSS]
+__constant__ EoTab2 c_eo2[KMAXN][6];   // [p][MAT_NS | MAT_DS | MAT_SH | MAT_NSS | MAT_M1 | MAT_K1]
 
 // The primitives are generic in the value type T: double (one vector per thread, plane kernels) or v2 (two
 // vectors per thread, line kernels).

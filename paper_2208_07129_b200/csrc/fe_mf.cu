@@ -17,6 +17,7 @@
 #include "fe_kernels_gen.cuh"
 #include "fe_kernels_plane.cuh"
 #include "fe_kernels_line.cuh"
+#include "fe_kernels_kron.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {
@@ -78,9 +79,9 @@ struct DeviceGuard {
 
 // Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
 // 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
-void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[4]) {
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[6]) {
   const int n = t.n, h = n / 2, m = n / 2;
-  long double M[6][fe::MAXN * fe::MAXN];
+  long double M[8][fe::MAXN * fe::MAXN];
   for (int q = 0; q < n; ++q)
     for (int i = 0; i < n; ++i) {
       const long double sq = sqrtl(t.wl[q]), si = sqrtl(t.wl[i]);
@@ -113,8 +114,25 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[4])
       for (int q = 0; q < n; ++q) M[5][q * n + i] = M[0][q * n + i] * si;
     }
   }
-  fe::EoTab tabs[6];
-  for (int k = 0; k < 6; ++k) {
+  // M[6] = M1 = Ns^T Ns (1D mass matrix, = N^T W N) and M[7] = K1 = (Ds Ns)^T (Ds Ns) (1D stiffness matrix, = D^T W D),
+  // both with the n_q-point rule: the Kronecker factors of the cell matrix of a uniform box (fe_kernels_kron.cuh)
+  {
+    long double DN[fe::MAXN * fe::MAXN];
+    for (int q = 0; q < n; ++q)
+      for (int i = 0; i < n; ++i) {
+        long double acc = 0.0L;
+        for (int r = 0; r < n; ++r) acc += M[2][q * n + r] * M[0][r * n + i];
+        DN[q * n + i] = acc;
+      }
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) {
+        long double am = 0.0L, ak = 0.0L;
+        for (int q = 0; q < n; ++q) { am += M[0][q * n + i] * M[0][q * n + j]; ak += DN[q * n + i] * DN[q * n + j]; }
+        M[6][i * n + j] = am; M[7][i * n + j] = ak;
+      }
+  }
+  fe::EoTab tabs[8];
+  for (int k = 0; k < 8; ++k) {
     std::memset(&tabs[k], 0, sizeof(fe::EoTab));
     for (int q = 0; q < h; ++q) {
       for (int i = 0; i < h; ++i) {
@@ -131,8 +149,8 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[4])
   for (int k = 0; k < 5; ++k) out[k] = tabs[k];
   // the plane / line kernels' tables: Ns, Ds (the transposes reuse them) and Ds^T Ds / 2, plus the halved middle
   // column / row
-  const int src[4] = {0, 2, 4, 5};
-  for (int k2 = 0; k2 < 4; ++k2) {
+  const int src[6] = {0, 2, 4, 5, 6, 7};
+  for (int k2 = 0; k2 < 6; ++k2) {
     const fe::EoTab& s = tabs[src[k2]];
     fe::EoTab2& d = out2[k2];
     std::memset(&d, 0, sizeof(fe::EoTab2));
@@ -202,10 +220,10 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
   if (e == cudaSuccess) {
     fe::EoTab eo[5];
-    fe::EoTab2 eo2[4];
+    fe::EoTab2 eo2[6];
     make_eo_tables(tab, eo, eo2);
     e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 5 * p);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 4 * p);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 6 * p);
   }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
 
