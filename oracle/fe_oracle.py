@@ -159,10 +159,10 @@ def collocation_derivative_1d(p: int, nq: int | None = None) -> np.ndarray:
 # --------------------------------------------------------------------------------------
 
 
-def tables_3d(p: int):
+def tables_3d(p: int, nq: int | None = None):
     """Dense Nf[Q][I], Df[s][Q][I] (s = 0,1,2) and W[Q] with I = i1 + n i2 + n^2 i3 (Eq. 18 order,
     PAPER.md:308) and Q = q1 + n q2 + n^2 q3."""
-    _, _, w, N1, D1 = tables_1d(p)
+    _, _, w, N1, D1 = tables_1d(p, nq)
     # np.kron(A, B)[a*nb + b', ...]: the LEFT factor carries the slowest index.
     Nf = np.kron(N1, np.kron(N1, N1))
     Df = np.stack([
@@ -174,13 +174,16 @@ def tables_3d(p: int):
     return Nf, Df, W
 
 
-def reference_points_3d(p: int):
+def reference_points_3d(p: int, nq: int | None = None):
     """(n^3, 3) quadrature points in Q order and (n^3, 3) GLL nodes in I order."""
-    xi, xq, _, _, _ = tables_1d(p)
+    xi, xq, _, _, _ = tables_1d(p, nq)
     n = p + 1
-    q = np.arange(n ** 3)
-    i1, i2, i3 = q % n, (q // n) % n, q // (n * n)
-    return np.stack([xq[i1], xq[i2], xq[i3]], 1), np.stack([xi[i1], xi[i2], xi[i3]], 1)
+    nq = n if nq is None else nq
+    q = np.arange(nq ** 3)
+    q1, q2, q3 = q % nq, (q // nq) % nq, q // (nq * nq)
+    i = np.arange(n ** 3)
+    i1, i2, i3 = i % n, (i // n) % n, i // (n * n)
+    return np.stack([xq[q1], xq[q2], xq[q3]], 1), np.stack([xi[i1], xi[i2], xi[i3]], 1)
 
 
 # --------------------------------------------------------------------------------------
@@ -307,12 +310,12 @@ class Mesh:
         return out
 
 
-def quadrature_point_coordinates(mesh: Mesh) -> np.ndarray:
+def quadrature_point_coordinates(mesh: Mesh, nq: int | None = None) -> np.ndarray:
     """(ncells, n_q^3, 3) physical coordinates x_Q^(e) of the quadrature points, cells in
     lexicographic order (x fastest), Q = q1 + n q2 + n^2 q3."""
-    qp, _ = reference_points_3d(mesh.p)
+    qp, _ = reference_points_3d(mesh.p, nq)
     ncx, ncy, ncz = mesh.ncells
-    out = np.zeros((ncx * ncy * ncz, mesh.n ** 3, 3))
+    out = np.zeros((ncx * ncy * ncz, qp.shape[0], 3))
     for ez in range(ncz):
         for ey in range(ncy):
             for ex in range(ncx):
@@ -346,15 +349,17 @@ class Operator:
     K + sigma M."""
 
     def __init__(self, mesh: Mesh, sigma: float, ck: float = 1.0, cm: float = 1.0, form_matrices: bool = False,
-                 kappa=None):
+                 kappa=None, nq: int | None = None):
         """kappa: None (constant sigma) or an array [ncells][n_q^3] of values at the quadrature points of every cell
         (cells in lexicographic order, x fastest; Eq. 22, the "precomputed potential" of
-        PAPER.md:796), which then replaces sigma."""
+        PAPER.md:796), which then replaces sigma.  nq: Gauss points per direction, n_p = p + 1 by default; the paper
+        also benchmarks n_q = n_p + 2."""
         self.mesh, self.sigma, self.ck, self.cm = mesh, float(sigma), float(ck), float(cm)
+        self.nq = mesh.p + 1 if nq is None else int(nq)      # points per direction; n_p + 2 = over-integration (NEXT-2)
         self.kappa = None if kappa is None else np.asarray(kappa, dtype=np.float64).reshape(
-            mesh.ncells[0] * mesh.ncells[1] * mesh.ncells[2], (mesh.p + 1) ** 3)
-        self.Nf, self.Df, self.W = tables_3d(mesh.p)
-        self.qpts, _ = reference_points_3d(mesh.p)
+            mesh.ncells[0] * mesh.ncells[1] * mesh.ncells[2], self.nq ** 3)
+        self.Nf, self.Df, self.W = tables_3d(mesh.p, self.nq)
+        self.qpts, _ = reference_points_3d(mesh.p, self.nq)
         self.form_matrices = form_matrices
         self._Ae_uniform = None
         if mesh.vertices is None and self.kappa is None:

@@ -140,12 +140,13 @@ def test_global_operator_kronecker_closed_form(bc, p):
 
 
 # ------------------------------------------------------------------ brute force, one distorted cell, long double
-def _brute_force_cell(p, verts8, sigma):
+def _brute_force_cell(p, verts8, sigma, nq=None):
     """A_e[I][J] by explicit loops over (I, J, Q) in long double with its own basis evaluation
     (monomial coefficients) and its own Jacobian (monomial form of the trilinear map)."""
     n = p + 1
+    nq = n if nq is None else nq
     xi = orc.gll_nodes(p)
-    xq, w = orc.gauss_legendre(n)
+    xq, w = orc.gauss_legendre(nq)
     # monomial coefficients of l_i, lowest degree first
     coef = []
     for i in range(n):
@@ -156,8 +157,8 @@ def _brute_force_cell(p, verts8, sigma):
         coef.append(c)
     val = lambda c, x: sum(c[k] * x ** k for k in range(len(c)))
     der = lambda c, x: sum(k * c[k] * x ** (k - 1) for k in range(1, len(c)))
-    L = np.array([[val(coef[i], xq[q]) for i in range(n)] for q in range(n)])
-    dL = np.array([[der(coef[i], xq[q]) for i in range(n)] for q in range(n)])
+    L = np.array([[val(coef[i], xq[q]) for i in range(n)] for q in range(nq)])
+    dL = np.array([[der(coef[i], xq[q]) for i in range(n)] for q in range(nq)])
     # trilinear map in monomial form: x = sum_{abc in {0,1}} m[abc] xi1^a xi2^b xi3^c
     V = np.asarray(verts8, dtype=LD)
     mono = np.zeros((2, 2, 2, 3), dtype=LD)
@@ -168,9 +169,9 @@ def _brute_force_cell(p, verts8, sigma):
                 for c in range(2):
                     mono[a, b, c] += V[v] * (s[0] ** a) * (s[1] ** b) * (s[2] ** c) / LD(8)
     A = np.zeros((n ** 3, n ** 3), dtype=LD)
-    for q3 in range(n):
-        for q2 in range(n):
-            for q1 in range(n):
+    for q3 in range(nq):
+        for q2 in range(nq):
+            for q1 in range(nq):
                 x = (xq[q1], xq[q2], xq[q3])
                 Jm = np.zeros((3, 3), dtype=LD)
                 for a in range(2):
