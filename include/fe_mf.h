@@ -135,7 +135,8 @@ int fe_fill_uniform(double *out_dev, long long count, unsigned long long seed, l
  *   H = K + M^kappa with kappa(x) given at the quadrature points, and H~ = M^-1/2 H M^-1/2 with M the mass matrix
  *   evaluated by the (p+1)-point Gauss-Lobatto-Legendre rule on the nodes, hence diagonal.
  *
- * fe_mf_set_kappa: kappa_host is a HOST array [ncells][n^3] (cells x fastest, point Q = q1 + n q2 + n^2 q3 at the
+ * fe_mf_set_kappa: kappa_host is a HOST array [ncells][n^3] (n = points per direction of the current rule, p + 1 unless
+ *   fe_mf_set_quadrature changed it; cells x fastest, point Q = q1 + n q2 + n^2 q3 at the
  *   Gauss points of the cell: kappa_Q = kappa(x_Q)), copied; it replaces sigma in every later call
  *   (G_QQ = kappa_Q det J w_Q).  NULL restores the constant sigma.  The context must be a uniform box
  *   (FE_GEOM_AFFINE without vertices) or have been created with FE_GEOM_QPOINT, else EINVAL (one metric per cell of a
@@ -151,6 +152,18 @@ int fe_fill_uniform(double *out_dev, long long count, unsigned long long seed, l
  * All three synchronise the device (they are setup calls, not stream-ordered) and return FE_MF_* codes.
  */
 int fe_mf_set_kappa(fe_mf_ctx *ctx, const double *kappa_host);
+
+/*
+ * fe_mf_set_quadrature: nq Gauss points per direction instead of n_p = p + 1 (the paper also
+ * benchmarks n_q = n_p + 2); p + 1 <= nq <= 12, else EINVAL; nq = p + 1 restores the default.
+ * Everything else keeps its meaning (N becomes n_q x n_p, the gradients are taken by collocation on the n_q points,
+ * D = D~ N of PAPER.md:188, per-point geometry and kappa live on the n_q^3 points).  On affine cells with constant
+ * kappa the result does not change (the n_p-point rule is already exact there).  A kappa array set before belongs
+ * to the points of the old rule and is dropped (constant sigma again): call fe_mf_set_kappa afterwards with
+ * [ncells][nq^3] values.  With nq != p + 1 every call runs on one plain kernel (rectangular tables, gather /
+ * atomic scatter): functional, not tuned.  Synchronises the device.
+ */
+int fe_mf_set_quadrature(fe_mf_ctx *ctx, int nq);
 int fe_mf_set_mass_scaling(fe_mf_ctx *ctx, int on);
 int fe_mf_mass_diagonal(fe_mf_ctx *ctx, double *out_host);
 

@@ -39,6 +39,7 @@ SYMBOLS = {
     "fe_mf_last_launch_count": (C.c_int, [C.c_void_p]),
     "fe_mf_set_variant": (C.c_int, [C.c_void_p, C.c_int]),
     "fe_mf_set_kappa": (C.c_int, [C.c_void_p, _PD]),
+    "fe_mf_set_quadrature": (C.c_int, [C.c_void_p, C.c_int]),
     "fe_mf_set_mass_scaling": (C.c_int, [C.c_void_p, C.c_int]),
     "fe_mf_mass_diagonal": (C.c_int, [C.c_void_p, _PD]),
     "fe_mf_last_error": (C.c_char_p, [C.c_void_p]),
@@ -110,6 +111,7 @@ class FeMf:
         self.ndofs = int(self._l.fe_mf_ndofs(self._ctx))
         self.p, self.device = int(p), int(device)
         self.ncells = tuple(int(c) for c in ncells)
+        self.nq = int(p) + 1
 
     @classmethod
     def from_workload(cls, w, device: int = 0) -> "FeMf":
@@ -167,10 +169,15 @@ class FeMf:
             self._raise(self._l.fe_mf_set_kappa(self._ctx, None))
             return
         k = np.ascontiguousarray(kappa, dtype=np.float64)
-        n3 = (self.p + 1) ** 3
+        n3 = self.nq ** 3
         if k.size != self.ncells[0] * self.ncells[1] * self.ncells[2] * n3:
             raise ValueError("kappa must have ncells * (p+1)^3 entries")
         self._raise(self._l.fe_mf_set_kappa(self._ctx, k.ctypes.data_as(_PD)))
+
+    def set_quadrature(self, nq: int):
+        """nq Gauss points per direction (p + 1 = default); a kappa array set before is dropped."""
+        self._raise(self._l.fe_mf_set_quadrature(self._ctx, int(nq)))
+        self.nq = int(nq)
 
     def set_mass_scaling(self, on: bool):
         self._raise(self._l.fe_mf_set_mass_scaling(self._ctx, 1 if on else 0))

@@ -37,6 +37,27 @@ cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStr
   return cudaGetLastError();
 }
 
+// ---- kind 11: n_q != n_p points per direction (over-integration): plain kernel with rectangular tables
+int oi_bv(int nq, int nvec) {
+  int bv = 16;
+  while (bv > 1 && ((size_t)4 * nq * nq * nq * bv * 8 > kMaxSmem / 2 - 4096 || bv > nvec)) bv >>= 1;
+  return bv;
+}
+template <int PDEG>
+cudaError_t launch_general_oi(const fe_mf_ctx* c, const fe::ApplyParams& prm, cudaStream_t st) {
+  const int nq = c->nq_oi;
+  fe::OiParams O{nq, c->oi_N, c->oi_D, c->oi_w, c->oi_geom, c->oi_geom_stride};
+  const size_t smem = ((size_t)4 * nq * nq * nq * prm.bv + (size_t)nq * (PDEG + 1) + (size_t)nq * nq) * sizeof(double);
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(fe::fe_apply_general_oi<PDEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  fe::fe_apply_general_oi<PDEG><<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
+  return cudaGetLastError();
+}
+
 // ---- kind 2: even-odd Cartesian kernel, one vector per thread, 8 vectors per block
 template <int PDEG>
 struct CartCfg {
@@ -303,6 +324,7 @@ cudaError_t launch_kron(const fe_mf_ctx* c, const fe::ApplyParams& prm, const CU
 
 // ---- which kernel serves (ctx, nvec, pointers)
 int pick_kernel(const fe_mf_ctx* c, int nvec, const void* W, const void* Z) {
+  if (c->nq_oi) return 11;   // n_q != n_p: only the plain kernel with rectangular tables
   if (c->variant == 1) return 1;
   // NEXT-1 operator: a uniform box with mass scaling runs on the Cartesian TMA kernels instantiated with EIG (kappa per
   // point, M^-1/2 inside the interpolation tables); kappa without mass scaling on such a context only on the general
@@ -341,6 +363,7 @@ int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
     case 6: return c->p == 8 ? 4 : kGenBv;
     case 8: return 16;
     case 10: return kron_bv(c->p);
+    case 11: return oi_bv(c->nq_oi, nvec);
     default: return line_bv(c, nvec);
   }
 }
@@ -410,7 +433,11 @@ int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, in
     for (int k = 0; k < 7; ++k) P.ug[k] /= c->detj0;
     P.dscale = nullptr;
   }
-  if (kind == 6 && P.dscale) {
+  if (kind == 11) {
+#define FE_CALL(p_) launch_general_oi<p_>(c, P, st)
+    FE_DISPATCH_P(FE_CALL)
+#undef FE_CALL
+  } else if (kind == 6 && P.dscale) {
 #define FE_CALL(p_) launch_gen<p_, true>(c, P, tw, tz, st)
     FE_DISPATCH_P(FE_CALL)
 #undef FE_CALL
@@ -696,6 +723,7 @@ extern "C" const char* fe_mf_kernel_name(const fe_mf_ctx* ctx, int nvec) {
     case 6: return "fe_apply_gen_tma";
     case 8: return "fe_apply_cart_plane";
     case 10: return "fe_apply_cart_kron";
+    case 11: return "fe_apply_general_oi";
     default: return "fe_apply_cart_line";
   }
 }

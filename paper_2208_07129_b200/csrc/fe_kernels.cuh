@@ -174,6 +174,132 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
   }
 }
 
+// ---- n_q != n_p Gauss points per direction (over-integration) ----------------
+// Plain sum factorisation with RECTANGULAR 1D tables (N: n_q x n_p) and the collocation derivative on the n_q points
+// (D = D~ N), n_q a run-time value: the general fallback of this operator variant, any geometry, any nvec.
+struct OiParams {
+  int nq;                     // Gauss points per direction
+  const double* Nq;           // [nq][n]   N[q][i] = l_i(xq_q)
+  const double* Dq;           // [nq][nq]  D~[q][r] = l~_r'(xq_q)
+  const double* wq;           // [nq]
+  const double* geom;         // geom_mode 2: [cell][7][nq^3] (no w factor), else unused
+  long long geom_stride;
+};
+
+// dst (+)= M src along direction `dir` of a (d0, d1, d2) x bv array; M is mo x mi (or its transpose, stored mi x mo)
+__device__ __forceinline__ void contract_rt(const double* M, int ldm, bool trans, int mo, int mi, int dir, const double* src,
+                                            double* dst, int d0, int d1, int d2, int bv, bool add, int tid, int nth) {
+  const int e0 = dir == 0 ? mo : d0, e1 = dir == 1 ? mo : d1, e2 = dir == 2 ? mo : d2;
+  const int total = e0 * e1 * e2 * bv;
+  const int sstride = (dir == 0 ? 1 : (dir == 1 ? d0 : d0 * d1)) * bv;
+  for (int t = tid; t < total; t += nth) {
+    const int beta = t % bv, r = t / bv;
+    const int o0 = r % e0, o1 = (r / e0) % e1, o2 = r / (e0 * e1);
+    const int o = dir == 0 ? o0 : (dir == 1 ? o1 : o2);
+    const int s0 = dir == 0 ? 0 : o0, s1 = dir == 1 ? 0 : o1, s2 = dir == 2 ? 0 : o2;
+    const double* sp = src + (size_t)(s0 + d0 * (s1 + d1 * s2)) * bv + beta;
+    double acc = add ? dst[t] : 0.0;
+    for (int i = 0; i < mi; ++i) acc = fma(trans ? M[i * ldm + o] : M[o * ldm + i], sp[(size_t)i * sstride], acc);
+    dst[t] = acc;
+  }
+}
+
+template <int PDEG>
+__global__ void __launch_bounds__(256) fe_apply_general_oi(const ApplyParams P, const OiParams O) {
+  constexpr int N = PDEG + 1;
+  const int nq = O.nq, nq3 = nq * nq * nq;
+  extern __shared__ double smem[];
+  const int bv = P.bv;
+  double* B0 = smem;
+  double* B1 = B0 + (size_t)nq3 * bv;
+  double* B2 = B1 + (size_t)nq3 * bv;
+  double* T = B2 + (size_t)nq3 * bv;
+  double* sN = T + (size_t)nq3 * bv;      // [nq][N]
+  double* sD = sN + nq * N;               // [nq][nq]
+  const int tid = threadIdx.x, nth = blockDim.x;
+  const int vb = blockIdx.x % P.nvb;
+  const int cell = blockIdx.x / P.nvb;
+  const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
+  const int v0 = vb * bv;
+  for (int t = tid; t < nq * N; t += nth) sN[t] = O.Nq[t];
+  for (int t = tid; t < nq * nq; t += nth) sD[t] = O.Dq[t];
+  // S2 gather into B0 as (N, N, N)
+  for (int t = tid; t < N * N * N * bv; t += nth) {
+    const int beta = t % bv, I = t / bv;
+    const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+    int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+    bool live = (v0 + beta) < P.nvec;
+    if (P.dirichlet) {
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+    } else {
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+    }
+    double xv = live ? P.W[global_node(P, ix, iy, iz) * P.nvec + v0 + beta] : 0.0;
+    if (P.dscale && live) xv *= __ldg(P.dscale + global_node(P, ix, iy, iz));
+    B0[t] = xv;
+  }
+  __syncthreads();
+  // S3 interpolate to the n_q^3 points (Alg. 1 with rectangular N)
+  contract_rt(sN, N, false, nq, N, 0, B0, B1, N, N, N, bv, false, tid, nth); __syncthreads();
+  contract_rt(sN, N, false, nq, N, 1, B1, B0, nq, N, N, bv, false, tid, nth); __syncthreads();
+  contract_rt(sN, N, false, nq, N, 2, B0, T, nq, nq, N, bv, false, tid, nth); __syncthreads();
+  // S4 reference gradients by collocation on the quadrature points
+  contract_rt(sD, nq, false, nq, nq, 0, T, B0, nq, nq, nq, bv, false, tid, nth);
+  contract_rt(sD, nq, false, nq, nq, 1, T, B1, nq, nq, nq, bv, false, tid, nth);
+  contract_rt(sD, nq, false, nq, nq, 2, T, B2, nq, nq, nq, bv, false, tid, nth);
+  __syncthreads();
+  // S5 quadrature-point scaling (Alg. 2 l.5-6; Eq. 22-23)
+  for (int t = tid; t < nq3 * bv; t += nth) {
+    const int Q = t / bv;
+    const int q1 = Q % nq, q2 = (Q / nq) % nq, q3 = Q / (nq * nq);
+    const double wq = __ldg(O.wq + q1) * __ldg(O.wq + q2) * __ldg(O.wq + q3);
+    double g[7];
+    if (P.geom_mode == 2) {
+      const double* gp = O.geom + (size_t)cell * O.geom_stride + Q;
+#pragma unroll
+      for (int k = 0; k < 7; ++k) g[k] = __ldg(gp + (size_t)k * nq3) * wq;
+    } else {
+#pragma unroll
+      for (int k = 0; k < 7; ++k) g[k] = (P.geom_mode == 1 ? __ldg(P.geom + (size_t)cell * 7 + k) : P.ug[k]) * wq;
+      if (P.kappa) g[6] *= __ldg(P.kappa + (size_t)cell * nq3 + Q);
+    }
+    const double a = B0[t], b = B1[t], c = B2[t];
+    B0[t] = g[0] * a + g[1] * b + g[2] * c;
+    B1[t] = g[1] * a + g[3] * b + g[4] * c;
+    B2[t] = g[2] * a + g[4] * b + g[5] * c;
+    T[t] = g[6] * T[t];
+  }
+  __syncthreads();
+  // S6 transposed gradients, accumulated on the mass term
+  contract_rt(sD, nq, true, nq, nq, 0, B0, T, nq, nq, nq, bv, true, tid, nth); __syncthreads();
+  contract_rt(sD, nq, true, nq, nq, 1, B1, T, nq, nq, nq, bv, true, tid, nth); __syncthreads();
+  contract_rt(sD, nq, true, nq, nq, 2, B2, T, nq, nq, nq, bv, true, tid, nth); __syncthreads();
+  // S7 integrate back to the nodes (N^T, rectangular)
+  contract_rt(sN, N, true, N, nq, 2, T, B0, nq, nq, nq, bv, false, tid, nth); __syncthreads();
+  contract_rt(sN, N, true, N, nq, 1, B0, B1, nq, nq, N, bv, false, tid, nth); __syncthreads();
+  contract_rt(sN, N, true, N, nq, 0, B1, B0, nq, N, N, bv, false, tid, nth); __syncthreads();
+  // S8 scatter-add
+  for (int t = tid; t < N * N * N * bv; t += nth) {
+    const int beta = t % bv, I = t / bv;
+    const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+    int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+    bool live = (v0 + beta) < P.nvec;
+    if (P.dirichlet) {
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+    } else {
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+    }
+    if (live) {
+      const double dv = P.dscale ? __ldg(P.dscale + global_node(P, ix, iy, iz)) : 1.0;
+      atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], P.alpha * (dv * B0[t]));
+    }
+  }
+}
+
 // S1 / S9 pre-pass: Z <- beta*Z + gamma*W  (Eq. B.1's bX + cY part)
 __global__ void fe_axpby_kernel(double* __restrict__ Z, const double* __restrict__ W, double beta, double gamma,
                                 size_t count) {

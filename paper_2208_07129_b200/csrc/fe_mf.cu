@@ -46,6 +46,11 @@ struct fe_mf_ctx {
   double* kappa_dev = nullptr;    // geom_mode 0: kappa at the quadrature points [cell][n^3] (set_kappa, or sigma everywhere
                                   // once mass scaling is on: the EIG kernels always read it)
   bool kappa_user = false;
+  // n_q != n_p points per direction (0 = off): tables and per-point geometry of that rule
+  int nq_oi = 0;
+  double *oi_N = nullptr, *oi_D = nullptr, *oi_w = nullptr, *oi_geom = nullptr;
+  long long oi_geom_stride = 0;
+  std::vector<double> oi_detq;   // geom_mode 2: det J at the n_q^3 points [cell][nq^3]
   double detj0 = 1.0;             // geom_mode 0: det J of every cell
   int variant = 0;
   int last_launches = 0;
@@ -316,6 +321,7 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
   if (ctx->ctrl) cudaFree(ctx->ctrl);
   if (ctx->dscale_dev) cudaFree(ctx->dscale_dev);
   if (ctx->kappa_dev) cudaFree(ctx->kappa_dev);
+  { double* b[] = {ctx->oi_N, ctx->oi_D, ctx->oi_w, ctx->oi_geom}; for (double* q : b) if (q) cudaFree(q); }
   if (ctx->ws_x) cudaFree(ctx->ws_x);
   if (ctx->ws_y) cudaFree(ctx->ws_y);
   for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
@@ -330,12 +336,14 @@ extern "C" int fe_mf_set_kappa(fe_mf_ctx* ctx, const double* kappa_host) {
     return fail(ctx, FE_MF_EINVAL, "fe_mf_set_kappa needs a uniform box or a context created with FE_GEOM_QPOINT");
   DeviceGuard guard(ctx->device);
   if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
-  const size_t nn = (size_t)ctx->n * ctx->n * ctx->n, total = nn * (size_t)ctx->ncells;
+  const int nqe = ctx->nq_oi ? ctx->nq_oi : ctx->n;   // points per direction of the current rule
+  const size_t nn = (size_t)nqe * nqe * nqe, total = nn * (size_t)ctx->ncells;
   if (ctx->geom_mode == 0) {   // uniform box: the raw kappa array, read by the EIG kernels and the general kernel
     FE_CUDA(ctx, cudaDeviceSynchronize());
     ctx->kappa_user = kappa_host != nullptr;
     if (!kappa_host && !ctx->mass_scaled) {
       if (ctx->kappa_dev) cudaFree(ctx->kappa_dev);
+  { double* b[] = {ctx->oi_N, ctx->oi_D, ctx->oi_w, ctx->oi_geom}; for (double* q : b) if (q) cudaFree(q); }
       ctx->kappa_dev = nullptr;
       return FE_MF_OK;
     }
@@ -355,10 +363,96 @@ extern "C" int fe_mf_set_kappa(fe_mf_ctx* ctx, const double* kappa_host) {
   std::vector<double> g;
   try { g.resize(total); } catch (...) { return fail(ctx, FE_MF_ENOMEM, "out of host memory (kappa)"); }
   // G_QQ = kappa_Q det J; the weight w_Q lives in the sqrt(w)-scaled 1D tables
-  for (size_t i = 0; i < total; ++i) g[i] = (kappa_host ? kappa_host[i] : ctx->sigma) * ctx->detq[i];
+  const std::vector<double>& det = ctx->nq_oi ? ctx->oi_detq : ctx->detq;
+  for (size_t i = 0; i < total; ++i) g[i] = (kappa_host ? kappa_host[i] : ctx->sigma) * det[i];
   FE_CUDA(ctx, cudaDeviceSynchronize());
-  FE_CUDA(ctx, cudaMemcpy2D(ctx->geom_dev + 6 * nn, (size_t)ctx->geom_stride * sizeof(double), g.data(), nn * sizeof(double),
+  double* gdst = ctx->nq_oi ? ctx->oi_geom : ctx->geom_dev;
+  const size_t gstride = (size_t)(ctx->nq_oi ? ctx->oi_geom_stride : ctx->geom_stride);
+  FE_CUDA(ctx, cudaMemcpy2D(gdst + 6 * nn, gstride * sizeof(double), g.data(), nn * sizeof(double),
                             nn * sizeof(double), (size_t)ctx->ncells, cudaMemcpyHostToDevice));
+  return FE_MF_OK;
+}
+
+// ---- n_q != n_p Gauss points per direction ------------------------------------------------------
+
+extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (nq < ctx->n || nq > 12) return fail(ctx, FE_MF_EINVAL, "need p + 1 <= nq <= 12");
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
+  FE_CUDA(ctx, cudaDeviceSynchronize());
+  { double** b[] = {&ctx->oi_N, &ctx->oi_D, &ctx->oi_w, &ctx->oi_geom}; for (double** q : b) if (*q) { cudaFree(*q); *q = nullptr; } }
+  ctx->oi_detq.clear();
+  const bool had_kappa = ctx->kappa_user;
+  ctx->nq_oi = (nq == ctx->n) ? 0 : nq;
+  // a kappa array belongs to the points of one rule: back to the constant sigma
+  if (ctx->geom_mode == 0) {
+    ctx->kappa_user = false;
+    if (ctx->kappa_dev) { cudaFree(ctx->kappa_dev); ctx->kappa_dev = nullptr; }
+    if (ctx->mass_scaled && !ctx->nq_oi) { const int rc = fe_mf_set_kappa(ctx, nullptr); if (rc != FE_MF_OK) return rc; }
+  } else if (ctx->geom_mode == 2 && !ctx->nq_oi && had_kappa) {
+    const int rc = fe_mf_set_kappa(ctx, nullptr);
+    if (rc != FE_MF_OK) return rc;
+  }
+  if (!ctx->nq_oi) return FE_MF_OK;
+  const int n = ctx->n;
+  // tables of the nq-point rule in long double: N[q][i] = l_i(xq_q) on the GLL nodes, D~ on the quadrature points
+  long double xi[16], xq[16], w[16], c[16];
+  fe::gll_nodes(ctx->p, xi);
+  fe::gauss_legendre(nq, xq, w);
+  std::vector<double> hN((size_t)nq * n), hD((size_t)nq * nq), hw(nq);
+  for (int q = 0; q < nq; ++q) {
+    hw[q] = (double)w[q];
+    for (int i = 0; i < n; ++i) {
+      long double v = 1.0L;
+      for (int j = 0; j < n; ++j) if (j != i) v *= (xq[q] - xi[j]) / (xi[i] - xi[j]);
+      hN[(size_t)q * n + i] = (double)v;
+    }
+  }
+  for (int r = 0; r < nq; ++r) { c[r] = 1.0L; for (int j = 0; j < nq; ++j) if (j != r) c[r] *= (xq[r] - xq[j]); }
+  for (int q = 0; q < nq; ++q)
+    for (int r = 0; r < nq; ++r) {
+      long double v = 0.0L;
+      if (q != r) v = (c[q] / c[r]) / (xq[q] - xq[r]);
+      else for (int j = 0; j < nq; ++j) if (j != q) v += 1.0L / (xq[q] - xq[j]);
+      hD[(size_t)q * nq + r] = (double)v;
+    }
+  auto upload = [&](double** dst, const std::vector<double>& src) {
+    if (cudaMalloc(dst, src.size() * sizeof(double)) != cudaSuccess) { *dst = nullptr; return false; }
+    return cudaMemcpy(*dst, src.data(), src.size() * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess;
+  };
+  if (!upload(&ctx->oi_N, hN) || !upload(&ctx->oi_D, hD) || !upload(&ctx->oi_w, hw)) {
+    ctx->nq_oi = 0;
+    return fail(ctx, FE_MF_ENOMEM, "table upload failed (quadrature)");
+  }
+  if (ctx->geom_mode == 2) {   // per-point metric at the nq^3 points (Eq. 7c evaluated at every point of the rule)
+    const size_t nn = (size_t)nq * nq * nq;
+    ctx->oi_geom_stride = (long long)(7 * nn);
+    std::vector<double> G;
+    try { G.resize(7 * nn * (size_t)ctx->ncells); ctx->oi_detq.resize(nn * (size_t)ctx->ncells); }
+    catch (...) { ctx->nq_oi = 0; return fail(ctx, FE_MF_ENOMEM, "out of host memory (geometry)"); }
+    const double* verts = ctx->verts.empty() ? nullptr : ctx->verts.data();
+    for (int ez = 0; ez < ctx->ncz; ++ez)
+      for (int ey = 0; ey < ctx->ncy; ++ey)
+        for (int ex = 0; ex < ctx->ncx; ++ex) {
+          double v[8][3], J[3][3], m[7];
+          cell_vertices(ctx, verts, ctx->lo, ctx->h, ex, ey, ez, v);
+          const size_t cell = (size_t)ex + (size_t)ctx->ncx * ((size_t)ey + (size_t)ctx->ncy * ez);
+          double* g = G.data() + cell * 7 * nn;
+          for (int q3 = 0; q3 < nq; ++q3)
+            for (int q2 = 0; q2 < nq; ++q2)
+              for (int q1 = 0; q1 < nq; ++q1) {
+                const double x3[3] = {(double)xq[q1], (double)xq[q2], (double)xq[q3]};
+                fe::trilinear_jacobian(v, x3, J);
+                if (!fe::metric_from_jacobian(J, m)) { ctx->nq_oi = 0; return fail(ctx, FE_MF_EINVAL, "non-positive det J at a quadrature point"); }
+                const size_t Q = (size_t)q1 + (size_t)nq * (q2 + (size_t)nq * q3);
+                for (int k = 0; k < 6; ++k) g[(size_t)k * nn + Q] = m[k];
+                g[6 * nn + Q] = ctx->sigma * m[6];
+                ctx->oi_detq[cell * nn + Q] = m[6];
+              }
+        }
+    if (!upload(&ctx->oi_geom, G)) { ctx->nq_oi = 0; return fail(ctx, FE_MF_ENOMEM, "geometry upload failed (quadrature)"); }
+  }
   return FE_MF_OK;
 }
 
@@ -422,7 +516,7 @@ extern "C" int fe_mf_set_mass_scaling(fe_mf_ctx* ctx, int on) {
   ctx->mass_scaled = on != 0;
   if (ctx->geom_mode == 0) {
     // the EIG kernels read kappa per point: constant sigma becomes an array while the scaling is on
-    if (on && !ctx->kappa_dev) return fe_mf_set_kappa(ctx, nullptr);
+    if (on && !ctx->kappa_dev && !ctx->nq_oi) return fe_mf_set_kappa(ctx, nullptr);
     if (!on && ctx->kappa_dev && !ctx->kappa_user) { cudaFree(ctx->kappa_dev); ctx->kappa_dev = nullptr; }
   }
   return FE_MF_OK;
