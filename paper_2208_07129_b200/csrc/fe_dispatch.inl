@@ -54,6 +54,16 @@ cudaError_t launch_general_oi(const fe_mf_ctx* c, const fe::ApplyParams& prm, cu
     if (e != cudaSuccess) return e;
     configured = smem;
   }
+  if (nq == PDEG + 3) {   // the paper's n_q = n_p + 2: compile-time sizes, line tasks
+    static size_t configured2 = 0;
+    if (smem > configured2) {
+      cudaError_t e = cudaFuncSetAttribute(fe::fe_apply_oi<PDEG, PDEG + 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e != cudaSuccess) return e;
+      configured2 = smem;
+    }
+    fe::fe_apply_oi<PDEG, PDEG + 3><<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
+    return cudaGetLastError();
+  }
   fe::fe_apply_general_oi<PDEG><<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
   return cudaGetLastError();
 }
@@ -723,7 +733,7 @@ extern "C" const char* fe_mf_kernel_name(const fe_mf_ctx* ctx, int nvec) {
     case 6: return "fe_apply_gen_tma";
     case 8: return "fe_apply_cart_plane";
     case 10: return "fe_apply_cart_kron";
-    case 11: return "fe_apply_general_oi";
+    case 11: return ctx->nq_oi == ctx->p + 3 ? "fe_apply_oi" : "fe_apply_general_oi";
     default: return "fe_apply_cart_line";
   }
 }

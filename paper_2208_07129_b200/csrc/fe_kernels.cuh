@@ -300,6 +300,133 @@ __global__ void __launch_bounds__(256) fe_apply_general_oi(const ApplyParams P, 
   }
 }
 
+// Tables of the n_q = n_p + 2 rule, packed per degree: [N (nq x n) | D~ (nq x nq)] at oi_offset(p); constant-bank FMA
+// operands like the other tables (uploaded by fe_mf_set_quadrature; the values depend on p only)
+template <int P_> struct OiOffset { static constexpr int value = OiOffset<P_ - 1>::value + (P_ + 2) * P_ + (P_ + 2) * (P_ + 2); };
+template <> struct OiOffset<1> { static constexpr int value = 0; };
+__constant__ double c_oi[OiOffset<9>::value];
+inline int oi_offset(int p) {
+  int off = 0;
+  for (int k = 2; k <= p; ++k) off += (k + 2) * k + (k + 2) * (k + 2);
+  return off;
+}
+
+// The same with compile-time sizes (the paper's n_q = n_p + 2) and LINE tasks: one thread contracts one line of one
+// vector in registers (one tile read and one tile write per point and pass instead of n reads per output).
+// Array (D0, D1, D2) x bv -> the extent along DIR becomes MO; M = c_oi + MOFF is [MO][MI] (TRANS: stored [MI][MO]).
+template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ADD, int MOFF>
+__device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int bv, int tid,
+                                               int nth) {
+  const double* M = c_oi + MOFF;
+  constexpr int MI = DIR == 0 ? D0 : (DIR == 1 ? D1 : D2);
+  constexpr int EA = DIR == 0 ? D1 : D0, EB = DIR == 2 ? D1 : D2;          // the two other extents, in index order
+  constexpr int SS = DIR == 0 ? 1 : (DIR == 1 ? D0 : D0 * D1);              // source stride along DIR (in points)
+  constexpr int E0 = DIR == 0 ? MO : D0, E1 = DIR == 1 ? MO : D1;            // destination extents
+  constexpr int DS = DIR == 0 ? 1 : (DIR == 1 ? E0 : E0 * E1);
+  const int nlines = EA * EB * bv;
+  for (int t = tid; t < nlines; t += nth) {
+    const int beta = t % bv, r = t / bv, a = r % EA, b = r / EA;
+    // point index of the line start in source / destination
+    const int sbase = DIR == 0 ? D0 * (a + D1 * b) : (DIR == 1 ? a + D0 * D1 * b : a + D0 * b);
+    const int dbase = DIR == 0 ? E0 * (a + E1 * b) : (DIR == 1 ? a + E0 * E1 * b : a + E0 * b);
+    double x[MI];
+#pragma unroll
+    for (int i = 0; i < MI; ++i) x[i] = src[(size_t)(sbase + i * SS) * bv + beta];
+#pragma unroll
+    for (int o = 0; o < MO; ++o) {
+      double acc = ADD ? dst[(size_t)(dbase + o * DS) * bv + beta] : 0.0;
+#pragma unroll
+      for (int i = 0; i < MI; ++i) acc = fma(TRANS ? M[i * MO + o] : M[o * MI + i], x[i], acc);
+      dst[(size_t)(dbase + o * DS) * bv + beta] = acc;
+    }
+  }
+}
+
+template <int PDEG, int NQ>
+__global__ void __launch_bounds__(256) fe_apply_oi(const ApplyParams P, const OiParams O) {
+  constexpr int N = PDEG + 1, NQ3 = NQ * NQ * NQ;
+  extern __shared__ double smem[];
+  const int bv = P.bv;
+  double* B0 = smem;
+  double* B1 = B0 + (size_t)NQ3 * bv;
+  double* B2 = B1 + (size_t)NQ3 * bv;
+  double* T = B2 + (size_t)NQ3 * bv;
+  constexpr int ON = OiOffset<PDEG>::value, OD = OiOffset<PDEG>::value + NQ * N;   // N [NQ][N] and D~ [NQ][NQ] in c_oi
+  const int tid = threadIdx.x, nth = blockDim.x;
+  const int vb = blockIdx.x % P.nvb;
+  const int cell = blockIdx.x / P.nvb;
+  const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
+  const int v0 = vb * bv;
+  for (int t = tid; t < N * N * N * bv; t += nth) {
+    const int beta = t % bv, I = t / bv;
+    const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+    int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+    bool live = (v0 + beta) < P.nvec;
+    if (P.dirichlet) {
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+    } else {
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+    }
+    double xv = live ? P.W[global_node(P, ix, iy, iz) * P.nvec + v0 + beta] : 0.0;
+    if (P.dscale && live) xv *= __ldg(P.dscale + global_node(P, ix, iy, iz));
+    B0[t] = xv;
+  }
+  __syncthreads();
+  contract_lines<N, N, N, 0, NQ, false, false, ON>(B0, B1, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, N, N, 1, NQ, false, false, ON>(B1, B0, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, N, 2, NQ, false, false, ON>(B0, T, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, false, false, OD>(T, B0, bv, tid, nth);
+  contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD>(T, B1, bv, tid, nth);
+  contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD>(T, B2, bv, tid, nth);
+  __syncthreads();
+  for (int t = tid; t < NQ3 * bv; t += nth) {
+    const int Q = t / bv;
+    const int q1 = Q % NQ, q2 = (Q / NQ) % NQ, q3 = Q / (NQ * NQ);
+    const double wq = __ldg(O.wq + q1) * __ldg(O.wq + q2) * __ldg(O.wq + q3);
+    double g[7];
+    if (P.geom_mode == 2) {
+      const double* gp = O.geom + (size_t)cell * O.geom_stride + Q;
+#pragma unroll
+      for (int k = 0; k < 7; ++k) g[k] = __ldg(gp + (size_t)k * NQ3) * wq;
+    } else {
+#pragma unroll
+      for (int k = 0; k < 7; ++k) g[k] = (P.geom_mode == 1 ? __ldg(P.geom + (size_t)cell * 7 + k) : P.ug[k]) * wq;
+      if (P.kappa) g[6] *= __ldg(P.kappa + (size_t)cell * NQ3 + Q);
+    }
+    const double a = B0[t], b = B1[t], c = B2[t];
+    B0[t] = g[0] * a + g[1] * b + g[2] * c;
+    B1[t] = g[1] * a + g[3] * b + g[4] * c;
+    B2[t] = g[2] * a + g[4] * b + g[5] * c;
+    T[t] = g[6] * T[t];
+  }
+  __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD>(B0, T, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, OD>(B1, T, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, OD>(B2, T, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, N, true, false, ON>(T, B0, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, N, 1, N, true, false, ON>(B0, B1, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, N, N, 0, N, true, false, ON>(B1, B0, bv, tid, nth); __syncthreads();
+  for (int t = tid; t < N * N * N * bv; t += nth) {
+    const int beta = t % bv, I = t / bv;
+    const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+    int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+    bool live = (v0 + beta) < P.nvec;
+    if (P.dirichlet) {
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+    } else {
+      if (ix >= P.ndx) ix -= P.ndx;
+      if (iy >= P.ndy) iy -= P.ndy;
+      if (iz >= P.ndz) iz -= P.ndz;
+    }
+    if (live) {
+      const double dv = P.dscale ? __ldg(P.dscale + global_node(P, ix, iy, iz)) : 1.0;
+      atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], P.alpha * (dv * B0[t]));
+    }
+  }
+}
+
 // S1 / S9 pre-pass: Z <- beta*Z + gamma*W  (Eq. B.1's bX + cY part)
 __global__ void fe_axpby_kernel(double* __restrict__ Z, const double* __restrict__ W, double beta, double gamma,
                                 size_t count) {

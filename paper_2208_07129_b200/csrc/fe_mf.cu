@@ -425,6 +425,11 @@ extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
     ctx->nq_oi = 0;
     return fail(ctx, FE_MF_ENOMEM, "table upload failed (quadrature)");
   }
+  if (nq == ctx->p + 3) {   // the compile-time kernel of n_q = n_p + 2 reads its tables from constant memory
+    std::vector<double> pack(hN);
+    pack.insert(pack.end(), hD.begin(), hD.end());
+    FE_CUDA(ctx, cudaMemcpyToSymbol(fe::c_oi, pack.data(), pack.size() * sizeof(double), sizeof(double) * fe::oi_offset(ctx->p)));
+  }
   if (ctx->geom_mode == 2) {   // per-point metric at the nq^3 points (Eq. 7c evaluated at every point of the rule)
     const size_t nn = (size_t)nq * nq * nq;
     ctx->oi_geom_stride = (long long)(7 * nn);

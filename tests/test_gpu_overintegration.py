@@ -52,7 +52,7 @@ def test_apply_with_np_plus_2_points(env, p, bc, kind):
     op, mesh = make_pair(env, p, bc, kind)
     nq = p + 3
     op.set_quadrature(nq)
-    assert op.kernel_name(8) == "fe_apply_general_oi"
+    assert op.kernel_name(8) == "fe_apply_oi"
     oo = orc.Operator(mesh, 0.7, nq=nq)
     for nvec in (8, 3):
         X = inputs.multivector(51, mesh.ndof, nvec)
@@ -72,6 +72,7 @@ def test_sheared_cells_and_other_point_counts(env):
     base = orc.Operator(mesh, 0.7).apply(X)
     for nq in (5, 6, 9):
         op.set_quadrature(nq)
+        assert op.kernel_name(4) == ("fe_apply_oi" if nq == 6 else "fe_apply_general_oi")
         assert relerr(run(torch, op, X, 4), base) <= TOL       # affine cells: every rule with nq >= p + 1 is exact
     with pytest.raises(binding.FeMfError) as e:
         op.set_quadrature(3)
