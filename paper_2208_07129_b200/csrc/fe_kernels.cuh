@@ -343,7 +343,7 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ src, d
 }
 
 template <int PDEG, int NQ>
-__global__ void __launch_bounds__(256) fe_apply_oi(const ApplyParams P, const OiParams O) {
+__global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const OiParams O) {
   constexpr int N = PDEG + 1, NQ3 = NQ * NQ * NQ;
   extern __shared__ double smem[];
   const int bv = P.bv;
