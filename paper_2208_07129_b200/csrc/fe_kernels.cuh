@@ -381,8 +381,9 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
   contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD>(T, B1, bv, tid, nth);
   contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD>(T, B2, bv, tid, nth);
   __syncthreads();
-  for (int t = tid; t < NQ3 * bv; t += nth) {
-    const int Q = t / bv;
+  // one thread = one point for all the block's vectors (the 7 factors are loaded once), two points in flight
+#pragma unroll 2
+  for (int Q = tid; Q < NQ3; Q += nth) {
     const int q1 = Q % NQ, q2 = (Q / NQ) % NQ, q3 = Q / (NQ * NQ);
     const double wq = __ldg(O.wq + q1) * __ldg(O.wq + q2) * __ldg(O.wq + q3);
     double g[7];
@@ -395,11 +396,14 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
       for (int k = 0; k < 7; ++k) g[k] = (P.geom_mode == 1 ? __ldg(P.geom + (size_t)cell * 7 + k) : P.ug[k]) * wq;
       if (P.kappa) g[6] *= __ldg(P.kappa + (size_t)cell * NQ3 + Q);
     }
-    const double a = B0[t], b = B1[t], c = B2[t];
-    B0[t] = g[0] * a + g[1] * b + g[2] * c;
-    B1[t] = g[1] * a + g[3] * b + g[4] * c;
-    B2[t] = g[2] * a + g[4] * b + g[5] * c;
-    T[t] = g[6] * T[t];
+    for (int beta = 0; beta < bv; ++beta) {
+      const int t = Q * bv + beta;
+      const double a = B0[t], b = B1[t], c = B2[t];
+      B0[t] = g[0] * a + g[1] * b + g[2] * c;
+      B1[t] = g[1] * a + g[3] * b + g[4] * c;
+      B2[t] = g[2] * a + g[4] * b + g[5] * c;
+      T[t] = g[6] * T[t];
+    }
   }
   __syncthreads();
   contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD>(B0, T, bv, tid, nth); __syncthreads();
