@@ -180,3 +180,20 @@ def test_mass_scaled_chebyshev_filter(env, p, bc, kind):
     assert relerr(Yd.cpu().numpy(), Yo) <= 1e-11
     if kind == "uniform":
         assert op.last_launch_count() <= m + 1
+
+
+@pytest.mark.parametrize("kind", ["uniform", "perturbed_q"])
+def test_host_path_with_mass_scaled_operator(env, kind):
+    """fe_mf_apply_host (host buffers, column chunks on two streams) applies the operator the context is set to."""
+    torch, orc, binding = env
+    op, mesh = make_pair(env, 6, inputs.BC_PERIODIC, kind, ncells=(2, 2, 3))
+    kap = smooth_potential(orc, mesh)
+    op.set_kappa(kap)
+    op.set_mass_scaling(True)
+    oo = orc.Operator(mesh, 0.0, kappa=kap)
+    d = 1.0 / np.sqrt(orc.lumped_mass_diagonal(mesh))
+    nvec = 40                                       # three chunks, the last one partial
+    X = inputs.multivector(61, mesh.ndof, nvec)
+    Xh = torch.from_numpy(X).pin_memory(); Yh = torch.empty_like(Xh).pin_memory()
+    op.apply_host(Xh, Yh, nvec)
+    assert relerr(Yh.numpy(), oo.apply_mass_scaled(X, d)) <= TOL
