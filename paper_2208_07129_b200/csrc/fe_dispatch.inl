@@ -39,7 +39,7 @@ cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStr
 
 // ---- kind 11: n_q != n_p points per direction (over-integration): plain kernel with rectangular tables
 int oi_bv(int nq, int nvec) {
-  int bv = 16;
+  int bv = 4;   // the compile-time kernel is instantiated for 2 and 4 vectors per block
   while (bv > 1 && ((size_t)4 * nq * nq * nq * bv * 8 > kMaxSmem / 2 - 4096 || bv > nvec)) bv >>= 1;
   return bv;
 }
@@ -54,14 +54,16 @@ cudaError_t launch_general_oi(const fe_mf_ctx* c, const fe::ApplyParams& prm, cu
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  if (nq == PDEG + 3) {   // the paper's n_q = n_p + 2: compile-time sizes, line tasks
-    static size_t configured2 = 0;
-    if (smem > configured2) {
-      cudaError_t e = cudaFuncSetAttribute(fe::fe_apply_oi<PDEG, PDEG + 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (nq == PDEG + 3 && (prm.bv == 2 || prm.bv == 4)) {   // the paper's n_q = n_p + 2: compile-time sizes, line tasks
+    auto kern = prm.bv == 2 ? fe::fe_apply_oi<PDEG, PDEG + 3, 2> : fe::fe_apply_oi<PDEG, PDEG + 3, 4>;
+    static size_t configured2[2] = {0, 0};
+    size_t& conf = configured2[prm.bv == 4];
+    if (smem > conf) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       if (e != cudaSuccess) return e;
-      configured2 = smem;
+      conf = smem;
     }
-    fe::fe_apply_oi<PDEG, PDEG + 3><<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
+    kern<<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
     return cudaGetLastError();
   }
   fe::fe_apply_general_oi<PDEG><<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
@@ -733,7 +735,7 @@ extern "C" const char* fe_mf_kernel_name(const fe_mf_ctx* ctx, int nvec) {
     case 6: return "fe_apply_gen_tma";
     case 8: return "fe_apply_cart_plane";
     case 10: return "fe_apply_cart_kron";
-    case 11: return ctx->nq_oi == ctx->p + 3 ? "fe_apply_oi" : "fe_apply_general_oi";
+    case 11: return (ctx->nq_oi == ctx->p + 3 && oi_bv(ctx->nq_oi, nvec) >= 2) ? "fe_apply_oi" : "fe_apply_general_oi";
     default: return "fe_apply_cart_line";
   }
 }

@@ -314,9 +314,8 @@ inline int oi_offset(int p) {
 // The same with compile-time sizes (the paper's n_q = n_p + 2) and LINE tasks: one thread contracts one line of one
 // vector in registers (one tile read and one tile write per point and pass instead of n reads per output).
 // Array (D0, D1, D2) x bv -> the extent along DIR becomes MO; M = c_oi + MOFF is [MO][MI] (TRANS: stored [MI][MO]).
-template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ADD, int MOFF>
-__device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int bv, int tid,
-                                               int nth) {
+template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ADD, int MOFF, int bv>
+__device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int tid, int nth) {
   const double* M = c_oi + MOFF;
   constexpr int MI = DIR == 0 ? D0 : (DIR == 1 ? D1 : D2);
   constexpr int EA = DIR == 0 ? D1 : D0, EB = DIR == 2 ? D1 : D2;          // the two other extents, in index order
@@ -342,11 +341,10 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ src, d
   }
 }
 
-template <int PDEG, int NQ>
+template <int PDEG, int NQ, int bv>
 __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const OiParams O) {
   constexpr int N = PDEG + 1, NQ3 = NQ * NQ * NQ;
   extern __shared__ double smem[];
-  const int bv = P.bv;
   double* B0 = smem;
   double* B1 = B0 + (size_t)NQ3 * bv;
   double* B2 = B1 + (size_t)NQ3 * bv;
@@ -374,12 +372,12 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
     B0[t] = xv;
   }
   __syncthreads();
-  contract_lines<N, N, N, 0, NQ, false, false, ON>(B0, B1, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, N, N, 1, NQ, false, false, ON>(B1, B0, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, N, 2, NQ, false, false, ON>(B0, T, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, false, false, OD>(T, B0, bv, tid, nth);
-  contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD>(T, B1, bv, tid, nth);
-  contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD>(T, B2, bv, tid, nth);
+  contract_lines<N, N, N, 0, NQ, false, false, ON, bv>(B0, B1, tid, nth); __syncthreads();
+  contract_lines<NQ, N, N, 1, NQ, false, false, ON, bv>(B1, B0, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, N, 2, NQ, false, false, ON, bv>(B0, T, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, false, false, OD, bv>(T, B0, tid, nth);
+  contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD, bv>(T, B1, tid, nth);
+  contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD, bv>(T, B2, tid, nth);
   __syncthreads();
   // one thread = one point for all the block's vectors (the 7 factors are loaded once), two points in flight
 #pragma unroll 2
@@ -406,12 +404,12 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
     }
   }
   __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD>(B0, T, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, OD>(B1, T, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, OD>(B2, T, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, N, true, false, ON>(T, B0, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, N, 1, N, true, false, ON>(B0, B1, bv, tid, nth); __syncthreads();
-  contract_lines<NQ, N, N, 0, N, true, false, ON>(B1, B0, bv, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD, bv>(B0, T, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, OD, bv>(B1, T, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, OD, bv>(B2, T, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, N, true, false, ON, bv>(T, B0, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, N, 1, N, true, false, ON, bv>(B0, B1, tid, nth); __syncthreads();
+  contract_lines<NQ, N, N, 0, N, true, false, ON, bv>(B1, B0, tid, nth); __syncthreads();
   for (int t = tid; t < N * N * N * bv; t += nth) {
     const int beta = t % bv, I = t / bv;
     const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
