@@ -315,15 +315,19 @@ inline int oi_offset(int p) {
 // vector in registers (one tile read and one tile write per point and pass instead of n reads per output).
 // Array (D0, D1, D2) x bv -> the extent along DIR becomes MO; M = c_oi + MOFF is [MO][MI] (TRANS: stored [MI][MO]).
 template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ADD, int MOFF, int bv>
-__device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int tid, int nth) {
-  const double* M = c_oi + MOFF;
+__device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int tid) {
+  constexpr int nth = 256;   // the block size, as a constant: the trip count of the line loop is then known (1 or 2), and
+                             // the table values are not hoisted out of it into more uniform registers than exist
   constexpr int MI = DIR == 0 ? D0 : (DIR == 1 ? D1 : D2);
   constexpr int EA = DIR == 0 ? D1 : D0, EB = DIR == 2 ? D1 : D2;          // the two other extents, in index order
   constexpr int SS = DIR == 0 ? 1 : (DIR == 1 ? D0 : D0 * D1);              // source stride along DIR (in points)
   constexpr int E0 = DIR == 0 ? MO : D0, E1 = DIR == 1 ? MO : D1;            // destination extents
   constexpr int DS = DIR == 0 ? 1 : (DIR == 1 ? E0 : E0 * E1);
-  const int nlines = EA * EB * bv;
-  for (int t = tid; t < nlines; t += nth) {
+  constexpr int nlines = EA * EB * bv;
+#pragma unroll
+  for (int t0 = 0; t0 < nlines; t0 += nth) {
+    const int t = t0 + tid;
+    if (t >= nlines) break;
     const int beta = t % bv, r = t / bv, a = r % EA, b = r / EA;
     // point index of the line start in source / destination
     const int sbase = DIR == 0 ? D0 * (a + D1 * b) : (DIR == 1 ? a + D0 * D1 * b : a + D0 * b);
@@ -335,7 +339,7 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ src, d
     for (int o = 0; o < MO; ++o) {
       double acc = ADD ? dst[(size_t)(dbase + o * DS) * bv + beta] : 0.0;
 #pragma unroll
-      for (int i = 0; i < MI; ++i) acc = fma(TRANS ? M[i * MO + o] : M[o * MI + i], x[i], acc);
+      for (int i = 0; i < MI; ++i) acc = fma(TRANS ? c_oi[MOFF + i * MO + o] : c_oi[MOFF + o * MI + i], x[i], acc);
       dst[(size_t)(dbase + o * DS) * bv + beta] = acc;
     }
   }
@@ -372,12 +376,12 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
     B0[t] = xv;
   }
   __syncthreads();
-  contract_lines<N, N, N, 0, NQ, false, false, ON, bv>(B0, B1, tid, nth); __syncthreads();
-  contract_lines<NQ, N, N, 1, NQ, false, false, ON, bv>(B1, B0, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, N, 2, NQ, false, false, ON, bv>(B0, T, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, false, false, OD, bv>(T, B0, tid, nth);
-  contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD, bv>(T, B1, tid, nth);
-  contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD, bv>(T, B2, tid, nth);
+  contract_lines<N, N, N, 0, NQ, false, false, ON, bv>(B0, B1, tid); __syncthreads();
+  contract_lines<NQ, N, N, 1, NQ, false, false, ON, bv>(B1, B0, tid); __syncthreads();
+  contract_lines<NQ, NQ, N, 2, NQ, false, false, ON, bv>(B0, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, false, false, OD, bv>(T, B0, tid);
+  contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD, bv>(T, B1, tid);
+  contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD, bv>(T, B2, tid);
   __syncthreads();
   // one thread = one point for all the block's vectors (the 7 factors are loaded once), two points in flight
 #pragma unroll 2
@@ -404,12 +408,12 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
     }
   }
   __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD, bv>(B0, T, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, OD, bv>(B1, T, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, OD, bv>(B2, T, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, N, true, false, ON, bv>(T, B0, tid, nth); __syncthreads();
-  contract_lines<NQ, NQ, N, 1, N, true, false, ON, bv>(B0, B1, tid, nth); __syncthreads();
-  contract_lines<NQ, N, N, 0, N, true, false, ON, bv>(B1, B0, tid, nth); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD, bv>(B0, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, OD, bv>(B1, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, OD, bv>(B2, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, N, true, false, ON, bv>(T, B0, tid); __syncthreads();
+  contract_lines<NQ, NQ, N, 1, N, true, false, ON, bv>(B0, B1, tid); __syncthreads();
+  contract_lines<NQ, N, N, 0, N, true, false, ON, bv>(B1, B0, tid); __syncthreads();
   for (int t = tid; t < N * N * N * bv; t += nth) {
     const int beta = t % bv, I = t / bv;
     const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
