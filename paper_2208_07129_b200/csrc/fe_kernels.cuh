@@ -300,21 +300,26 @@ __global__ void __launch_bounds__(256) fe_apply_general_oi(const ApplyParams P, 
   }
 }
 
-// Tables of the n_q = n_p + 2 rule, packed per degree: [N (nq x n) | D~ (nq x nq)] at oi_offset(p); constant-bank FMA
-// operands like the other tables (uploaded by fe_mf_set_quadrature; the values depend on p only)
-template <int P_> struct OiOffset { static constexpr int value = OiOffset<P_ - 1>::value + (P_ + 2) * P_ + (P_ + 2) * (P_ + 2); };
+// Tables of the n_q = n_p + 2 rule, packed per degree at oi_offset(p) as even / odd halves (uploaded by
+// fe_mf_set_quadrature; the values depend on p only): [Ne | No | De | Do], N (nq x n) centro-symmetric, D~ (nq x nq)
+// centro-antisymmetric (SURVEY.md 8(c) reading 14), Me[o][i] = (M[o][i] + M[o][C-1-i]) / 2, Mo[o][i] = (M[o][i] - M[o][C-1-i]) / 2
+// for o < ceil(R/2), i < ceil(C/2).  Constant-bank FMA operands like the other tables.
+constexpr int oi_size(int p) { return 2 * ((p + 4) / 2) * ((p + 2) / 2) + 2 * ((p + 4) / 2) * ((p + 4) / 2); }
+template <int P_> struct OiOffset { static constexpr int value = OiOffset<P_ - 1>::value + oi_size(P_ - 1); };
 template <> struct OiOffset<1> { static constexpr int value = 0; };
 __constant__ double c_oi[OiOffset<9>::value];
 inline int oi_offset(int p) {
   int off = 0;
-  for (int k = 2; k <= p; ++k) off += (k + 2) * k + (k + 2) * (k + 2);
+  for (int k = 1; k < p; ++k) off += oi_size(k);
   return off;
 }
 
-// The same with compile-time sizes (the paper's n_q = n_p + 2) and LINE tasks: one thread contracts one line of one
-// vector in registers (one tile read and one tile write per point and pass instead of n reads per output).
-// Array (D0, D1, D2) x bv -> the extent along DIR becomes MO; M = c_oi + MOFF is [MO][MI] (TRANS: stored [MI][MO]).
-template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ADD, int MOFF, int bv>
+// The same with compile-time sizes (the paper's n_q = n_p + 2), LINE tasks and even-odd contractions: one thread
+// contracts one line of one vector in registers (one tile read and one tile write per point and pass instead of n reads
+// per output).  Array (D0, D1, D2) x bv -> the extent along DIR becomes MO.  The table at c_oi + MOFF is the [Me | Mo]
+// pair of a matrix stored [MO][MI] (TRANS: [MI][MO], applied transposed); ANTI: centro-antisymmetric (D~), else
+// centro-symmetric (N).  y_o = u + v, y_{MO-1-o} = +-(u - v) with u, v the even / odd half products.
+template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ANTI, bool ADD, int MOFF, int bv>
 __device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int tid) {
   constexpr int nth = 256;   // the block size, as a constant: the trip count of the line loop is then known (1 or 2), and
                              // the table values are not hoisted out of it into more uniform registers than exist
@@ -324,6 +329,11 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ src, d
   constexpr int E0 = DIR == 0 ? MO : D0, E1 = DIR == 1 ? MO : D1;            // destination extents
   constexpr int DS = DIR == 0 ? 1 : (DIR == 1 ? E0 : E0 * E1);
   constexpr int nlines = EA * EB * bv;
+  constexpr int HI = (MI + 1) / 2, FI = MI / 2, HO = (MO + 1) / 2, FO = MO / 2;
+  constexpr int HC = TRANS ? HO : HI;                                        // columns of the stored half tables
+  constexpr int TE = MOFF, TO = MOFF + HI * HO;                              // Me, Mo
+  // a transposed antisymmetric matrix has its even part in the stored odd half and vice versa
+  constexpr int UE = (TRANS && ANTI) ? TO : TE, UO = (TRANS && ANTI) ? TE : TO;
 #pragma unroll
   for (int t0 = 0; t0 < nlines; t0 += nth) {
     const int t = t0 + tid;
@@ -332,15 +342,38 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ src, d
     // point index of the line start in source / destination
     const int sbase = DIR == 0 ? D0 * (a + D1 * b) : (DIR == 1 ? a + D0 * D1 * b : a + D0 * b);
     const int dbase = DIR == 0 ? E0 * (a + E1 * b) : (DIR == 1 ? a + E0 * E1 * b : a + E0 * b);
-    double x[MI];
+    double xe[HI], xo[FI > 0 ? FI : 1];
 #pragma unroll
-    for (int i = 0; i < MI; ++i) x[i] = src[(size_t)(sbase + i * SS) * bv + beta];
+    for (int i = 0; i < FI; ++i) {
+      const double p = src[(size_t)(sbase + i * SS) * bv + beta], q = src[(size_t)(sbase + (MI - 1 - i) * SS) * bv + beta];
+      xe[i] = p + q;
+      xo[i] = p - q;
+    }
+    if (MI & 1) xe[FI] = src[(size_t)(sbase + FI * SS) * bv + beta];
 #pragma unroll
-    for (int o = 0; o < MO; ++o) {
-      double acc = ADD ? dst[(size_t)(dbase + o * DS) * bv + beta] : 0.0;
+    for (int o = 0; o < FO; ++o) {
+      double u = 0.0, v = 0.0;
 #pragma unroll
-      for (int i = 0; i < MI; ++i) acc = fma(TRANS ? c_oi[MOFF + i * MO + o] : c_oi[MOFF + o * MI + i], x[i], acc);
-      dst[(size_t)(dbase + o * DS) * bv + beta] = acc;
+      for (int i = 0; i < HI; ++i) u = fma(TRANS ? c_oi[UE + i * HC + o] : c_oi[UE + o * HC + i], xe[i], u);
+#pragma unroll
+      for (int i = 0; i < FI; ++i) v = fma(TRANS ? c_oi[UO + i * HC + o] : c_oi[UO + o * HC + i], xo[i], v);
+      double* d0 = dst + (size_t)(dbase + o * DS) * bv + beta;
+      double* d1 = dst + (size_t)(dbase + (MO - 1 - o) * DS) * bv + beta;
+      const double y0 = u + v, y1 = ANTI ? v - u : u - v;
+      *d0 = ADD ? *d0 + y0 : y0;
+      *d1 = ADD ? *d1 + y1 : y1;
+    }
+    if (MO & 1) {   // middle output: the odd (symmetric matrix) or even (antisymmetric) half vanishes
+      double y = 0.0;
+      if (ANTI) {
+#pragma unroll
+        for (int i = 0; i < FI; ++i) y = fma(TRANS ? c_oi[UO + i * HC + FO] : c_oi[UO + FO * HC + i], xo[i], y);
+      } else {
+#pragma unroll
+        for (int i = 0; i < HI; ++i) y = fma(TRANS ? c_oi[UE + i * HC + FO] : c_oi[UE + FO * HC + i], xe[i], y);
+      }
+      double* d0 = dst + (size_t)(dbase + FO * DS) * bv + beta;
+      *d0 = ADD ? *d0 + y : y;
     }
   }
 }
@@ -353,13 +386,17 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
   double* B1 = B0 + (size_t)NQ3 * bv;
   double* B2 = B1 + (size_t)NQ3 * bv;
   double* T = B2 + (size_t)NQ3 * bv;
-  constexpr int ON = OiOffset<PDEG>::value, OD = OiOffset<PDEG>::value + NQ * N;   // N [NQ][N] and D~ [NQ][NQ] in c_oi
+  constexpr int ON = OiOffset<PDEG>::value, OD = ON + 2 * ((NQ + 1) / 2) * ((N + 1) / 2);   // [Ne | No] and [De | Do] in c_oi
   const int tid = threadIdx.x, nth = blockDim.x;
   const int vb = blockIdx.x % P.nvb;
   const int cell = blockIdx.x / P.nvb;
   const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
   const int v0 = vb * bv;
-  for (int t = tid; t < N * N * N * bv; t += nth) {
+  // S2 gather: compile-time trip count, so that all the loads of a thread are in flight together
+#pragma unroll
+  for (int t0 = 0; t0 < N * N * N * bv; t0 += 256) {
+    const int t = t0 + tid;
+    if (t >= N * N * N * bv) break;
     const int beta = t % bv, I = t / bv;
     const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
@@ -371,21 +408,24 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
       if (iy >= P.ndy) iy -= P.ndy;
       if (iz >= P.ndz) iz -= P.ndz;
     }
-    double xv = live ? P.W[global_node(P, ix, iy, iz) * P.nvec + v0 + beta] : 0.0;
-    if (P.dscale && live) xv *= __ldg(P.dscale + global_node(P, ix, iy, iz));
-    B0[t] = xv;
+    const long long node = live ? global_node(P, ix, iy, iz) : 0;
+    double xv = __ldg(P.W + node * P.nvec + (live ? v0 + beta : 0));
+    const double dv = P.dscale ? __ldg(P.dscale + node) : 1.0;
+    B0[t] = live ? xv * dv : 0.0;
   }
   __syncthreads();
-  contract_lines<N, N, N, 0, NQ, false, false, ON, bv>(B0, B1, tid); __syncthreads();
-  contract_lines<NQ, N, N, 1, NQ, false, false, ON, bv>(B1, B0, tid); __syncthreads();
-  contract_lines<NQ, NQ, N, 2, NQ, false, false, ON, bv>(B0, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, false, false, OD, bv>(T, B0, tid);
-  contract_lines<NQ, NQ, NQ, 1, NQ, false, false, OD, bv>(T, B1, tid);
-  contract_lines<NQ, NQ, NQ, 2, NQ, false, false, OD, bv>(T, B2, tid);
+  contract_lines<N, N, N, 0, NQ, false, false, false, ON, bv>(B0, B1, tid); __syncthreads();
+  contract_lines<NQ, N, N, 1, NQ, false, false, false, ON, bv>(B1, B0, tid); __syncthreads();
+  contract_lines<NQ, NQ, N, 2, NQ, false, false, false, ON, bv>(B0, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, false, true, false, OD, bv>(T, B0, tid);
+  contract_lines<NQ, NQ, NQ, 1, NQ, false, true, false, OD, bv>(T, B1, tid);
+  contract_lines<NQ, NQ, NQ, 2, NQ, false, true, false, OD, bv>(T, B2, tid);
   __syncthreads();
   // one thread = one point for all the block's vectors (the 7 factors are loaded once), two points in flight
-#pragma unroll 2
-  for (int Q = tid; Q < NQ3; Q += nth) {
+#pragma unroll
+  for (int Q0 = 0; Q0 < NQ3; Q0 += 256) {
+    const int Q = Q0 + tid;
+    if (Q >= NQ3) break;
     const int q1 = Q % NQ, q2 = (Q / NQ) % NQ, q3 = Q / (NQ * NQ);
     const double wq = __ldg(O.wq + q1) * __ldg(O.wq + q2) * __ldg(O.wq + q3);
     double g[7];
@@ -408,12 +448,12 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
     }
   }
   __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, OD, bv>(B0, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, OD, bv>(B1, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, OD, bv>(B2, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, N, true, false, ON, bv>(T, B0, tid); __syncthreads();
-  contract_lines<NQ, NQ, N, 1, N, true, false, ON, bv>(B0, B1, tid); __syncthreads();
-  contract_lines<NQ, N, N, 0, N, true, false, ON, bv>(B1, B0, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, true, OD, bv>(B0, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, true, OD, bv>(B1, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, true, OD, bv>(B2, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, NQ, 2, N, true, false, false, ON, bv>(T, B0, tid); __syncthreads();
+  contract_lines<NQ, NQ, N, 1, N, true, false, false, ON, bv>(B0, B1, tid); __syncthreads();
+  contract_lines<NQ, N, N, 0, N, true, false, false, ON, bv>(B1, B0, tid); __syncthreads();
   for (int t = tid; t < N * N * N * bv; t += nth) {
     const int beta = t % bv, I = t / bv;
     const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);

@@ -426,8 +426,21 @@ extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
     return fail(ctx, FE_MF_ENOMEM, "table upload failed (quadrature)");
   }
   if (nq == ctx->p + 3) {   // the compile-time kernel of n_q = n_p + 2 reads its tables from constant memory
-    std::vector<double> pack(hN);
-    pack.insert(pack.end(), hD.begin(), hD.end());
+    // even / odd halves [Ne | No | De | Do] (layout: fe_kernels.cuh, c_oi), halved in long double from the symmetrised pair
+    std::vector<double> pack;
+    auto halves = [&](const std::vector<double>& M, int R, int C, double sgn) {
+      const int hR = (R + 1) / 2, hC = (C + 1) / 2;
+      for (int part = 0; part < 2; ++part)
+        for (int o = 0; o < hR; ++o)
+          for (int i = 0; i < hC; ++i) {
+            // the centro-(anti)symmetry is enforced exactly: entry (o, i) is averaged with its image (R-1-o, C-1-i)
+            const long double a = 0.5L * ((long double)M[(size_t)o * C + i] + sgn * (long double)M[(size_t)(R - 1 - o) * C + (C - 1 - i)]);
+            const long double b = 0.5L * ((long double)M[(size_t)o * C + (C - 1 - i)] + sgn * (long double)M[(size_t)(R - 1 - o) * C + i]);
+            pack.push_back((double)(part == 0 ? 0.5L * (a + b) : 0.5L * (a - b)));
+          }
+    };
+    halves(hN, nq, n, 1.0);
+    halves(hD, nq, nq, -1.0);
     FE_CUDA(ctx, cudaMemcpyToSymbol(fe::c_oi, pack.data(), pack.size() * sizeof(double), sizeof(double) * fe::oi_offset(ctx->p)));
   }
   if (ctx->geom_mode == 2) {   // per-point metric at the nq^3 points (Eq. 7c evaluated at every point of the rule)
