@@ -340,7 +340,7 @@ def run_ours(args):
                 torch.cuda.empty_cache()
             except Exception as exc:
                 others.append({"config": cfg_o, "error": str(exc)[:200]})
-        # config 3 with n_q = n_p + 2 points per direction (functional kernel, not tuned)
+        # config 3 with n_q = n_p + 2 points per direction (even-odd line-task kernel)
         try:
             wo = inputs.configs()[3]
             opo = binding.FeMf.from_workload(wo, device=local)

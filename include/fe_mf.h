@@ -160,8 +160,9 @@ int fe_mf_set_kappa(fe_mf_ctx *ctx, const double *kappa_host);
  * D = D~ N of PAPER.md:188, per-point geometry and kappa live on the n_q^3 points).  On affine cells with constant
  * kappa the result does not change (the n_p-point rule is already exact there).  A kappa array set before belongs
  * to the points of the old rule and is dropped (constant sigma again): call fe_mf_set_kappa afterwards with
- * [ncells][nq^3] values.  With nq != p + 1 every call runs on one plain kernel (rectangular tables, gather /
- * atomic scatter): functional, not tuned.  Synchronises the device.
+ * [ncells][nq^3] values.  With nq = p + 3 the calls run on an even-odd line-task kernel with compile-time sizes, with any
+ * other nq != p + 1 on one plain kernel (rectangular tables); both gather with loads and scatter with atomics.
+ * Synchronises the device.
  */
 int fe_mf_set_quadrature(fe_mf_ctx *ctx, int nq);
 int fe_mf_set_mass_scaling(fe_mf_ctx *ctx, int on);
