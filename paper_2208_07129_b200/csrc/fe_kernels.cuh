@@ -320,7 +320,20 @@ inline int oi_offset(int p) {
 // pair of a matrix stored [MO][MI] (TRANS: [MI][MO], applied transposed); ANTI: centro-antisymmetric (D~), else
 // centro-symmetric (N).  y_o = u + v, y_{MO-1-o} = +-(u - v) with u, v the even / odd half products.
 template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ANTI, bool ADD, int MOFF, int bv>
-__device__ __forceinline__ void contract_lines(const double* __restrict__ src, double* __restrict__ dst, int tid) {
+__device__ __forceinline__ void contract_lines_impl(const double* src, double* dst, int tid);
+// INPLACE: src == dst (square operator, !ADD): a thread reads its whole line before it writes, and no two lines overlap
+template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ANTI, bool ADD, int MOFF, int bv, bool INPLACE = false>
+__device__ __forceinline__ void contract_lines(const double* src, double* dst, int tid) {
+  if (INPLACE) {
+    contract_lines_impl<D0, D1, D2, DIR, MO, TRANS, ANTI, ADD, MOFF, bv>(src, dst, tid);
+  } else {
+    const double* __restrict__ s = src;
+    double* __restrict__ d = dst;
+    contract_lines_impl<D0, D1, D2, DIR, MO, TRANS, ANTI, ADD, MOFF, bv>(s, d, tid);
+  }
+}
+template <int D0, int D1, int D2, int DIR, int MO, bool TRANS, bool ANTI, bool ADD, int MOFF, int bv>
+__device__ __forceinline__ void contract_lines_impl(const double* src, double* dst, int tid) {
   constexpr int nth = 256;   // the block size, as a constant: the trip count of the line loop is then known (1 or 2), and
                              // the table values are not hoisted out of it into more uniform registers than exist
   constexpr int MI = DIR == 0 ? D0 : (DIR == 1 ? D1 : D2);
@@ -378,6 +391,78 @@ __device__ __forceinline__ void contract_lines(const double* __restrict__ src, d
   }
 }
 
+// The even-odd product of contract_lines on a line held in registers: y = M x (TRANS: M^T x), table pair at c_oi + MOFF.
+template <int MI, int MO, bool TRANS, bool ANTI, int MOFF>
+__device__ __forceinline__ void eo_line(const double (&x)[MI], double (&y)[MO]) {
+  constexpr int HI = (MI + 1) / 2, FI = MI / 2, HO = (MO + 1) / 2, FO = MO / 2;
+  constexpr int HC = TRANS ? HO : HI;
+  constexpr int TE = MOFF, TO = MOFF + HI * HO;
+  constexpr int UE = (TRANS && ANTI) ? TO : TE, UO = (TRANS && ANTI) ? TE : TO;
+  double xe[HI], xo[FI > 0 ? FI : 1];
+#pragma unroll
+  for (int i = 0; i < FI; ++i) { xe[i] = x[i] + x[MI - 1 - i]; xo[i] = x[i] - x[MI - 1 - i]; }
+  if (MI & 1) xe[FI] = x[FI];
+#pragma unroll
+  for (int o = 0; o < FO; ++o) {
+    double u = 0.0, v = 0.0;
+#pragma unroll
+    for (int i = 0; i < HI; ++i) u = fma(TRANS ? c_oi[UE + i * HC + o] : c_oi[UE + o * HC + i], xe[i], u);
+#pragma unroll
+    for (int i = 0; i < FI; ++i) v = fma(TRANS ? c_oi[UO + i * HC + o] : c_oi[UO + o * HC + i], xo[i], v);
+    y[o] = u + v;
+    y[MO - 1 - o] = ANTI ? v - u : u - v;
+  }
+  if (MO & 1) {
+    double m = 0.0;
+    if (ANTI) {
+#pragma unroll
+      for (int i = 0; i < FI; ++i) m = fma(TRANS ? c_oi[UO + i * HC + FO] : c_oi[UO + FO * HC + i], xo[i], m);
+    } else {
+#pragma unroll
+      for (int i = 0; i < HI; ++i) m = fma(TRANS ? c_oi[UE + i * HC + FO] : c_oi[UE + FO * HC + i], xe[i], m);
+    }
+    y[FO] = m;
+  }
+}
+
+// z-lines, forward: T = N_z B (N -> NQ points) and, from the same registers, G2 = D~_z T (one tile read, two writes).
+// z-lines, backward: R = D~_z^T G2 + T + G0 + G1 on the line, then N_z^T R (NQ -> N) written IN PLACE over the first N
+// entries of the G2 line (a thread reads its whole line before it writes; lines of different threads are disjoint).
+template <int N, int NQ, int ON, int OD, int bv, bool BACK>
+__device__ __forceinline__ void z_lines(double* B0, double* B1, double* B2, double* T, int tid) {
+  constexpr int nlines = NQ * NQ * bv, ZS = NQ * NQ;
+#pragma unroll
+  for (int t0 = 0; t0 < nlines; t0 += 256) {
+    const int t = t0 + tid;
+    if (t >= nlines) break;
+    const int beta = t % bv, r = t / bv;       // r = a + NQ b: the line's first point
+    if (!BACK) {
+      double x[N], y[NQ], d[NQ];
+#pragma unroll
+      for (int i = 0; i < N; ++i) x[i] = B0[(size_t)(r + i * ZS) * bv + beta];
+      eo_line<N, NQ, false, false, ON>(x, y);
+#pragma unroll
+      for (int o = 0; o < NQ; ++o) T[(size_t)(r + o * ZS) * bv + beta] = y[o];
+      eo_line<NQ, NQ, false, true, OD>(y, d);
+#pragma unroll
+      for (int o = 0; o < NQ; ++o) B2[(size_t)(r + o * ZS) * bv + beta] = d[o];
+    } else {
+      double x[NQ], y[NQ], z[N];
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) x[i] = B2[(size_t)(r + i * ZS) * bv + beta];
+      eo_line<NQ, NQ, true, true, OD>(x, y);
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) {
+        const size_t k = (size_t)(r + i * ZS) * bv + beta;
+        y[i] += (T[k] + B0[k]) + B1[k];
+      }
+      eo_line<NQ, N, true, false, ON>(y, z);
+#pragma unroll
+      for (int o = 0; o < N; ++o) B2[(size_t)(r + o * ZS) * bv + beta] = z[o];
+    }
+  }
+}
+
 template <int PDEG, int NQ, int bv>
 __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const OiParams O) {
   constexpr int N = PDEG + 1, NQ3 = NQ * NQ * NQ;
@@ -431,10 +516,9 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
   __syncthreads();
   contract_lines<N, N, N, 0, NQ, false, false, false, ON, bv>(B0, B1, tid); __syncthreads();
   contract_lines<NQ, N, N, 1, NQ, false, false, false, ON, bv>(B1, B0, tid); __syncthreads();
-  contract_lines<NQ, NQ, N, 2, NQ, false, false, false, ON, bv>(B0, T, tid); __syncthreads();
+  z_lines<N, NQ, ON, OD, bv, false>(B0, B1, B2, T, tid); __syncthreads();   // N_z and D~_z chained in registers
   contract_lines<NQ, NQ, NQ, 0, NQ, false, true, false, OD, bv>(T, B0, tid);
   contract_lines<NQ, NQ, NQ, 1, NQ, false, true, false, OD, bv>(T, B1, tid);
-  contract_lines<NQ, NQ, NQ, 2, NQ, false, true, false, OD, bv>(T, B2, tid);
   __syncthreads();
   // S5: one thread = one point for all the block's vectors (the 7 factors are loaded once); the factors of PF points are
   // loaded before the first is used
@@ -479,11 +563,12 @@ __global__ void __launch_bounds__(256, 2) fe_apply_oi(const ApplyParams P, const
     }
   }
   __syncthreads();
-  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, true, OD, bv>(B0, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, true, OD, bv>(B1, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, NQ, true, true, true, OD, bv>(B2, T, tid); __syncthreads();
-  contract_lines<NQ, NQ, NQ, 2, N, true, false, false, ON, bv>(T, B0, tid); __syncthreads();
-  contract_lines<NQ, NQ, N, 1, N, true, false, false, ON, bv>(B0, B1, tid); __syncthreads();
+  // S6: D~^T_x and D~^T_y in place on their own tiles (no barrier between them), then the z-lines add the four terms
+  // and go on to N^T_z in registers: 11 block barriers per cell instead of 14, no read-modify-write of T
+  contract_lines<NQ, NQ, NQ, 0, NQ, true, true, false, OD, bv, true>(B0, B0, tid);
+  contract_lines<NQ, NQ, NQ, 1, NQ, true, true, false, OD, bv, true>(B1, B1, tid); __syncthreads();
+  z_lines<N, NQ, ON, OD, bv, true>(B0, B1, B2, T, tid); __syncthreads();
+  contract_lines<NQ, NQ, N, 1, N, true, false, false, ON, bv>(B2, B1, tid); __syncthreads();
   contract_lines<NQ, N, N, 0, N, true, false, false, ON, bv>(B1, B0, tid); __syncthreads();
   for (int t = tid; t < N * N * N * bv; t += nth) {
     const int beta = t % bv, I = t / bv;
