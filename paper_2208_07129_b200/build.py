@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libfe_mf.so")
 SOURCES = ["fe_mf.cu", "fe_probe.cu"]
-DEPS = ["fe_kernels.cuh", "fe_kernels_eo.cuh", "fe_kernels_cart2.cuh", "fe_kernels_tma.cuh", "fe_kernels_gen.cuh", "fe_kernels_plane.cuh", "fe_kernels_line.cuh", "fe_kernels_kron.cuh", "fe_init_ahead.cuh", "fe_tables.h", "fe_dispatch.inl", os.path.join("..", "..", "include", "fe_mf.h")]
+DEPS = ["fe_kernels.cuh", "fe_kernels_eo.cuh", "fe_kernels_cart2.cuh", "fe_kernels_tma.cuh", "fe_kernels_gen.cuh", "fe_kernels_plane.cuh", "fe_kernels_line.cuh", "fe_kernels_kron.cuh", "fe_kernels_oi.cuh", "fe_init_ahead.cuh", "fe_tables.h", "fe_dispatch.inl", os.path.join("..", "..", "include", "fe_mf.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

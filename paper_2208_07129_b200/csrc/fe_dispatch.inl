@@ -38,6 +38,7 @@ cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStr
 }
 
 // ---- kind 11: n_q != n_p points per direction (over-integration): plain kernel with rectangular tables
+bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim, int padx);
 int oi_bv(int nq, int nvec) {
   int bv = 4;   // the compile-time kernel is instantiated for 2 and 4 vectors per block
   while (bv > 1 && ((size_t)4 * nq * nq * nq * bv * 8 > kMaxSmem / 2 - 4096 || bv > nvec)) bv >>= 1;
@@ -63,7 +64,14 @@ cudaError_t launch_general_oi(const fe_mf_ctx* c, const fe::ApplyParams& prm, cu
       if (e != cudaSuccess) return e;
       conf = smem;
     }
-    kern<<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);
+    // interior cells take their tile through TMA (same conditions as the other TMA kernels); the rest of the cells, and
+    // calls that do not meet them, gather with loads and scatter with atomics inside the same kernel
+    CUtensorMap tw, tz;
+    memset(&tw, 0, sizeof(tw)); memset(&tz, 0, sizeof(tz));
+    const bool aligned = ((((uintptr_t)prm.W) | ((uintptr_t)prm.Z)) & 15) == 0;
+    const int use_tma = !(prm.nvec & 1) && aligned && c->variant != 1 &&
+                        make_tensor_map(&tw, c, prm.W, prm.nvec, prm.bv, 0, 0) && make_tensor_map(&tz, c, prm.Z, prm.nvec, prm.bv, 0, 0);
+    kern<<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(tw, tz, prm, O, use_tma);
     return cudaGetLastError();
   }
   fe::fe_apply_general_oi<PDEG><<<(unsigned)(c->ncells * prm.nvb), 256, smem, st>>>(prm, O);

@@ -18,6 +18,7 @@
 #include "fe_kernels_plane.cuh"
 #include "fe_kernels_line.cuh"
 #include "fe_kernels_kron.cuh"
+#include "fe_kernels_oi.cuh"
 #include "fe_tables.h"
 
 struct fe_mf_ctx {
