@@ -161,7 +161,7 @@ int fe_mf_set_kappa(fe_mf_ctx *ctx, const double *kappa_host);
  * kappa the result does not change (the n_p-point rule is already exact there).  A kappa array set before belongs
  * to the points of the old rule and is dropped (constant sigma again): call fe_mf_set_kappa afterwards with
  * [ncells][nq^3] values.  With nq = p + 3 the calls run on an even-odd line-task kernel with compile-time sizes, with any
- * other nq != p + 1 on one plain kernel (rectangular tables); both gather with loads and scatter with atomics.
+ * other nq != p + 1 on one plain kernel (rectangular tables, loads and atomics).
  * Synchronises the device.
  */
 int fe_mf_set_quadrature(fe_mf_ctx *ctx, int nq);

@@ -114,3 +114,32 @@ def test_kappa_mass_scaling_and_filter_with_np_plus_2_points(env, kind, bc):
     op.set_mass_scaling(False)
     op.set_quadrature(p + 1)
     assert relerr(run(torch, op, X, nvec), orc.Operator(mesh, 0.7).apply(X)) <= TOL
+
+
+@pytest.mark.parametrize("p", [2, 5])
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+def test_interior_cells_take_the_tma_path(env, p, bc):
+    """Cells that neither wrap around nor touch the Dirichlet boundary load their tile with one bulk tensor copy and
+    leave through one bulk tensor reduction (fe_kernels_oi.cuh); (4, 3, 4) cells have such cells under both boundary
+    conditions, and 6 vectors leave a vector tail for the TMA unit to zero-fill and clip."""
+    torch, orc, binding = env
+    op, mesh = make_pair(env, p, bc, "perturbed_q", ncells=(4, 3, 4))
+    nq = p + 3
+    op.set_quadrature(nq)
+    oo = orc.Operator(mesh, 0.7, nq=nq)
+    for nvec in (6, 2):
+        assert op.kernel_name(nvec) == "fe_apply_oi"
+        X = inputs.multivector(57, mesh.ndof, nvec)
+        Y = run(torch, op, X, nvec)
+        assert relerr(Y, oo.apply(X)) <= TOL
+        op.set_variant(1)                     # the same kernel with loads and atomics on every cell
+        Y1 = run(torch, op, X, nvec)
+        op.set_variant(0)
+        assert relerr(Y, Y1) <= 1e-14
+    # Eq. B.1 through the TMA path: Z <- a A W + b Z + c W
+    X = inputs.multivector(58, mesh.ndof, 4)
+    Z = inputs.multivector(59, mesh.ndof, 4)
+    Xd, Zd = torch.from_numpy(X).cuda(), torch.from_numpy(Z).cuda()
+    op.apply_axpby(0.7, Xd, -0.3, 1.9, Zd, 4)
+    torch.cuda.synchronize()
+    assert relerr(Zd.cpu().numpy(), 0.7 * oo.apply(X) - 0.3 * Z + 1.9 * X) <= TOL
