@@ -188,7 +188,8 @@ int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
  * 1 general fallback kernel, 2 one-vector-per-thread Cartesian kernel (LDG/RED), 7 full-metric TMA kernel on a
  * Cartesian mesh, 8 plane kernel (p = 6, 7), 10 / 11 line kernel with 16 / 8 vectors per block, 12 Kronecker-product kernel (uniform box, constant
  * kappa; fe_kernels_kron.cuh), 19 plane kernel
- * that also initialises the output (one cooperative launch).  Returns EINVAL if unknown. */
+ * that also initialises the output (one cooperative launch), 21 / 22 over-integration kernel with three / two 2-vector
+ * blocks per SM (with 1: loads and atomics on every cell instead of TMA).  Returns EINVAL if unknown. */
 int fe_mf_set_variant(fe_mf_ctx *ctx, int variant);
 
 /* Message of the last failing call on ctx; with ctx == NULL, of the last failing fe_mf_create on

@@ -39,8 +39,9 @@ cudaError_t launch_general(const fe::ApplyParams& prm, long long ncells, cudaStr
 
 // ---- kind 11: n_q != n_p points per direction (over-integration): plain kernel with rectangular tables
 bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim, int padx);
-int oi_bv(int nq, int nvec) {
-  int bv = 4;   // the compile-time kernel is instantiated for 2 and 4 vectors per block
+int oi_bv(int nq, int nvec, int variant = 0) {
+  // the compile-time kernel is instantiated for 2 and 4 vectors per block; 2 wherever three such blocks fit an SM
+  int bv = ((size_t)3 * ((size_t)4 * nq * nq * nq * 2 * 8 + 4096) <= kMaxSmem || variant == 21 || variant == 22) ? 2 : 4;
   while (bv > 1 && ((size_t)4 * nq * nq * nq * bv * 8 > kMaxSmem / 2 - 4096 || bv > nvec)) bv >>= 1;
   return bv;
 }
@@ -56,9 +57,16 @@ cudaError_t launch_general_oi(const fe_mf_ctx* c, const fe::ApplyParams& prm, cu
     configured = smem;
   }
   if (nq == PDEG + 3 && (prm.bv == 2 || prm.bv == 4)) {   // the paper's n_q = n_p + 2: compile-time sizes, line tasks
-    auto kern = prm.bv == 2 ? fe::fe_apply_oi<PDEG, PDEG + 3, 2> : fe::fe_apply_oi<PDEG, PDEG + 3, 4>;
-    static size_t configured2[2] = {0, 0};
-    size_t& conf = configured2[prm.bv == 4];
+    // 2-vector blocks, three or four per SM, where four tiles fit that often (n_q <= 10 / n_q <= 9): measured faster
+    // than two 4-vector blocks (p = 6: 25.4 -> 27.2 with three); variants 21 / 22 force three / two for comparison
+    constexpr size_t TB2 = (size_t)4 * (PDEG + 3) * (PDEG + 3) * (PDEG + 3) * 2 * 8 + 4096;
+    constexpr int MB = 4 * TB2 <= kMaxSmem ? 4 : (3 * TB2 <= kMaxSmem ? 3 : 2);
+    const int mb = prm.bv != 2 ? 2 : (c->variant == 22 ? 2 : (c->variant == 21 ? (MB >= 3 ? 3 : 2) : MB));
+    auto kern = prm.bv == 4 ? fe::fe_apply_oi<PDEG, PDEG + 3, 4>
+              : mb == 4 ? fe::fe_apply_oi<PDEG, PDEG + 3, 2, MB == 4 ? 4 : 2>
+              : mb == 3 ? fe::fe_apply_oi<PDEG, PDEG + 3, 2, MB >= 3 ? 3 : 2> : fe::fe_apply_oi<PDEG, PDEG + 3, 2>;
+    static size_t configured2[4] = {0, 0, 0, 0};
+    size_t& conf = configured2[prm.bv == 4 ? 0 : mb - 1];
     if (smem > conf) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       if (e != cudaSuccess) return e;
@@ -383,7 +391,7 @@ int kernel_bv(const fe_mf_ctx* c, int kind, int nvec) {
     case 6: return c->p == 8 ? 4 : kGenBv;
     case 8: return 16;
     case 10: return kron_bv(c->p);
-    case 11: return oi_bv(c->nq_oi, nvec);
+    case 11: return oi_bv(c->nq_oi, nvec, c->variant);
     default: return line_bv(c, nvec);
   }
 }
@@ -753,7 +761,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
   const bool known = variant == 0 || variant == 1 || variant == 2 || variant == 7 || variant == 8 || variant == 10 ||
-                     variant == 11 || variant == 12 || variant == 19;
+                     variant == 11 || variant == 12 || variant == 19 || variant == 21 || variant == 22;
   if (!known) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;

@@ -169,8 +169,8 @@ __device__ __forceinline__ void z_lines(double* B0, double* B1, double* B2, doub
   }
 }
 
-template <int PDEG, int NQ, int bv>
-__global__ void __launch_bounds__(256, 2)
+template <int PDEG, int NQ, int bv, int MINB = 2>
+__global__ void __launch_bounds__(256, MINB)
 fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ, const ApplyParams P,
             const OiParams O, int use_tma) {
   constexpr int N = PDEG + 1, NQ3 = NQ * NQ * NQ;
