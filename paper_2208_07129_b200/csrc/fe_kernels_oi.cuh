@@ -186,14 +186,15 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
   const int cell = blockIdx.x / P.nvb;
   const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
   const int v0 = vb * bv;
-  // S2 gather.  A cell whose tile neither wraps around nor touches the Dirichlet boundary takes it through ONE 4-D
-  // tensor-map bulk copy (box (bv, n, n, n) = the layout of B0; the vector tail is zero-filled by the TMA unit); the
-  // other cells, and contexts with the M^-1/2 diagonal, gather with loads, branch-free and in two stages (all the loads
-  // of a thread are issued before the first is consumed: with one load per dependent iteration the phase took 30 % of
-  // the kernel, ncu)
+  // S2 gather: ONE 4-D tensor-map bulk copy per block (box (bv, n, n, n) = the layout of B0; the vector tail and the
+  // nodes past the end of a periodic mesh are zero-filled by the TMA unit).  A cell that wraps around then fetches its
+  // wrapped nodes with loads, a cell on the Dirichlet boundary zeroes its boundary nodes in the tile.  Contexts with the
+  // M^-1/2 diagonal, and calls the TMA conditions exclude, gather with loads, branch-free and in two stages (all the
+  // loads of a thread are issued before the first is consumed: with one load per dependent iteration the phase took
+  // 30 % of the kernel, ncu)
   const bool special = P.dirichlet ? (ex == 0 || ex == P.ncx - 1 || ey == 0 || ey == P.ncy - 1 || ez == 0 || ez == P.ncz - 1)
                                    : (ex == P.ncx - 1 || ey == P.ncy - 1 || ez == P.ncz - 1);
-  const bool tma = use_tma && !special && !P.dscale;   // uniform over the block
+  const bool tma = use_tma && !P.dscale;   // uniform over the block
   constexpr int TOT = N * N * N * bv, GI = (TOT + 255) / 256;
   if (tma) {
     if (tid == 0) {
@@ -204,6 +205,26 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
     }
     __syncthreads();
     mbar_wait(&bar, 0);
+    if (special) {
+#pragma unroll
+      for (int k = 0; k < GI; ++k) {
+        const int t = k * 256 + tid;
+        const int beta = t % bv, I = t / bv;
+        const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+        int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+        const bool in = (k + 1) * 256 <= TOT || t < TOT;
+        if (P.dirichlet) {
+          const bool bnd = ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1;
+          if (in && bnd) B0[t] = 0.0;
+        } else {
+          const bool wrapped = ix >= P.ndx || iy >= P.ndy || iz >= P.ndz;
+          ix = ix >= P.ndx ? ix - P.ndx : ix;
+          iy = iy >= P.ndy ? iy - P.ndy : iy;
+          iz = iz >= P.ndz ? iz - P.ndz : iz;
+          if (in && wrapped && (v0 + beta) < P.nvec) B0[t] = __ldg(P.W + global_node(P, ix, iy, iz) * P.nvec + v0 + beta);
+        }
+      }
+    }
   } else
   {
     double xv[GI];
@@ -295,8 +316,24 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
   z_lines<N, NQ, ON, OD, bv, true>(B0, B1, B2, T, tid); __syncthreads();
   contract_lines<NQ, NQ, N, 1, N, true, false, false, ON, bv>(B2, B1, tid); __syncthreads();
   contract_lines<NQ, N, N, 0, N, true, false, false, ON, bv>(B1, B0, tid); __syncthreads();
-  // S8 scatter-add: ONE bulk tensor reduction (add.f64 in L2, clipped at the vector tail) or, on the other cells, atomics
+  // S8 scatter-add: ONE bulk tensor reduction (add.f64 in L2, clipped at the vector tail and at the end of the mesh)
   if (tma) {
+    if (special) {   // wrapped nodes (clipped by the reduction) leave through atomics; Dirichlet boundary rows add 0
+      for (int t = tid; t < TOT; t += nth) {
+        const int beta = t % bv, I = t / bv;
+        const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
+        int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
+        if (P.dirichlet) {
+          if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) B0[t] = 0.0;
+        } else {
+          const bool wrapped = ix >= P.ndx || iy >= P.ndy || iz >= P.ndz;
+          ix = ix >= P.ndx ? ix - P.ndx : ix;
+          iy = iy >= P.ndy ? iy - P.ndy : iy;
+          iz = iz >= P.ndz ? iz - P.ndz : iz;
+          if (wrapped && (v0 + beta) < P.nvec) atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], B0[t]);
+        }
+      }
+    }
     fence_async_smem();
     __syncthreads();
     if (tid == 0) {

@@ -119,9 +119,9 @@ def test_kappa_mass_scaling_and_filter_with_np_plus_2_points(env, kind, bc):
 @pytest.mark.parametrize("p", [2, 5])
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
 def test_interior_cells_take_the_tma_path(env, p, bc):
-    """Cells that neither wrap around nor touch the Dirichlet boundary load their tile with one bulk tensor copy and
-    leave through one bulk tensor reduction (fe_kernels_oi.cuh); (4, 3, 4) cells have such cells under both boundary
-    conditions, and 6 vectors leave a vector tail for the TMA unit to zero-fill and clip."""
+    """Every cell loads its tile with one bulk tensor copy and leaves through one bulk tensor reduction
+    (fe_kernels_oi.cuh); cells that wrap around or touch the Dirichlet boundary patch the tile.  (4, 3, 4) cells have
+    interior, wrap-around and boundary cells, and 6 vectors leave a vector tail for the TMA unit to zero-fill and clip."""
     torch, orc, binding = env
     op, mesh = make_pair(env, p, bc, "perturbed_q", ncells=(4, 3, 4))
     nq = p + 3
