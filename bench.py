@@ -340,29 +340,31 @@ def run_ours(args):
                 torch.cuda.empty_cache()
             except Exception as exc:
                 others.append({"config": cfg_o, "error": str(exc)[:200]})
-        # config 3 with n_q = n_p + 2 points per direction (even-odd line-task kernel)
-        try:
-            wo = inputs.configs()[3]
-            opo = binding.FeMf.from_workload(wo, device=local)
-            opo.set_quadrature(wo.p + 3)
-            no = wo.ndof * wo.nvec
-            Xo = torch.empty(no, dtype=torch.float64, device="cuda"); Yo_ = torch.zeros_like(Xo)
-            binding.fill_uniform(Xo, wo.seed)
-            for _ in range(2):
-                opo.accumulate(1.0, Xo, Yo_, wo.nvec)
-            ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-            ev[0].record(stream)
-            for _ in range(5):
-                opo.accumulate(1.0, Xo, Yo_, wo.nvec)
-            ev[1].record(stream)
-            torch.cuda.synchronize()
-            t_kern = ev[0].elapsed_time(ev[1]) / 5
-            others.append({"workload": wo.name + " with n_q = n_p + 2", "p": wo.p, "nvec": wo.nvec,
-                           "kernel": opo.kernel_name(wo.nvec), "kernel_only": no / (t_kern * 1e-3) / 1e9, "kernel_ms": t_kern})
-            del Xo, Yo_, opo
-            torch.cuda.empty_cache()
-        except Exception as exc:
-            others.append({"workload": "n_q = n_p + 2", "error": str(exc)[:200]})
+        # n_q = n_p + 2 points per direction on the meshes of configs 3, 4, 2 (even-odd line-task
+        # kernel); kernel only
+        for cfg_o, nv_o in ((3, 16), (4, 16), (2, 32)):
+            try:
+                wo = inputs.configs()[cfg_o]
+                opo = binding.FeMf.from_workload(wo, device=local)
+                opo.set_quadrature(wo.p + 3)
+                no = wo.ndof * nv_o
+                Xo = torch.empty(no, dtype=torch.float64, device="cuda"); Yo_ = torch.zeros_like(Xo)
+                binding.fill_uniform(Xo, wo.seed)
+                for _ in range(2):
+                    opo.accumulate(1.0, Xo, Yo_, nv_o)
+                ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                ev[0].record(stream)
+                for _ in range(5):
+                    opo.accumulate(1.0, Xo, Yo_, nv_o)
+                ev[1].record(stream)
+                torch.cuda.synchronize()
+                t_kern = ev[0].elapsed_time(ev[1]) / 5
+                others.append({"workload": wo.name + " with n_q = n_p + 2", "p": wo.p, "nvec": nv_o,
+                               "kernel": opo.kernel_name(nv_o), "kernel_only": no / (t_kern * 1e-3) / 1e9, "kernel_ms": t_kern})
+                del Xo, Yo_, opo
+                torch.cuda.empty_cache()
+            except Exception as exc:
+                others.append({"workload": "cfg%d with n_q = n_p + 2" % cfg_o, "error": str(exc)[:200]})
 
     # ---- roofline of the dominant kernel
     diag = (w.geom == inputs.GEOM_AFFINE)
