@@ -77,6 +77,8 @@ long long fe_mf_ndofs(const fe_mf_ctx *ctx);
  *                does not synchronise the host (it can be captured in a CUDA graph after a first call).
  *                A context owns the work counters of its persistent kernels: calls on ONE context must be
  *                stream-ordered (use one context per stream for concurrent applies).
+ *                Pointers need only be 8-byte aligned; the TMA kernels serve 16-byte aligned pointers with an even
+ *                nvec, everything else runs on kernels with plain loads and atomics (same result, slower).
  * Errors: EINVAL (null pointers, nvec < 1, aliasing), ECUDA.
  */
 int fe_mf_apply(fe_mf_ctx *ctx, const double *X_dev, double *Y_dev, int nvec, void *cuda_stream);
@@ -116,8 +118,8 @@ int fe_cheb_filter(fe_mf_ctx *ctx, double *X_dev, double *Y_dev, int nvec, int m
 /*
  * fe_mf_apply_host -- end-to-end convenience: same as fe_mf_apply but X_host / Y_host are HOST
  * buffers (pinned memory recommended).  The library stages column blocks through an internal
- * device workspace (H2D copy, kernels, D2H copy, overlapped on internal streams) and returns
- * after Y_host is complete.  Errors as fe_mf_apply plus ENOMEM.
+ * device workspace (H2D copy, kernels, D2H copy, overlapped on two internal streams, each with its own
+ * work counter) and returns after Y_host is complete.  Errors as fe_mf_apply plus ENOMEM.
  */
 int fe_mf_apply_host(fe_mf_ctx *ctx, const double *X_host, double *Y_host, int nvec);
 
@@ -184,12 +186,10 @@ int fe_mf_shape(const fe_mf_ctx *ctx, int nd[3], int *bc, int *cuda_device);
 const char *fe_mf_kernel_name(const fe_mf_ctx *ctx, int nvec);   /* static string, never NULL */
 int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
 
-/* Select a kernel variant (0 = default: chosen from degree, geometry and nvec).  For profiling/ablation only:
- * 1 general fallback kernel, 2 one-vector-per-thread Cartesian kernel (LDG/RED), 7 full-metric TMA kernel on a
- * Cartesian mesh, 8 plane kernel (p = 6, 7), 10 / 11 line kernel with 16 / 8 vectors per block, 12 Kronecker-product kernel (uniform box, constant
- * kappa; fe_kernels_kron.cuh), 19 plane kernel
- * that also initialises the output (one cooperative launch), 21 / 22 over-integration kernel with three / two 2-vector
- * blocks per SM (with 1: loads and atomics on every cell instead of TMA).  Returns EINVAL if unknown. */
+/* Select a kernel variant (0 = default: chosen from degree, geometry and nvec).  For tests and profiling only:
+ * 1 general fallback kernel (with n_q != n_p: loads and atomics on every cell instead of TMA), 2 one-vector-per-thread
+ * Cartesian kernel (LDG/RED), 7 full-metric TMA kernel on a Cartesian mesh, 8 plane kernel (p = 6), 10 / 11 line
+ * kernel with 16 / 8 vectors per block.  Returns EINVAL if unknown. */
 int fe_mf_set_variant(fe_mf_ctx *ctx, int variant);
 
 /* Message of the last failing call on ctx; with ctx == NULL, of the last failing fe_mf_create on

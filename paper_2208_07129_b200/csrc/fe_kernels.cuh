@@ -5,39 +5,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-namespace fe {
+#include "fe_params.h"
 
-constexpr int KMAXN = 9;
+namespace fe {
 
 // 1D tables per degree p (functions of p only, so contexts can share them).
 // c_N[p][q*n+i] = N1D, c_D[p][q*n+r] = D~1D, c_w[p][q] = Gauss weights.
-__constant__ double c_N[KMAXN][KMAXN * KMAXN];
-__constant__ double c_D[KMAXN][KMAXN * KMAXN];
-__constant__ double c_w[KMAXN][KMAXN];
-
-struct ApplyParams {
-  const double* __restrict__ W;   // input multivector  [ndof][nvec]
-  double* __restrict__ Z;         // output multivector [ndof][nvec], pre-initialised; Z += alpha*A*W
-  const double* __restrict__ geom;  // per-q-point: [cell][7][n^3]; per-cell: [cell][7]; or nullptr (uniform); no w_Q factor
-  double ug[7];                   // uniform Cartesian: G00,G01,G02,G11,G12,G22 (x det J), sigma*det J
-  double alpha;
-  int ncx, ncy, ncz;
-  int ndx, ndy, ndz;
-  int nvec;
-  int bv;                         // vectors per block
-  int nvb;                        // ceil(nvec / bv)
-  int dirichlet;                  // 1: boundary nodes read as 0 / not written
-  int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
-  int nsm;                        // SM count (persistent kernels)
-  long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
-  int* item_ctr;                  // persistent kernels: work counter (0 at launch); item = gridDim.x + atomicAdd after the first
-  double idw;                     // plane kernel with IDENT (periodic meshes): Z += alpha A W + idw W
-  const double* dscale;           // nullptr, or d = diag(M)^-1/2 [ndof] of the GLL-lumped mass matrix: Z += alpha d.(A (d.W))
-                                  // (Eq. B.1; kernels of kinds 1 and 6 only)
-  const double* kappa;            // nullptr, or kappa at the quadrature points [cell][n^3] of a uniform box (geom_mode 0):
-                                  // the mass factor is ug[6] * kappa_Q, ug[6] then holding det J without sigma
-                                  // (kind 1, and the Cartesian kernels instantiated with EIG)
-};
+// static: every translation unit that includes this header owns a private copy, filled by its upload function.
+static __constant__ double c_N[KMAXN][KMAXN * KMAXN];
+static __constant__ double c_D[KMAXN][KMAXN * KMAXN];
+static __constant__ double c_w[KMAXN][KMAXN];
 
 // y[q] = sum_i M[q][i] x[i] (TRANS = false) or sum_i M[i][q] x[i] (TRANS = true) along one line.
 template <int N, bool TRANS, bool ADD>
@@ -177,14 +154,6 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
 // ---- n_q != n_p Gauss points per direction (over-integration) ----------------
 // Plain sum factorisation with RECTANGULAR 1D tables (N: n_q x n_p) and the collocation derivative on the n_q points
 // (D = D~ N), n_q a run-time value: the general fallback of this operator variant, any geometry, any nvec.
-struct OiParams {
-  int nq;                     // Gauss points per direction
-  const double* Nq;           // [nq][n]   N[q][i] = l_i(xq_q)
-  const double* Dq;           // [nq][nq]  D~[q][r] = l~_r'(xq_q)
-  const double* wq;           // [nq]
-  const double* geom;         // geom_mode 2: [cell][7][nq^3] (no w factor), else unused
-  long long geom_stride;
-};
 
 // dst (+)= M src along direction `dir` of a (d0, d1, d2) x bv array; M is mo x mi (or its transpose, stored mi x mo)
 __device__ __forceinline__ void contract_rt(const double* M, int ldm, bool trans, int mo, int mi, int dir, const double* src,
@@ -297,80 +266,6 @@ __global__ void __launch_bounds__(256) fe_apply_general_oi(const ApplyParams P, 
       const double dv = P.dscale ? __ldg(P.dscale + global_node(P, ix, iy, iz)) : 1.0;
       atomicAdd(&P.Z[global_node(P, ix, iy, iz) * P.nvec + v0 + beta], P.alpha * (dv * B0[t]));
     }
-  }
-}
-
-// S1 / S9 pre-pass: Z <- beta*Z + gamma*W  (Eq. B.1's bX + cY part)
-__global__ void fe_axpby_kernel(double* __restrict__ Z, const double* __restrict__ W, double beta, double gamma,
-                                size_t count) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  const size_t n2 = count / 2;
-  double2* Z2 = reinterpret_cast<double2*>(Z);
-  const double2* W2 = reinterpret_cast<const double2*>(W);
-  for (size_t k = i; k < n2; k += stride) {
-    double2 z = Z2[k], w = W2[k];
-    z.x = beta * z.x + gamma * w.x;
-    z.y = beta * z.y + gamma * w.y;
-    Z2[k] = z;
-  }
-  if (i == 0 && (count & 1)) Z[count - 1] = beta * Z[count - 1] + gamma * W[count - 1];
-}
-
-// Z <- gamma*W (beta == 0: Z is not read, so it may hold anything, e.g. NaN from a fresh allocation)
-__global__ void fe_scale_copy_kernel(double* __restrict__ Z, const double* __restrict__ W, double gamma, size_t count) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (size_t k = i; k < count; k += stride) Z[k] = gamma * W[k];
-}
-
-__global__ void fe_scale_kernel(double* Z, double beta, size_t count) {   // Z <- beta Z
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  double2* Z2 = reinterpret_cast<double2*>(Z);
-  for (size_t k = i; k < count / 2; k += stride) { double2 z = Z2[k]; z.x *= beta; z.y *= beta; Z2[k] = z; }
-  if (i == 0 && (count & 1)) Z[count - 1] *= beta;
-}
-
-// The end of the scaled Chebyshev recurrence (fe_cheb_filter): A <- sa * A, B <- sb * B (swap = 0) or
-// A <- sa * B_old, B <- sb * A_old (swap = 1).  On a Dirichlet mesh (bnd = 1) the kernels never touch the boundary
-// nodes, whose entries follow the scalar recurrence: there A still holds the input x0, and A <- qa x0, B <- qb x0.
-__global__ void fe_scale2_kernel(double* __restrict__ A, double* __restrict__ B, double sa, double sb, int swap, size_t count,
-                                 int bnd, double qa, double qb, int ndx, int ndy, int ndz, int nvec) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (size_t k = i; k < count; k += stride) {
-    const double a = A[k], b = B[k];
-    if (bnd) {
-      const size_t node = k / (size_t)nvec;
-      const int ix = (int)(node % ndx), iy = (int)((node / ndx) % ndy), iz = (int)(node / ((size_t)ndx * ndy));
-      if (ix == 0 || ix == ndx - 1 || iy == 0 || iy == ndy - 1 || iz == 0 || iz == ndz - 1) {
-        A[k] = qa * a; B[k] = qb * a;
-        continue;
-      }
-    }
-    A[k] = sa * (swap ? b : a);
-    B[k] = sb * (swap ? a : b);
-  }
-}
-
-__global__ void fe_swap_kernel(double* __restrict__ A, double* __restrict__ B, size_t count) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (size_t k = i; k < count; k += stride) { double a = A[k]; A[k] = B[k]; B[k] = a; }
-}
-
-// Input generator; not part of the operator.
-__global__ void fe_fill_uniform_kernel(double* __restrict__ out, long long count, unsigned long long seed,
-                                       long long offset) {
-  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long k = i; k < count; k += stride) {
-    unsigned long long z = seed + (unsigned long long)(offset + k) * 0x9E3779B97F4A7C15ULL;
-    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
-    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
-    z ^= z >> 31;
-    out[k] = 2.0 * ((double)(z >> 11) * 0x1.0p-53) - 1.0;
   }
 }
 

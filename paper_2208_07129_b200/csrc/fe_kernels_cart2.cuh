@@ -14,10 +14,6 @@ __device__ __forceinline__ v2 operator-(v2 x, v2 y) { return {x.a - y.a, x.b - y
 __device__ __forceinline__ v2 vmul(double c, v2 x) { return {c * x.a, c * x.b}; }
 __device__ __forceinline__ v2 vfma(double c, v2 x, v2 y) { return {fma(c, x.a, y.a), fma(c, x.b, y.b)}; }
 
-enum { MAT_NS = 0, MAT_DS = 1, MAT_SH = 2, MAT_NSS = 3, MAT_M1 = 4, MAT_K1 = 5 };   // Ns, Ds, Ds^T Ds / 2 (symmetric type, like Ns),
-                                                          // Ns diag(w~)^-1/2 (mass-scaled interpolation, see EIG),
-                                                          // M1 = Ns^T Ns, K1 = (Ds Ns)^T (Ds Ns) (fe_kernels_kron.cuh)
-
 // y = M x or M^T x from the half tables of M (c_eo[PDEG][EO_NS] or c_eo[PDEG][EO_DS]).
 template <int PDEG, int MAT, bool TRANS, typename T>
 __device__ __forceinline__ void eo2(const T (&x)[PDEG + 1], T (&y)[PDEG + 1]) {

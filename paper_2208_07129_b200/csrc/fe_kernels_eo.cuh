@@ -13,22 +13,7 @@
 
 namespace fe {
 
-// Half tables of one n x n matrix M with M[n-1-q][n-1-i] = s M[q][i] (s = +1 "sym", -1 "anti"); h = n/2.
-//   P[q][i]  = (M[q][i] + M[q][n-1-i])/2   multiplies x+_i = x_i + x_{n-1-i}
-//   Mn[q][i] = (M[q][i] - M[q][n-1-i])/2   multiplies x-_i = x_i - x_{n-1-i}
-//   Pm[q]    = M[q][m]                      multiplies the middle entry (n odd)
-//   mid[i]   = M[m][i] (i < h), midm = M[m][m]: the middle row (n odd)
-// y_q = u + v, y_{n-1-q} = s (u - v) with u = P x+ + Pm x_m, v = Mn x-.
-struct EoTab {
-  double P[16];
-  double Mn[16];
-  double Pm[4];
-  double mid[4];
-  double midm;
-  double pad[3];
-};
-enum { EO_NS = 0, EO_NST = 1, EO_DS = 2, EO_DST = 3, EO_SH = 4 };   // EO_SH: Ds^T Ds / 2 (symmetric type)
-__constant__ EoTab c_eo[KMAXN][5];
+static __constant__ EoTab c_eo[KMAXN][5];
 
 template <int PDEG, int KIND>
 __device__ __forceinline__ void eo_apply(const double (&x)[PDEG + 1], double (&y)[PDEG + 1]) {

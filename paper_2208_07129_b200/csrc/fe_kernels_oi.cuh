@@ -10,15 +10,7 @@ namespace fe {
 // fe_mf_set_quadrature; the values depend on p only): [Ne | No | De | Do], N (nq x n) centro-symmetric, D~ (nq x nq)
 // centro-antisymmetric (SURVEY.md 8(c) reading 14), Me[o][i] = (M[o][i] + M[o][C-1-i]) / 2, Mo[o][i] = (M[o][i] - M[o][C-1-i]) / 2
 // for o < ceil(R/2), i < ceil(C/2).  Constant-bank FMA operands like the other tables.
-constexpr int oi_size(int p) { return 2 * ((p + 4) / 2) * ((p + 2) / 2) + 2 * ((p + 4) / 2) * ((p + 4) / 2); }
-template <int P_> struct OiOffset { static constexpr int value = OiOffset<P_ - 1>::value + oi_size(P_ - 1); };
-template <> struct OiOffset<1> { static constexpr int value = 0; };
-__constant__ double c_oi[OiOffset<9>::value];
-inline int oi_offset(int p) {
-  int off = 0;
-  for (int k = 1; k < p; ++k) off += oi_size(k);
-  return off;
-}
+static __constant__ double c_oi[OiOffset<9>::value];
 
 // The same with compile-time sizes (the paper's n_q = n_p + 2), LINE tasks and even-odd contractions: one thread
 // contracts one line of one vector in registers (one tile read and one tile write per point and pass instead of n reads

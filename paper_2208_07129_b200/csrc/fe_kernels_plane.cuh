@@ -23,7 +23,6 @@
 // middle-column tables (HALF) and by the scalar of the final accumulate.
 #pragma once
 #include "fe_kernels_tma.cuh"
-#include "fe_init_ahead.cuh"
 
 #ifndef FE_ZLOOP_PRAGMA   // the z-line loops of P2 / P4: rolled (small code) or unrolled (loads hoisted)
 #define FE_ZLOOP_PRAGMA _Pragma("unroll 1")
@@ -31,14 +30,7 @@
 
 namespace fe {
 
-struct EoTab2 {
-  double P[16], Mn[16];
-  double Pm[4], mid[4];
-  double Pmh[4], midh[4];   // Pm / 2, mid / 2
-  double midm, midmh;       // M[mid][mid] and half of it
-  double pad[2];
-};
-__constant__ EoTab2 c_eo2[KMAXN][6];   // [p][MAT_NS | MAT_DS | MAT_SH | MAT_NSS | MAT_M1 | MAT_K1]
+static __constant__ EoTab2 c_eo2[KMAXN][MAT_COUNT];   // [p][MAT_NS | MAT_DS | MAT_SH | MAT_NSS]
 
 // The primitives are generic in the value type T: double (one vector per thread, plane kernels) or v2 (two
 // vectors per thread, line kernels).
@@ -166,8 +158,7 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
 }
 
 // Z (+)= A W on uniform Cartesian cells (diagonal constant metric; alpha folded into P.ug).  One block = one
-// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta.  With I.mode != INIT_NONE the
-// kernel also initialises Z (fe_init_ahead.cuh) and must be launched cooperatively.
+// cell x BV vectors per item, persistent; thread (k, beta) = plane k of vector beta.
 // IDENT (periodic meshes): Z += alpha A W + idw W in the same pass.  The identity part is added cell by cell with
 // partition-of-unity weights (a node on a cell face in a direction is shared by two cells: weight 1/2 per
 // direction) in P4, on the nodal result, from the nodal values of W re-read through L2 (the tile that held them was
@@ -175,10 +166,10 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
 // EIG: the operator of the paper's eigenproblem on a uniform box, H~ = M^-1/2 (K + M^kappa) M^-1/2:
 // kappa is read per quadrature point (P.kappa [cell][n^3]) and the interpolation passes use the
 // mass-scaled tables MAT_NSS (the constant (1/det J) of M^-1 is folded into the metric constants by the host).
-template <int PDEG, int BV, int NT, int MINB, int IM, bool IDENT, bool EIG = false>
+template <int PDEG, int BV, int NT, int MINB, bool IDENT, bool EIG = false>
 __global__ void __launch_bounds__(NT, MINB)
 fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmZ,
-                    const __grid_constant__ ApplyParams P, const __grid_constant__ InitParams I, int nitems) {
+                    const __grid_constant__ ApplyParams P, int nitems) {
   using TL = DenseTile<PDEG, BV>;
   constexpr int N = PDEG + 1, H = N / 2, HH = H > 0 ? H : 1;
   constexpr int S1 = BV, S2 = N * BV, S3 = N * N * BV;   // element strides along x, y, z
@@ -199,12 +190,6 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   const bool dirichlet = P.dirichlet != 0;
   const int org = dirichlet ? -1 : 0;
   const double g2x = 2.0 * P.ug[0], g2y = 2.0 * P.ug[3], g4y = 4.0 * P.ug[3], g4z = 4.0 * P.ug[5], gm = P.ug[6];
-  constexpr bool init = (IM != 0);
-  constexpr int LOOK = 3;   // the items of layer L initialise chunk L+LOOK; layer L adds into chunks L and L+1
-  const int layer_items = P.ncx * P.ncy * P.nvb;
-  InitAhead<NT, IM> ia(I, P, PDEG, tid, layer_items);
-
-  ia.init_stage(smem_raw + 2 * TL::PITCH + 64);
   if (tid == 0) {
     mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -218,8 +203,6 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + org);
   }
   uint32_t parity = 0;
-  ia.startup(LOOK);
-  if (init && tid == 0) { s_next[1] = 0; s_next[2] = 1 << 30; }   // nothing reserved for the first item
   // Items are handed out dynamically (the first one is blockIdx.x): co-resident blocks do not run at the same
   // speed (the warp arbiter favours one of them), and a static round-robin would leave the slow ones behind.
   while (item < nitems) {
@@ -229,13 +212,10 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
     const bool special = wx || wy || wz;
     const bool dlow = dirichlet && (ex == 0 || ey == 0 || ez == 0);
-    // the next item and (init-ahead) this item's slices of chunk ez+LOOK: both consumed later, latency hidden
-    // (asm volatile: the compiler must not schedule anything that depends on the results up here)
-    unsigned nxt_raw = 0, sl0 = 0;
-    if (tid == 0) {
-      asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
-      if (init) sl0 = ia.grab(ez + LOOK);
-    }
+    // the next item: consumed later, latency hidden (asm volatile: the compiler must not schedule anything that
+    // depends on the result up here)
+    unsigned nxt_raw = 0;
+    if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
     mbar_wait(bar, parity);
     parity ^= 1u;
     if (special) {
@@ -269,9 +249,6 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     __syncthreads();
 
     // P2: z-lines (i1, i2 = k): T = Ns_z A -> A ; R = gm T + 4 gzz (DtD T)/4 -> B
-    // (init-ahead: the zero stores, or the loads of a first batch, are issued here and fly during P2)
-    // (the slices were reserved during the block's PREVIOUS item, so that the atomic's latency is never waited for)
-    if (init) { ia.accept(s_next[2], (unsigned)s_next[1]); ia.batch_begin(); ia.slot_issue(); }
     if (active) {
       double xn[N];   // software pipeline: the next line is in flight while this one is computed
 #pragma unroll
@@ -308,7 +285,6 @@ FE_ZLOOP_PRAGMA
       }
     }
     __syncthreads();
-    ia.slot();
 
     // P3: xy-plane i3 = k: R += Kx T (rows) ; R += Ky T, Ns^T along y (columns) ; Ns^T along x (rows)
     {
@@ -334,7 +310,6 @@ FE_ZLOOP_PRAGMA
           if (N & 1) r[j][H] = fma(g2x, m2, r[j][H]);
         }
       }
-      if (IM == 2) { __syncthreads(); ia.slot(); }   // an extra slot for the staged initialisation (no tile hazard here)
       if (active) {
 #pragma unroll
         for (int i = 0; i < N; ++i) {
@@ -364,7 +339,6 @@ FE_ZLOOP_PRAGMA
     if (tid == 0) {
       const int nxt = (int)(gridDim.x + nxt_raw);
       *s_next = nxt;
-      if (init) { s_next[1] = (int)sl0; s_next[2] = ez + LOOK; ia.prefetch_l2(ez + LOOK, sl0); }
       if (nxt < nitems) {
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
@@ -372,7 +346,6 @@ FE_ZLOOP_PRAGMA
         tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + org);
       }
     }
-    ia.slot();
     // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
     if (active) {
       double xn[N], wn[N];
@@ -419,11 +392,8 @@ FE_ZLOOP_PRAGMA
         for (int j = 0; j < N; ++j) b[j * S3] = x[j];
       }
     }
-    ia.wait_ready(ez + 1);   // the planes this cell adds into are initialised
     fence_async_smem();
     __syncthreads();
-    ia.publish_point();
-    ia.slot();
     if (special) plane_wrap_fixup<PDEG, BV, NT, true>(B, P, tid, ex, ey, ez, v0, wx, wy, wz);
     if (tid == 0) {
       tma_reduce_add_4d(&tmZ, B, v0, ex * PDEG, ey * PDEG, ez * PDEG);
@@ -431,13 +401,6 @@ FE_ZLOOP_PRAGMA
     }
     item = *s_next;   // written before the barrier that ended P4
   }
-  if (init) {   // the slices reserved during the last item
-    __syncthreads();
-    ia.accept(s_next[2], (unsigned)s_next[1]);
-    ia.batch_begin();
-    ia.drain();
-  }
-  ia.finish();
   if (tid == 0) tma_wait_all0();
 }
 

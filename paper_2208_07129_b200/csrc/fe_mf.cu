@@ -1,6 +1,4 @@
 // C-ABI of include/fe_mf.h: context, host-side setup, kernel dispatch.  sm_100a only.
-#include "../../include/fe_mf.h"
-
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
@@ -10,84 +8,28 @@
 #include <string>
 #include <vector>
 
-#include "fe_kernels.cuh"
-#include "fe_kernels_eo.cuh"
-#include "fe_kernels_cart2.cuh"
-#include "fe_kernels_tma.cuh"
-#include "fe_kernels_gen.cuh"
-#include "fe_kernels_plane.cuh"
-#include "fe_kernels_line.cuh"
-#include "fe_kernels_kron.cuh"
-#include "fe_kernels_oi.cuh"
+#include "fe_ctx.h"
 #include "fe_tables.h"
-
-struct fe_mf_ctx {
-  int ncx, ncy, ncz, p, n, bc, geom;
-  int ndx, ndy, ndz;
-  long long ndof, ncells;
-  double sigma;
-  int device;
-  int nsm = 148;
-  int geom_mode;            // 0 uniform, 1 per-cell, 2 per-q-point
-  double ug[7];
-  double* geom_dev = nullptr;
-  long long geom_stride = 7;   // doubles per cell in geom_dev
-  // control words of the persistent kernels, zeroed on the stream before each launch:
-  // [0] item counter, [4 .. 4+ncz) slice_ctr, [4+ncz .. 4+2 ncz) done  (fe_init_ahead.cuh)
-  unsigned* ctrl = nullptr;
-  size_t ctrl_bytes = 0;
-  bool coop = false;           // cooperative launches supported
-  // kappa at the quadrature points and the mass-scaled operator
-  std::vector<double> verts;   // copy of vertices_host (empty: uniform box)
-  double lo[3] = {0, 0, 0}, h[3] = {1, 1, 1};
-  std::vector<double> detq;    // geom_mode 2: det J at the quadrature points [cell][n^3]
-  double* dscale_dev = nullptr;   // diag(M)^-1/2 of the GLL-lumped mass matrix [ndof]
-  std::vector<double> mass_diag;  // diag(M) [ndof] (host copy, filled with dscale_dev)
-  bool mass_scaled = false;
-  double* kappa_dev = nullptr;    // geom_mode 0: kappa at the quadrature points [cell][n^3] (set_kappa, or sigma everywhere
-                                  // once mass scaling is on: the EIG kernels always read it)
-  bool kappa_user = false;
-  // n_q != n_p points per direction (0 = off): tables and per-point geometry of that rule
-  int nq_oi = 0;
-  double *oi_N = nullptr, *oi_D = nullptr, *oi_w = nullptr, *oi_geom = nullptr;
-  long long oi_geom_stride = 0;
-  std::vector<double> oi_detq;   // geom_mode 2: det J at the n_q^3 points [cell][nq^3]
-  double detj0 = 1.0;             // geom_mode 0: det J of every cell
-  int variant = 0;
-  int last_launches = 0;
-  // fe_mf_apply_host workspace
-  double* ws_x = nullptr; double* ws_y = nullptr; size_t ws_elems = 0;
-  cudaStream_t hs[2] = {nullptr, nullptr};
-  std::string err;
-};
 
 static thread_local std::string g_create_err = "";
 
-namespace {
-
+namespace fe_host {
 int fail(fe_mf_ctx* c, int code, const std::string& msg) {
   if (c) c->err = msg; else g_create_err = msg;
   return code;
 }
+}  // namespace fe_host
 
-#define FE_CUDA(c, call)                                                                      \
-  do {                                                                                        \
-    cudaError_t e_ = (call);                                                                  \
-    if (e_ != cudaSuccess)                                                                    \
-      return fail((c), FE_MF_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));       \
-  } while (0)
+using fe_host::fail;
+using fe_host::DeviceGuard;
 
-struct DeviceGuard {
-  int prev = -1; bool ok = false;
-  explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess) ok = true; }
-  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
-};
+namespace {
 
 // Even-odd half tables of the sqrt(w)-rescaled matrices: kind 0 Ns = diag(sqrt w) N,
 // 1 Ns^T, 2 Ds = diag(sqrt w) D~ diag(1/sqrt w), 3 Ds^T.
-void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[6]) {
+void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[fe::MAT_COUNT]) {
   const int n = t.n, h = n / 2, m = n / 2;
-  long double M[8][fe::MAXN * fe::MAXN];
+  long double M[6][fe::MAXN * fe::MAXN];
   for (int q = 0; q < n; ++q)
     for (int i = 0; i < n; ++i) {
       const long double sq = sqrtl(t.wl[q]), si = sqrtl(t.wl[i]);
@@ -120,25 +62,8 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[6])
       for (int q = 0; q < n; ++q) M[5][q * n + i] = M[0][q * n + i] * si;
     }
   }
-  // M[6] = M1 = Ns^T Ns (1D mass matrix, = N^T W N) and M[7] = K1 = (Ds Ns)^T (Ds Ns) (1D stiffness matrix, = D^T W D),
-  // both with the n_q-point rule: the Kronecker factors of the cell matrix of a uniform box (fe_kernels_kron.cuh)
-  {
-    long double DN[fe::MAXN * fe::MAXN];
-    for (int q = 0; q < n; ++q)
-      for (int i = 0; i < n; ++i) {
-        long double acc = 0.0L;
-        for (int r = 0; r < n; ++r) acc += M[2][q * n + r] * M[0][r * n + i];
-        DN[q * n + i] = acc;
-      }
-    for (int i = 0; i < n; ++i)
-      for (int j = 0; j < n; ++j) {
-        long double am = 0.0L, ak = 0.0L;
-        for (int q = 0; q < n; ++q) { am += M[0][q * n + i] * M[0][q * n + j]; ak += DN[q * n + i] * DN[q * n + j]; }
-        M[6][i * n + j] = am; M[7][i * n + j] = ak;
-      }
-  }
-  fe::EoTab tabs[8];
-  for (int k = 0; k < 8; ++k) {
+  fe::EoTab tabs[6];
+  for (int k = 0; k < 6; ++k) {
     std::memset(&tabs[k], 0, sizeof(fe::EoTab));
     for (int q = 0; q < h; ++q) {
       for (int i = 0; i < h; ++i) {
@@ -155,8 +80,8 @@ void make_eo_tables(const fe::Tables1D& t, fe::EoTab out[5], fe::EoTab2 out2[6])
   for (int k = 0; k < 5; ++k) out[k] = tabs[k];
   // the plane / line kernels' tables: Ns, Ds (the transposes reuse them) and Ds^T Ds / 2, plus the halved middle
   // column / row
-  const int src[6] = {0, 2, 4, 5, 6, 7};
-  for (int k2 = 0; k2 < 6; ++k2) {
+  const int src[fe::MAT_COUNT] = {0, 2, 4, 5};   // MAT_NS, MAT_DS, MAT_SH, MAT_NSS
+  for (int k2 = 0; k2 < fe::MAT_COUNT; ++k2) {
     const fe::EoTab& s = tabs[src[k2]];
     fe::EoTab2& d = out2[k2];
     std::memset(&d, 0, sizeof(fe::EoTab2));
@@ -221,15 +146,21 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   const fe::Tables1D tab = fe::make_tables(p);
   const int n = p + 1, nn = n * n * n;
   cudaError_t e;
-  e = cudaMemcpyToSymbol(fe::c_N, tab.N, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
-  if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_D, tab.Dt, sizeof(double) * n * n, sizeof(double) * fe::KMAXN * fe::KMAXN * p);
-  if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_w, tab.w, sizeof(double) * n, sizeof(double) * fe::KMAXN * p);
-  if (e == cudaSuccess) {
-    fe::EoTab eo[5];
-    fe::EoTab2 eo2[6];
-    make_eo_tables(tab, eo, eo2);
-    e = cudaMemcpyToSymbol(fe::c_eo, eo, sizeof(eo), sizeof(fe::EoTab) * 5 * p);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(fe::c_eo2, eo2, sizeof(eo2), sizeof(fe::EoTab2) * 6 * p);
+  {
+    // the tables are functions of p only: every context of degree p uploads the same values into slot p of the
+    // constant-memory arrays of each kernel translation unit (of the current device)
+    fe::HostTables ht;
+    std::memset(&ht, 0, sizeof(ht));
+    ht.p = p;
+    std::memcpy(ht.N, tab.N, sizeof(double) * n * n);
+    std::memcpy(ht.D, tab.Dt, sizeof(double) * n * n);
+    std::memcpy(ht.w, tab.w, sizeof(double) * n);
+    make_eo_tables(tab, ht.eo, ht.eo2);
+    e = fe_host::upload_tables_misc(ht);
+    if (e == cudaSuccess) e = fe_host::upload_tables_gen(ht);
+    if (e == cudaSuccess) e = fe_host::upload_tables_plane(ht);
+    if (e == cudaSuccess) e = fe_host::upload_tables_line16(ht);
+    if (e == cudaSuccess) e = fe_host::upload_tables_line8(ht);
   }
   if (e != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
 
@@ -296,9 +227,10 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
     e = cudaMemcpy(c->geom_dev, G.data(), G.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(c->geom_dev); delete c; return fail(nullptr, FE_MF_ECUDA, std::string("geometry upload: ") + cudaGetErrorString(e)); }
   }
-  c->coop = prop.cooperativeLaunch != 0;
-  c->ctrl_bytes = sizeof(unsigned) * (4 + 2 * (size_t)ncz);
-  if (cudaMalloc(&c->ctrl, c->ctrl_bytes) != cudaSuccess) { delete c; return fail(nullptr, FE_MF_ENOMEM, "cudaMalloc (control words) failed"); }
+  if (cudaMalloc(&c->ctrl, sizeof(unsigned) * fe_mf_ctx::kCtrlSlots * fe_mf_ctx::kCtrlWords) != cudaSuccess) {
+    cudaFree(c->geom_dev); delete c;
+    return fail(nullptr, FE_MF_ENOMEM, "cudaMalloc (control words) failed");
+  }
   *out = c;
   return FE_MF_OK;
 }
@@ -326,6 +258,7 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
   if (ctx->ws_x) cudaFree(ctx->ws_x);
   if (ctx->ws_y) cudaFree(ctx->ws_y);
   for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
+  for (int i = 0; i < 2; ++i) if (ctx->hev[i]) cudaEventDestroy(ctx->hev[i]);
   delete ctx;
 }
 
@@ -344,7 +277,6 @@ extern "C" int fe_mf_set_kappa(fe_mf_ctx* ctx, const double* kappa_host) {
     ctx->kappa_user = kappa_host != nullptr;
     if (!kappa_host && !ctx->mass_scaled) {
       if (ctx->kappa_dev) cudaFree(ctx->kappa_dev);
-  { double* b[] = {ctx->oi_N, ctx->oi_D, ctx->oi_w, ctx->oi_geom}; for (double* q : b) if (q) cudaFree(q); }
       ctx->kappa_dev = nullptr;
       return FE_MF_OK;
     }
@@ -371,6 +303,7 @@ extern "C" int fe_mf_set_kappa(fe_mf_ctx* ctx, const double* kappa_host) {
   const size_t gstride = (size_t)(ctx->nq_oi ? ctx->oi_geom_stride : ctx->geom_stride);
   FE_CUDA(ctx, cudaMemcpy2D(gdst + 6 * nn, gstride * sizeof(double), g.data(), nn * sizeof(double),
                             nn * sizeof(double), (size_t)ctx->ncells, cudaMemcpyHostToDevice));
+  ctx->kappa_user = kappa_host != nullptr;
   return FE_MF_OK;
 }
 
@@ -382,18 +315,20 @@ extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
   DeviceGuard guard(ctx->device);
   if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
   FE_CUDA(ctx, cudaDeviceSynchronize());
-  { double** b[] = {&ctx->oi_N, &ctx->oi_D, &ctx->oi_w, &ctx->oi_geom}; for (double** q : b) if (*q) { cudaFree(*q); *q = nullptr; } }
-  ctx->oi_detq.clear();
-  const bool had_kappa = ctx->kappa_user;
-  ctx->nq_oi = (nq == ctx->n) ? 0 : nq;
-  // a kappa array belongs to the points of one rule: back to the constant sigma
-  if (ctx->geom_mode == 0) {
-    ctx->kappa_user = false;
-    if (ctx->kappa_dev) { cudaFree(ctx->kappa_dev); ctx->kappa_dev = nullptr; }
-    if (ctx->mass_scaled && !ctx->nq_oi) { const int rc = fe_mf_set_kappa(ctx, nullptr); if (rc != FE_MF_OK) return rc; }
-  } else if (ctx->geom_mode == 2 && !ctx->nq_oi && had_kappa) {
+  // A kappa array belongs to the points of one rule: back to the constant sigma.  On a per-q-point context the
+  // caller's kappa sits inside the default rule's factors (slot 6 of geom_dev): rewrite them BEFORE the rule changes,
+  // otherwise the old kappa would silently come back with nq = p + 1.
+  if (ctx->geom_mode == 2 && ctx->kappa_user && !ctx->nq_oi) {
     const int rc = fe_mf_set_kappa(ctx, nullptr);
     if (rc != FE_MF_OK) return rc;
+  }
+  { double** b[] = {&ctx->oi_N, &ctx->oi_D, &ctx->oi_w, &ctx->oi_geom}; for (double** q : b) if (*q) { cudaFree(*q); *q = nullptr; } }
+  ctx->oi_detq.clear();
+  ctx->nq_oi = (nq == ctx->n) ? 0 : nq;
+  ctx->kappa_user = false;
+  if (ctx->geom_mode == 0) {
+    if (ctx->kappa_dev) { cudaFree(ctx->kappa_dev); ctx->kappa_dev = nullptr; }
+    if (ctx->mass_scaled && !ctx->nq_oi) { const int rc = fe_mf_set_kappa(ctx, nullptr); if (rc != FE_MF_OK) return rc; }
   }
   if (!ctx->nq_oi) return FE_MF_OK;
   const int n = ctx->n;
@@ -442,7 +377,7 @@ extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
     };
     halves(hN, nq, n, 1.0);
     halves(hD, nq, nq, -1.0);
-    FE_CUDA(ctx, cudaMemcpyToSymbol(fe::c_oi, pack.data(), pack.size() * sizeof(double), sizeof(double) * fe::oi_offset(ctx->p)));
+    FE_CUDA(ctx, fe_host::upload_tables_oi(pack.data(), pack.size(), (size_t)fe::oi_offset(ctx->p)));
   }
   if (ctx->geom_mode == 2) {   // per-point metric at the nq^3 points (Eq. 7c evaluated at every point of the rule)
     const size_t nn = (size_t)nq * nq * nq;
@@ -554,4 +489,3 @@ extern "C" int fe_mf_mass_diagonal(fe_mf_ctx* ctx, double* out_host) {
   return FE_MF_OK;
 }
 
-#include "fe_dispatch.inl"

@@ -1,0 +1,90 @@
+// Plain structs shared by the host code and every kernel translation unit: kernel parameters, the layouts of the
+// constant-memory tables and the host image of one degree's tables.  No CUDA code.
+#pragma once
+#include <cstddef>
+
+namespace fe {
+
+constexpr int KMAXN = 9;   // p <= 8
+
+struct ApplyParams {
+  const double* __restrict__ W;   // input multivector  [ndof][nvec]
+  double* __restrict__ Z;         // output multivector [ndof][nvec], pre-initialised; Z += alpha*A*W
+  const double* __restrict__ geom;  // per-q-point: [cell][7][n^3]; per-cell: [cell][7]; or nullptr (uniform); no w_Q factor
+  double ug[7];                   // uniform Cartesian: G00,G01,G02,G11,G12,G22 (x det J), sigma*det J
+  double alpha;
+  int ncx, ncy, ncz;
+  int ndx, ndy, ndz;
+  int nvec;
+  int bv;                         // vectors per block
+  int nvb;                        // ceil(nvec / bv)
+  int dirichlet;                  // 1: boundary nodes read as 0 / not written
+  int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
+  int nsm;                        // SM count (persistent kernels)
+  long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
+  int* item_ctr;                  // persistent kernels: work counter (0 at launch); item = gridDim.x + atomicAdd after the first
+  double idw;                     // Cartesian kernels with IDENT: Z += alpha A W + idw W
+  const double* dscale;           // nullptr, or d = diag(M)^-1/2 [ndof] of the GLL-lumped mass matrix: Z += alpha d.(A (d.W))
+                                  // (Eq. B.1; full-metric kernels only)
+  const double* kappa;            // nullptr, or kappa at the quadrature points [cell][n^3] of a uniform box (geom_mode 0):
+                                  // the mass factor is ug[6] * kappa_Q, ug[6] then holding det J without sigma
+                                  // (general kernel, and the Cartesian kernels instantiated with EIG)
+};
+
+// n_q != n_p Gauss points per direction
+struct OiParams {
+  int nq;                     // Gauss points per direction
+  const double* Nq;           // [nq][n]   N[q][i] = l_i(xq_q)
+  const double* Dq;           // [nq][nq]  D~[q][r] = l~_r'(xq_q)
+  const double* wq;           // [nq]
+  const double* geom;         // geom_mode 2: [cell][7][nq^3] (no w factor), else unused
+  long long geom_stride;
+};
+
+// Half tables of one n x n matrix M with M[n-1-q][n-1-i] = s M[q][i] (s = +1 "sym", -1 "anti"); h = n/2.
+//   P[q][i]  = (M[q][i] + M[q][n-1-i])/2   multiplies x+_i = x_i + x_{n-1-i}
+//   Mn[q][i] = (M[q][i] - M[q][n-1-i])/2   multiplies x-_i = x_i - x_{n-1-i}
+//   Pm[q]    = M[q][m]                      multiplies the middle entry (n odd)
+//   mid[i]   = M[m][i] (i < h), midm = M[m][m]: the middle row (n odd)
+// y_q = u + v, y_{n-1-q} = s (u - v) with u = P x+ + Pm x_m, v = Mn x-.
+struct EoTab {
+  double P[16];
+  double Mn[16];
+  double Pm[4];
+  double mid[4];
+  double midm;
+  double pad[3];
+};
+enum { EO_NS = 0, EO_NST = 1, EO_DS = 2, EO_DST = 3, EO_SH = 4 };   // EO_SH: Ds^T Ds / 2 (symmetric type)
+
+// The same with the halved middle column / row that the chained even/odd operators need (fe_kernels_plane.cuh)
+struct EoTab2 {
+  double P[16], Mn[16];
+  double Pm[4], mid[4];
+  double Pmh[4], midh[4];   // Pm / 2, mid / 2
+  double midm, midmh;       // M[mid][mid] and half of it
+  double pad[2];
+};
+enum { MAT_NS = 0, MAT_DS = 1, MAT_SH = 2, MAT_NSS = 3, MAT_COUNT = 4 };   // Ns, Ds, Ds^T Ds / 2 (symmetric type, like Ns),
+                                                                           // Ns diag(w~)^-1/2 (mass-scaled interpolation, EIG)
+
+// Host image of the tables of one degree p, uploaded into the constant memory of every kernel translation unit
+// (each unit owns a private copy of the symbols it uses: the library is built without relocatable device code)
+struct HostTables {
+  int p;
+  double N[KMAXN * KMAXN], D[KMAXN * KMAXN], w[KMAXN];
+  EoTab eo[5];
+  EoTab2 eo2[MAT_COUNT];
+};
+
+// Tables of the n_q = n_p + 2 rule, packed per degree at oi_offset(p) as even / odd halves: [Ne | No | De | Do]
+constexpr int oi_size(int p) { return 2 * ((p + 4) / 2) * ((p + 2) / 2) + 2 * ((p + 4) / 2) * ((p + 4) / 2); }
+template <int P_> struct OiOffset { static constexpr int value = OiOffset<P_ - 1>::value + oi_size(P_ - 1); };
+template <> struct OiOffset<1> { static constexpr int value = 0; };
+inline int oi_offset(int p) {
+  int off = 0;
+  for (int k = 1; k < p; ++k) off += oi_size(k);
+  return off;
+}
+
+}  // namespace fe

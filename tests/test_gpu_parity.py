@@ -298,11 +298,11 @@ def test_unit_cube_config5_interval_is_rejected(env):
         op.cheb_filter(X, Y, 1, 20, 2.0, 0.3, 0.0)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 8, 10, 11, 12, 19])
+@pytest.mark.parametrize("variant", [1, 2, 8, 10, 11])
 @pytest.mark.parametrize("p,bc", [(6, inputs.BC_DIRICHLET), (7, inputs.BC_PERIODIC), (8, inputs.BC_PERIODIC), (4, inputs.BC_PERIODIC)])
 def test_kernel_variants(env, variant, p, bc):
     """variant 1 = general fallback kernel, 2 = even-odd Cartesian kernel with one vector per thread (LDG/RED),
-    8 = plane kernel, 10 / 11 = line kernel with 16 / 8 vectors per block, 19 = plane kernel that also initialises Y."""
+    8 = plane kernel (p = 6 only; other degrees keep their default), 10 / 11 = line kernel with 16 / 8 vectors per block."""
     torch, orc, binding = env
     w = inputs.Workload(f"var_p{p}", p, (3, 2, 3), bc, inputs.GEOM_AFFINE, 0.8, (0.0, 0.0, 0.0), (1.5, 1.0, 2.0), 20, 500 + p)
     X = inputs.multivector(w.seed, w.ndof, w.nvec)
@@ -314,26 +314,24 @@ def test_kernel_variants(env, variant, p, bc):
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
 
 
-@pytest.mark.parametrize("variant", [0, 19])
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
-def test_plane_kernel_many_layers(env, bc, variant):
-    """p = 6, 9 cell layers in z (more than the init-ahead look-ahead), 40 vectors (a partial last block): plain apply
-    and Z <- beta Z + gamma W + alpha A W, with the initialisation as a separate pass (0) or folded into the
-    kernel (19: dynamic slices, cooperative launch)."""
+def test_plane_kernel_many_layers(env, bc):
+    """p = 6, 9 cell layers in z, 40 vectors (a partial last block): plain apply and Z <- beta Z + gamma W + alpha A W."""
     torch, orc, binding = env
     w = inputs.Workload("plane_layers", 6, (2, 3, 9), bc, inputs.GEOM_AFFINE, 0.7, (0.0, 0.0, 0.0), (1.0, 1.5, 3.0), 40, 4242)
     X = inputs.multivector(w.seed, w.ndof, w.nvec)
     Z0 = inputs.multivector(w.seed + 1, w.ndof, w.nvec)
     Yo = orc.Operator(oracle_mesh(orc, w), w.sigma).apply(X)
-    op = binding.FeMf.from_workload(w); op.set_variant(variant)
+    op = binding.FeMf.from_workload(w)
+    assert op.kernel_name(w.nvec) == "fe_apply_cart_plane"
     Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
     op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
-    assert op.last_launch_count() == 1                      # the zero fill of variant 0 is a driver memset
+    assert op.last_launch_count() == 1                      # the zero fill is a driver memset
     Zd = torch.from_numpy(Z0).cuda()
     op.apply_axpby(0.3, Xd, 0.5, -0.25, Zd, w.nvec); torch.cuda.synchronize()
     assert relerr(Zd.cpu().numpy(), 0.5 * Z0 - 0.25 * X + 0.3 * Yo) <= TOL
-    assert op.last_launch_count() == (1 if variant == 19 else 2)
+    assert op.last_launch_count() == 2
     Zd = torch.from_numpy(Z0).cuda()
     op.apply_axpby(0.3, Xd, 0.0, -0.25, Zd, w.nvec); torch.cuda.synchronize()
     assert relerr(Zd.cpu().numpy(), -0.25 * X + 0.3 * Yo) <= TOL
@@ -360,33 +358,3 @@ def test_general_metric_kernel_on_uniform_mesh(env, p):
     Xd = torch.from_numpy(X).cuda(); Yd = torch.empty_like(Xd)
     op.apply_axpby(0.5, Xd, 0.0, 0.0, Yd, w.nvec); torch.cuda.synchronize()
     assert relerr(Yd.cpu().numpy(), 0.5 * Yo) <= TOL
-
-
-@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
-@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6, 7, 8])
-def test_kronecker_kernel(env, p, bc):
-    """fe_apply_cart_kron (uniform box, constant kappa: the cell matrix as a sum of Kronecker products of the 1D mass and
-    stiffness matrices): apply, Eq. B.1 and the one-launch Chebyshev step, anisotropic cells, a partial vector block,
-    wrap / boundary cells in every direction, several items per block."""
-    torch, orc, binding = env
-    nc = (3, 4, 5) if p <= 3 else ((2, 3, 4) if p <= 6 else (2, 3, 2))
-    w = inputs.Workload(f"kron_p{p}", p, nc, bc, inputs.GEOM_AFFINE, 0.8, (0.0, -1.0, 2.0), (1.5, 0.5, 4.4), 20, 900 + p)
-    X = inputs.multivector(w.seed, w.ndof, w.nvec)
-    Z0 = inputs.multivector(w.seed + 1, w.ndof, w.nvec)
-    op_o = orc.Operator(oracle_mesh(orc, w), w.sigma)
-    Yo = op_o.apply(X)
-    op = binding.FeMf.from_workload(w)
-    op.set_variant(12)
-    assert op.kernel_name(w.nvec) == "fe_apply_cart_kron"
-    Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
-    op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
-    assert relerr(Yd.cpu().numpy(), Yo) <= TOL
-    Zd = torch.from_numpy(Z0).cuda()
-    op.apply_axpby(0.3, Xd, 0.5, -0.25, Zd, w.nvec); torch.cuda.synchronize()
-    assert relerr(Zd.cpu().numpy(), 0.5 * Z0 - 0.25 * X + 0.3 * Yo) <= TOL
-    m, a, b, a0 = 6, 1.5, 40.0, -0.2
-    Fo = orc.chebyshev_filter(op_o.apply, X, m, a, b, a0)
-    Fd = torch.full_like(Xd, float("nan"))
-    op.cheb_filter(Xd, Fd, w.nvec, m, a, b, a0); torch.cuda.synchronize()
-    assert relerr(Fd.cpu().numpy(), Fo) <= TOL
-    assert op.last_launch_count() <= m + 1
