@@ -28,7 +28,7 @@ UNITS = {
     "fe_dispatch.cu": HOST_DEPS,
     "fe_probe.cu": [FE_MF_H],
     "fe_tu_misc.cu": KERNEL_DEPS + ["fe_kernels_stream.cuh"],
-    "fe_tu_gen.cu": KERNEL_DEPS + ["fe_kernels_gen.cuh", "fe_kernels_plane.cuh", "fe_kernels_grp.cuh"],
+    "fe_tu_gen.cu": KERNEL_DEPS + ["fe_kernels_gen.cuh"],
     "fe_tu_plane.cu": KERNEL_DEPS + ["fe_kernels_plane.cuh"],
     "fe_tu_line16.cu": KERNEL_DEPS + ["fe_kernels_plane.cuh", "fe_kernels_line.cuh", "fe_line_launch.inl"],
     "fe_tu_line8.cu": KERNEL_DEPS + ["fe_kernels_plane.cuh", "fe_kernels_line.cuh", "fe_line_launch.inl"],

@@ -18,7 +18,6 @@ template <> struct GenCfg<6> { static constexpr int BV = 8, NT = 128, MINB = 3; 
 template <> struct GenCfg<7> { static constexpr int BV = 8, NT = 256, MINB = 1; };
 template <> struct GenCfg<8> { static constexpr int BV = 4, NT = 192, MINB = 2; };
 
-int gen_bv(const fe_mf_ctx* c, int) { return c->p == 8 ? 4 : 8; }
 
 template <int PDEG, bool MSC>
 static cudaError_t launch_gen_p(fe_mf_ctx* c, const fe::ApplyParams& prm, const CUtensorMap& tw, const CUtensorMap& tz,
@@ -35,6 +34,8 @@ static cudaError_t launch_gen_p(fe_mf_ctx* c, const fe::ApplyParams& prm, const 
   kern<<<(unsigned)grid, C::NT, SMEM, st>>>(tw, tz, prm, (int)nitems);
   return cudaGetLastError();
 }
+
+int gen_bv(const fe_mf_ctx* c, int) { return c->p == 8 ? 4 : 8; }
 
 cudaError_t launch_gen(fe_mf_ctx* c, const fe::ApplyParams& P, const CUtensorMap& tw, const CUtensorMap& tz, cudaStream_t st) {
   cudaError_t e = cudaErrorInvalidValue;

@@ -314,16 +314,18 @@ def test_kernel_variants(env, variant, p, bc):
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
 
 
+@pytest.mark.parametrize("variant", [0, 8])
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
-def test_plane_kernel_many_layers(env, bc):
-    """p = 6, 9 cell layers in z, 40 vectors (a partial last block): plain apply and Z <- beta Z + gamma W + alpha A W."""
+def test_plane_kernel_many_layers(env, bc, variant):
+    """p = 6, 9 cell layers in z, 40 vectors (a partial last block of 8: the default is then the line kernel, variant 8
+    forces the plane kernel): plain apply and Z <- beta Z + gamma W + alpha A W."""
     torch, orc, binding = env
     w = inputs.Workload("plane_layers", 6, (2, 3, 9), bc, inputs.GEOM_AFFINE, 0.7, (0.0, 0.0, 0.0), (1.0, 1.5, 3.0), 40, 4242)
     X = inputs.multivector(w.seed, w.ndof, w.nvec)
     Z0 = inputs.multivector(w.seed + 1, w.ndof, w.nvec)
     Yo = orc.Operator(oracle_mesh(orc, w), w.sigma).apply(X)
-    op = binding.FeMf.from_workload(w)
-    assert op.kernel_name(w.nvec) == "fe_apply_cart_plane"
+    op = binding.FeMf.from_workload(w); op.set_variant(variant)
+    assert op.kernel_name(w.nvec) == ("fe_apply_cart_plane" if variant == 8 else "fe_apply_cart_line")
     Xd = torch.from_numpy(X).cuda(); Yd = torch.full_like(Xd, float("nan"))
     op.apply(Xd, Yd, w.nvec); torch.cuda.synchronize()
     assert relerr(Yd.cpu().numpy(), Yo) <= TOL
