@@ -149,3 +149,102 @@ def test_cfg4_full_eigen_operator(env):
 def test_cfg3_full_eigen_operator(env):
     w = inputs.configs()[3]
     assert run_full_eigen_operator(env, w, w.nvec, nsamples=10) == "fe_apply_gen_tma"
+
+
+# ---------------------------------------------------------------- element-by-element at full size
+# A persistent kernel with a dynamic work counter can fail LOCALLY (an item skipped or done twice) where a handful of
+# sampled nodes will not look: the cases below compare EVERY row of the full-size result.  Two oracles: the cell-matrix
+# oracle (fe_oracle.Operator.apply) and, on the uniform Cartesian configs, the exactly integrated Kronecker closed form
+# (kron_oracle.kronecker_apply), which shares nothing with the first.
+def full_compare(Yg, Yo, what):
+    scale = float(np.abs(Yo).max())
+    err = float(np.abs(Yg - Yo).max() / scale)
+    worst_col = max(float(np.abs(Yg[:, j] - Yo[:, j]).max() / np.abs(Yo[:, j]).max()) for j in range(Yo.shape[1]))
+    assert err <= TOL, (what, err, worst_col)
+    return err
+
+
+@pytest.mark.parametrize("nvec", [1, 8])
+def test_cfg4_full_every_row_two_oracles(env, nvec):
+    """Config 4 (p = 7, 32^3 periodic cells, 11.2 M DoFs) at nvec 1 (cells-as-slots kernel) and 8 (line kernel)."""
+    torch, orc, binding = env
+    from oracle import kron_oracle as kro
+    w = inputs.configs()[4]
+    op = binding.FeMf.from_workload(w)
+    X = torch.empty(w.ndof * nvec, dtype=torch.float64, device="cuda")
+    Y = torch.full_like(X, float("nan"))
+    binding.fill_uniform(X, w.seed)
+    op.apply(X, Y, nvec); torch.cuda.synchronize()
+    Xh = X.cpu().numpy().reshape(w.ndof, nvec)
+    Yg = Y.cpu().numpy().reshape(w.ndof, nvec)
+    Yk = kro.kronecker_apply(w.ncells, w.p, "periodic", w.box_lo, w.box_hi, w.sigma, Xh)
+    full_compare(Yg, Yk, ("cfg4 kron", nvec, op.kernel_name(nvec)))
+    Yo = oracle_op(orc, w).apply(Xh)
+    full_compare(Yg, Yo, ("cfg4 cell-matrix", nvec, op.kernel_name(nvec)))
+
+
+def test_cfg3_full_every_row_four_columns(env):
+    """Config 3 (p = 8, perturbed mesh, per-q-point metric): the GPU applies all 16 columns, the cell-matrix oracle the
+    first, two middle and last column on the full mesh; every row of those columns is compared."""
+    torch, orc, binding = env
+    w = inputs.configs()[3]
+    nvec = w.nvec
+    op = binding.FeMf.from_workload(w)
+    X = torch.empty(w.ndof * nvec, dtype=torch.float64, device="cuda")
+    Y = torch.full_like(X, float("nan"))
+    binding.fill_uniform(X, w.seed)
+    op.apply(X, Y, nvec); torch.cuda.synchronize()
+    cols = [0, 5, 10, 15]
+    Xc = np.ascontiguousarray(X.view(w.ndof, nvec)[:, cols].cpu().numpy())
+    Yg = Y.view(w.ndof, nvec)[:, cols].cpu().numpy()
+    assert np.isfinite(Y.cpu().numpy()).all()
+    Yo = oracle_op(orc, w).apply(Xc)
+    full_compare(Yg, Yo, ("cfg3", op.kernel_name(nvec)))
+
+
+def test_cfg5_full_apply_every_row_eight_columns(env):
+    """Config 5's mesh and block (p = 6, 16^3 periodic cells on [0,10]^3, 1024 vectors = 64 vector blocks of the plane
+    kernel): a single apply of the whole block, 8 columns spread over the vector blocks compared on every row."""
+    torch, orc, binding = env
+    from oracle import kron_oracle as kro
+    w = inputs.configs()[5]
+    nvec = w.nvec
+    op = binding.FeMf.from_workload(w)
+    X = torch.empty(w.ndof * nvec, dtype=torch.float64, device="cuda")
+    Y = torch.full_like(X, float("nan"))
+    binding.fill_uniform(X, w.seed)
+    op.apply(X, Y, nvec); torch.cuda.synchronize()
+    assert op.kernel_name(nvec) == "fe_apply_cart_plane"
+    cols = [0, 15, 16, 300, 517, 800, 1008, 1023]
+    Xc = np.ascontiguousarray(X.view(w.ndof, nvec)[:, cols].cpu().numpy())
+    Yg = Y.view(w.ndof, nvec)[:, cols].cpu().numpy()
+    Yk = kro.kronecker_apply(w.ncells, w.p, "periodic", w.box_lo, w.box_hi, w.sigma, Xc)
+    full_compare(Yg, Yk, "cfg5 kron")
+    Yo = oracle_op(orc, w).apply(Xc)
+    full_compare(Yg, Yo, "cfg5 cell-matrix")
+    # the other 1016 columns: finite, and the column sums of K X vanish on a periodic mesh (K 1 = 0), i.e.
+    # 1^T (A X) = sigma 1^T M X = sigma * (cell volume weights) -- checked against the Kronecker row sums
+    (Mx, _), (My, _), (Mz, _) = kro.matrices_1d(w.ncells, w.p, "periodic", w.box_lo, w.box_hi)
+    wgt = np.einsum("k,j,i->kji", Mz.sum(0), My.sum(0), Mx.sum(0)).reshape(-1)
+    lhs = Y.view(w.ndof, nvec).sum(0).cpu().numpy()
+    rhs = w.sigma * (torch.from_numpy(wgt).cuda()[:, None] * X.view(w.ndof, nvec)).sum(0).cpu().numpy()
+    assert np.isfinite(lhs).all()
+    assert np.abs(lhs - rhs).max() <= 1e-9 * max(np.abs(rhs).max(), 1.0)
+
+
+def test_cfg2_full_every_row_kronecker(env):
+    """Config 2 (the bench workload, Dirichlet): all 32 columns, every row, against the Kronecker closed form (the
+    cell-matrix oracle is compared on the full block inside bench.py's cpu_baseline leg)."""
+    torch, orc, binding = env
+    from oracle import kron_oracle as kro
+    w = inputs.configs()[2]
+    nvec = w.nvec
+    op = binding.FeMf.from_workload(w)
+    X = torch.empty(w.ndof * nvec, dtype=torch.float64, device="cuda")
+    Y = torch.full_like(X, float("nan"))
+    binding.fill_uniform(X, w.seed)
+    op.apply(X, Y, nvec); torch.cuda.synchronize()
+    Xh = X.cpu().numpy().reshape(w.ndof, nvec)
+    Yg = Y.cpu().numpy().reshape(w.ndof, nvec)
+    Yk = kro.kronecker_apply(w.ncells, w.p, "dirichlet", w.box_lo, w.box_hi, w.sigma, Xh)
+    full_compare(Yg, Yk, "cfg2 kron")
