@@ -190,22 +190,26 @@ def run_ours(args):
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
+    # EXACTLY args.steps steps between two events on the launching stream; one more event after every step gives the
+    # per-step distribution (median / min) without touching the timed region's length
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record(stream)
+    for i in range(args.steps):
         op.apply(X, Y, nvec)
-    e1.record(stream)
+        ev[i + 1].record(stream)
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = ev[0].elapsed_time(ev[-1])
+    step_ms = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps))
     # the dominant kernel alone (same launch configuration), events on the launching stream
-    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    k0.record(stream)
-    for _ in range(args.steps):
+    kv = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    kv[0].record(stream)
+    for i in range(args.steps):
         op.accumulate(1.0, X, Y, nvec)
-    k1.record(stream)
+        kv[i + 1].record(stream)
     torch.cuda.synchronize()
     clocks = sampler.stop()
-    ms_kernel = k0.elapsed_time(k1) / args.steps
+    ms_kernel = kv[0].elapsed_time(kv[-1]) / args.steps
+    kern_ms = sorted(kv[i].elapsed_time(kv[i + 1]) for i in range(args.steps))
     ms_total = sharding.max_over_ranks(ms_total, dist, "cuda")
     ms_step = ms_total / args.steps
     value = sharding.aggregate_throughput(count, world, ms_step * 1e-3) / 1e9
@@ -359,12 +363,56 @@ def run_ours(args):
                 ev[1].record(stream)
                 torch.cuda.synchronize()
                 t_kern = ev[0].elapsed_time(ev[1]) / 5
+                # the operator is the full-metric one on every mesh here (the over-integration kernel has no Cartesian
+                # special case): roofline with the rectangular even-odd count of roofline.work_per_dof_vec_oi
+                so_oi, _ = roofline.work_per_dof_vec_oi(wo.p, wo.p + 3, False)
                 others.append({"workload": wo.name + " with n_q = n_p + 2", "p": wo.p, "nvec": nv_o,
-                               "kernel": opo.kernel_name(nv_o), "kernel_only": no / (t_kern * 1e-3) / 1e9, "kernel_ms": t_kern})
+                               "kernel": opo.kernel_name(nv_o), "kernel_only": no / (t_kern * 1e-3) / 1e9, "kernel_ms": t_kern,
+                               "fp64_instr_per_dof_vec": so_oi,
+                               "frac": no * so_oi * 2.0 / (t_kern * 1e-3) / 1e12 / fp64_peak})
                 del Xo, Yo_, opo
                 torch.cuda.empty_cache()
             except Exception as exc:
                 others.append({"workload": "cfg%d with n_q = n_p + 2" % cfg_o, "error": str(exc)[:200]})
+
+    # ---- config 1 (p = 4, 8^3 cells, 8 vectors: 1.7 us of work, launch-bound): SURVEY.md 8(d) asks for it inside a CUDA
+    #      graph of >= 100 back-to-back applies
+    small = None
+    if rank == 0 and world == 1 and not args.no_others and args.config == 2:
+        try:
+            w1 = inputs.configs()[1]
+            op1 = binding.FeMf.from_workload(w1, device=local)
+            n1 = w1.ndof * w1.nvec
+            X1 = torch.empty(n1, dtype=torch.float64, device="cuda"); Y1 = torch.empty_like(X1)
+            binding.fill_uniform(X1, w1.seed)
+            gs = torch.cuda.Stream()
+            with torch.cuda.stream(gs):
+                op1.apply(X1, Y1, w1.nvec, stream=gs)
+                gs.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=gs):
+                    for _ in range(100):
+                        op1.apply(X1, Y1, w1.nvec, stream=gs)
+                g.replay(); gs.synchronize()
+                tg = []
+                for _ in range(5):
+                    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    g0.record(gs); g.replay(); g1.record(gs); gs.synchronize()
+                    tg.append(g0.elapsed_time(g1) / 100)
+                # the same 100 applies launched one by one
+                l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                l0.record(gs)
+                for _ in range(100):
+                    op1.apply(X1, Y1, w1.nvec, stream=gs)
+                l1.record(gs); gs.synchronize()
+            s1, _ = roofline.work_per_dof_vec(w1.p, True)
+            small = {"workload": w1.name, "nvec": w1.nvec, "kernel": op1.kernel_name(w1.nvec),
+                     "us_per_apply_in_graph_of_100": min(tg) * 1e3, "us_per_apply_launched": l0.elapsed_time(l1) * 10.0,
+                     "value_in_graph": n1 / (min(tg) * 1e-3) / 1e9,
+                     "frac_in_graph": n1 * s1 * 2.0 / (min(tg) * 1e-3) / 1e12 / fp64_peak}
+            del X1, Y1, op1, g
+        except Exception as exc:
+            small = {"error": str(exc)[:200]}
 
     # ---- roofline of the dominant kernel
     diag = (w.geom == inputs.GEOM_AFFINE)
@@ -387,12 +435,24 @@ def run_ours(args):
             traffic = json.load(open(tfile)).get(f"cfg{args.config}_nvec{nvec}_variant{args.variant}")
         except Exception:
             traffic = None
+    sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965
+    nsm = torch.cuda.get_device_properties(local).multi_processor_count
+    counters = None   # executed FP64 instructions per DoF*vec of this kernel, from the committed ncu capture
+    cfile = os.path.join(ROOT, "profiles", "counters.json")
+    if os.path.exists(cfile):
+        try:
+            counters = json.load(open(cfile)).get(f"cfg{args.config}_nvec{nvec}_variant{args.variant}")
+        except Exception:
+            counters = None
     roof = {"bound": "alu", "achieved": achieved_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved_tf / fp64_peak,
             "traffic": traffic, "kernel": op.kernel_name(nvec), "kernel_ms": ms_kernel,
-            "peak_source": "fe_probe_peaks: FP64 FMA chain measured live in this run (burst)",
-            "flop_convention": "2 x algorithmic FP64 instructions of the plain even-odd method (%.1f instr, %.1f flops per DoF*vec); the kernel may execute fewer (executed_fp64_instr_per_dof_vec, DESIGN.md section 5)" % (slots, flops),
-            "executed_fp64_instr_per_dof_vec": (roofline.executed_instr_per_dof_vec_cartesian(w.p)
-                                                if op.kernel_name(nvec) in ("fe_apply_cart_plane", "fe_apply_cart_line") else None),
+            "kernel_ms_median": kern_ms[len(kern_ms) // 2], "kernel_ms_min": kern_ms[0],
+            "peak_source": "fe_probe_peaks: FP64 FMA chain measured live in this run (burst); MEASURED_PEAKS.json has no FP64 figure",
+            "peak_nominal": nsm * 64 * 2 * sm_mhz * 1e6 / 1e12,
+            "peak_nominal_source": "%d SMs x 64 FP64 FMA/clk x 2 x %d MHz (SM clock sampled during the timed region)" % (nsm, sm_mhz),
+            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full capture committed under profiles/ (profiles/traffic.json)",
+            "executed_fp64": counters,
+            "flop_convention": "2 x algorithmic FP64 instructions of the plain even-odd method (%.1f instr, %.1f flops per DoF*vec); the kernel may execute fewer (executed_fp64: ncu counters, DESIGN.md section 5)" % (slots, flops),
             "t_roof_ms": t_roof * 1e3, "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
             "frac_of_t_roof": t_roof * 1e3 / ms_kernel,
             "hbm": {"achieved": count * roofline.bytes_per_dof_vec(w.p, w.geom == inputs.GEOM_QPOINT, bv) / (ms_kernel * 1e-3) / 1e9,
@@ -425,11 +485,12 @@ def run_ours(args):
 
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-               "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+               "ms_per_step": ms_step, "ms_per_step_median": step_ms[len(step_ms) // 2], "ms_per_step_min": step_ms[0],
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                "data": "synthetic", "config": config_dict(w, nvec, {"bv": bv, "variant": args.variant,
                                                                      "sharding": "vector columns, no collective"}),
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roof,
-               "cpu_baseline": cpu, "chebyshev": cheb, "other_configs": others}
+               "cpu_baseline": cpu, "chebyshev": cheb, "other_configs": others, "config1_cuda_graph": small}
         print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

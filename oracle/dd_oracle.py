@@ -1,0 +1,102 @@
+"""CPU oracle of the domain-decomposed apply -- TEST INFRASTRUCTURE, NOT THE PRODUCT (same rules
+as fe_oracle.py: only tests/, smoke() and bench.py's cpu_baseline legs may import it).
+
+The paper distributes the mesh over tasks t; a task holds its locally-owned DoFs followed by the "ghost" DoFs on the
+shared subdomain boundary that another task owns, and evaluates (Eq. 6 / 16)
+
+    V = sum_t  P^(t)T [ C^(t)T ( sum_{e in E_t} Q^(e,t)T A^(e) Q^(e,t) ) C^(t) ] P^(t) U
+
+P^(t) = the partitioner: extraction of task t's owned + ghost rows (the ghost rows arrive by point-to-point messages,
+PAPER.md:746, Alg. 5 l.1/3/8); P^(t)T = the reverse: ghost rows of V^(t) are sent to their owner and ADDED (Alg. 5
+l.5/10/12).  Here the subdomains are z-SLABS of the structured mesh (the simplest instance: every task has at most
+two neighbours, or itself across the periodic boundary):
+
+    task t owns the cell layers z0_t <= ez < z1_t and the node planes  z0_t p <= iz < z1_t p  (the last task of a
+    Dirichlet mesh also owns the boundary plane ncz p); its one ghost plane is  iz = z1_t p  (owned by task t+1; on a
+    periodic mesh the last task's ghost plane is plane 0 of task 0).  Local row order = plane order: owned planes
+    first, then the ghost plane -- the layout of PAPER.md:748 ("m_loc followed by m_ghost").
+
+Everything is written out with index arrays (P^(t) as a row list), cell by cell, through fe_oracle's element
+matrices: no kernels, no fusion.  Pins (tests/test_oracle_dd.py): every global node has exactly one owner; the ghost
+count is one node plane; sum_t P^(t)T V^(t) reproduces fe_oracle.Operator.apply for any number of slabs on periodic,
+Dirichlet and perturbed meshes (an exact identity up to summation order); with the ghost exchange or the halo add
+left out the identity fails at the cut planes.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def slab_layers(ncz: int, nslabs: int):
+    """Cell layers [z0, z1) of each task: as even as possible, the first ncz % nslabs tasks take one more."""
+    if nslabs < 1 or nslabs > ncz:
+        raise ValueError("need 1 <= nslabs <= ncz")
+    base, rem = divmod(ncz, nslabs)
+    out, z = [], 0
+    for t in range(nslabs):
+        n = base + (1 if t < rem else 0)
+        out.append((z, z + n))
+        z += n
+    return out
+
+
+def slab_rows(mesh, z0: int, z1: int):
+    """Global rows of task t's local multivector, in local order: node planes z0 p .. z1 p (inclusive), wrapped on a
+    periodic mesh.  Returns (rows, n_owned): the first n_owned rows are locally owned, the rest is the ghost plane."""
+    p, (ndx, ndy, ndz) = mesh.p, mesh.nd
+    plane = ndx * ndy
+    planes = [iz % ndz if mesh.bc == "periodic" else iz for iz in range(z0 * p, z1 * p + 1)]
+    rows = np.concatenate([iz * plane + np.arange(plane) for iz in planes])
+    last_is_owned = mesh.bc != "periodic" and z1 == mesh.ncells[2]      # the physical boundary plane
+    n_owned = len(rows) if last_is_owned else len(rows) - plane
+    return rows, n_owned
+
+
+def slab_apply(op, z0: int, z1: int, U_loc: np.ndarray) -> np.ndarray:
+    """V^(t) = C^(t)T ( sum_{e in E_t} Q^T A^(e) Q ) C^(t) U^(t) on the cells of layers z0 <= ez < z1, in the LOCAL
+    row order of slab_rows.  Constraints are those of the global mesh restricted to the task (Dirichlet boundary
+    nodes of the physical boundary only: a cut plane is not a boundary)."""
+    m = op.mesh
+    p, (ndx, ndy, ndz) = m.p, m.nd
+    plane = ndx * ndy
+    V = np.zeros_like(U_loc)
+    for ez in range(z0, z1):
+        for ey in range(m.ncells[1]):
+            for ex in range(m.ncells[0]):
+                idx, mask = m.cell_dofs(ex, ey, ez)              # global rows (wrapped on periodic meshes)
+                giz = idx // plane
+                # local plane = global plane - z0 p; the wrapped top plane of a periodic mesh is the ghost plane
+                liz = giz - z0 * p
+                if m.bc == "periodic":
+                    liz = np.where(liz < 0, liz + ndz, liz)
+                    if ez == z1 - 1:                              # top layer: its top nodes live in the ghost plane
+                        top = (ez * p + m._i[2]) == z1 * p
+                        liz = np.where(top, (z1 - z0) * p, liz)
+                lidx = liz * plane + idx % plane
+                U = U_loc[lidx]
+                if mask is not None:
+                    U[mask] = 0.0
+                W = op.cell_apply(ex, ey, ez, U)
+                if mask is not None:
+                    W[mask] = 0.0
+                V[lidx] += W
+    return V
+
+
+def dd_apply(op, X: np.ndarray, nslabs: int, exchange_ghosts: bool = True, halo_add: bool = True) -> np.ndarray:
+    """V = sum_t P^(t)T V^(t), V^(t) = A^(t) P^(t) U.  The two switches exist for the pins only (what breaks without
+    each communication step)."""
+    m = op.mesh
+    X = np.asarray(X, dtype=np.float64)
+    V = np.zeros_like(X)
+    for (z0, z1) in slab_layers(m.ncells[2], nslabs):
+        rows, n_owned = slab_rows(m, z0, z1)
+        U_loc = X[rows].copy()                                   # P^(t) U: owned rows + received ghost rows
+        if not exchange_ghosts:
+            U_loc[n_owned:] = 0.0
+        V_loc = slab_apply(op, z0, z1, U_loc)
+        if halo_add:
+            np.add.at(V, rows, V_loc)                            # P^(t)T: owned rows stay, ghost rows go to their owner
+        else:
+            np.add.at(V, rows[:n_owned], V_loc[:n_owned])
+    return V

@@ -41,6 +41,35 @@ def work_per_dof_vec(p: int, diagonal_metric: bool, even_odd: bool = True):
     return (fma + other) / p ** 3, (2 * fma + other) / p ** 3
 
 
+def work_per_dof_vec_oi(p: int, nq: int, diagonal_metric: bool = False):
+    """The same count for n_q != n_p Gauss points per direction: rectangular
+    even-odd contractions.  A line through a table with mi inputs and mo outputs costs
+    ceil(mo/2) ceil(mi/2) + floor(mo/2) floor(mi/2) FMA and 2 floor(mi/2) + 2 floor(mo/2) adds (split + combine).
+    Forward: N along x on n^2 lines (n -> nq), along y on nq n lines, along z on nq^2 lines; D~ (nq x nq) on nq^2 lines
+    per direction; the transposes mirror them; the quadrature-point step acts on nq^3 points.
+    Returns (FP64 instructions, flops) per DoF*vector."""
+    n = p + 1
+
+    def line(mi, mo):
+        fma = ((mo + 1) // 2) * ((mi + 1) // 2) + (mo // 2) * (mi // 2)
+        return fma, 2 * (mi // 2) + 2 * (mo // 2)
+
+    fma = other = 0
+    for lines, mi, mo in ((n * n, n, nq), (nq * n, n, nq), (nq * nq, n, nq)):       # N forward and N^T back
+        f, a = line(mi, mo)
+        fma += 2 * lines * f
+        other += 2 * lines * a
+    f, a = line(nq, nq)                                                              # D~ and D~^T, three directions
+    fma += 6 * nq * nq * f
+    other += 6 * nq * nq * a
+    if diagonal_metric:
+        other += 4 * nq ** 3
+    else:
+        fma += 6 * nq ** 3
+        other += 4 * nq ** 3
+    return (fma + other) / p ** 3, (2 * fma + other) / p ** 3
+
+
 def executed_instr_per_dof_vec_cartesian(p: int) -> float:
     """FP64 instructions the Cartesian plane / line kernels actually execute per DoF*vector:
     even/odd operators chained without combine+split, Ds^T g Ds applied as the one precomputed 1D operator
