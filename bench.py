@@ -414,6 +414,39 @@ def run_ours(args):
         except Exception as exc:
             small = {"error": str(exc)[:200]}
 
+    # ---- the decomposed apply (Alg. 5) on z-slabs, all tasks on this one GPU
+    #      (dd.SlabGroup: messages are device copies): what the partitioner, the ghost exchange and the halo add cost
+    #      on top of the fused kernels; config 4's mesh, 16 vectors
+    ddres = None
+    if rank == 0 and world == 1 and not args.no_others and args.config == 2:
+        try:
+            from paper_2208_07129_b200 import dd
+            wd = inputs.configs()[4]
+            nvd = 16
+            nd_ = wd.ndof * nvd
+            Xg = torch.empty(nd_, dtype=torch.float64, device="cuda"); binding.fill_uniform(Xg, wd.seed)
+            ddres = []
+            for ns in (1, 2, 4):
+                grp = dd.SlabGroup(wd, ns, device=local)
+                U = grp.scatter(Xg, nvd)
+                V = [torch.empty_like(u) for u in U]
+                for _ in range(2):
+                    grp.apply(U, V, nvd)
+                d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                d0.record(stream)
+                for _ in range(5):
+                    grp.apply(U, V, nvd)
+                d1.record(stream); torch.cuda.synchronize()
+                td = d0.elapsed_time(d1) / 5
+                ddres.append({"workload": wd.name, "nvec": nvd, "slabs": ns, "ms_per_apply": td,
+                              "value": nd_ / (td * 1e-3) / 1e9, "kernel": grp.ctxs[0].kernel_name(nvd),
+                              "halo_bytes_per_apply": 2 * 2 * ns * grp.plans[0].plane_nodes * nvd * 8})
+                del grp, U, V
+                torch.cuda.empty_cache()
+            del Xg
+        except Exception as exc:
+            ddres = {"error": str(exc)[:200]}
+
     # ---- roofline of the dominant kernel
     diag = (w.geom == inputs.GEOM_AFFINE)
     bv = op.batch_width(nvec)
@@ -490,7 +523,8 @@ def run_ours(args):
                "data": "synthetic", "config": config_dict(w, nvec, {"bv": bv, "variant": args.variant,
                                                                      "sharding": "vector columns, no collective"}),
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roof,
-               "cpu_baseline": cpu, "chebyshev": cheb, "other_configs": others, "config1_cuda_graph": small}
+               "cpu_baseline": cpu, "chebyshev": cheb, "other_configs": others, "config1_cuda_graph": small,
+               "decomposed_apply": ddres}
         print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

@@ -65,6 +65,31 @@ int fe_mf_create(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double sigma
                  const double box_lo[3], const double box_hi[3], const double *vertices_host,
                  int cuda_device);
 
+/*
+ * the distributed half of the paper (section 3.2.5, Alg. 5): the mesh is cut
+ * into subdomains, one per task; a task stores its locally-owned DoFs followed by the "ghost" DoFs on the shared
+ * subdomain boundary and evaluates  V = sum_t P^(t)T A^(t) P^(t) U :  ghost values of U arrive from
+ * their owner (P^(t)), the task applies the cells it owns, the ghost rows of the result go back to their owner and are
+ * ADDED there (P^(t)T).  Here the subdomains are z-SLABS of the structured mesh.
+ *
+ * fe_mf_create_slab: like fe_mf_create for ONE slab of ncz cell layers (box_lo / box_hi / vertices_host describe the
+ *   slab itself).  z_open bit 0 / bit 1: the low / high z face is a CUT plane, not a boundary: no Dirichlet mask there
+ *   and no periodic wrap in z.  A periodic mesh is periodic in x and y only for its slabs: z_open must be 3, and the
+ *   slab has nd_z = ncz p + 1 node planes.  Multivector of a slab context: planes 0 .. ncz p of the slab, i.e. its owned
+ *   planes followed by its top plane -- the ghost plane, owned by the next task (the last slab of a Dirichlet mesh owns
+ *   its top plane: z_open = 1).  fe_mf_apply on such a context computes V^(t) = A^(t) U^(t) with the fused kernels;
+ *   fe_cheb_filter, fe_mf_set_mass_scaling and fe_mf_mass_diagonal return EUNSUPPORTED (they need data of the
+ *   neighbouring slab at every step).
+ * fe_mf_halo_add: dst_dev[k] += src_dev[k], k < count (DEVICE pointers, stream-ordered): the P^(t)T step on the
+ *   receiving side -- the neighbour's ghost plane of V added into the owner's first plane.
+ * The exchange itself is point-to-point (two neighbours per slab): paper_2208_07129_b200/dd.py drives it with
+ * torch.distributed send / recv (NCCL between GPUs; the plane to send is a contiguous block of the multivector).
+ */
+int fe_mf_create_slab(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
+                      const double box_lo[3], const double box_hi[3], const double *vertices_host, int z_open,
+                      int cuda_device);
+int fe_mf_halo_add(double *dst_dev, const double *src_dev, long long count, void *cuda_stream);
+
 /* nd_x*nd_y*nd_z including Dirichlet boundary nodes; -1 if ctx is NULL. */
 long long fe_mf_ndofs(const fe_mf_ctx *ctx);
 

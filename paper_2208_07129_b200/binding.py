@@ -25,6 +25,9 @@ _PD = C.POINTER(C.c_double)
 SYMBOLS = {
     "fe_mf_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int, _D, C.c_int, C.c_int,
                                _PD, _PD, C.c_void_p, C.c_int]),
+    "fe_mf_create_slab": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int, _D, C.c_int, C.c_int,
+                                    _PD, _PD, C.c_void_p, C.c_int, C.c_int]),
+    "fe_mf_halo_add": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]),
     "fe_mf_ndofs": (C.c_longlong, [C.c_void_p]),
     "fe_mf_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "fe_mf_apply_axpby": (C.c_int, [C.c_void_p, _D, C.c_void_p, _D, _D, C.c_void_p, C.c_int, C.c_void_p]),
@@ -92,7 +95,8 @@ class FeMf:
 
     def __init__(self, ncells: Sequence[int], p: int, sigma: float, bc: int, geom: int = FE_GEOM_AFFINE,
                  box_lo=(0.0, 0.0, 0.0), box_hi=(1.0, 1.0, 1.0), vertices: Optional[np.ndarray] = None,
-                 device: int = 0):
+                 device: int = 0, z_open: Optional[int] = None):
+        """z_open: None = a whole mesh (fe_mf_create); 0..3 = one z-slab of a decomposed mesh (fe_mf_create_slab)."""
         self._l = lib()
         self._ctx = C.c_void_p()
         lo = (C.c_double * 3)(*[float(v) for v in box_lo])
@@ -104,8 +108,12 @@ class FeMf:
                 raise ValueError("vertices must have shape (ncz+1, ncy+1, ncx+1, 3)")
             self._verts = v
             vptr = v.ctypes.data_as(C.c_void_p)
-        rc = self._l.fe_mf_create(C.byref(self._ctx), int(ncells[0]), int(ncells[1]), int(ncells[2]), int(p),
-                                  float(sigma), int(bc), int(geom), lo, hi, vptr, int(device))
+        if z_open is None:
+            rc = self._l.fe_mf_create(C.byref(self._ctx), int(ncells[0]), int(ncells[1]), int(ncells[2]), int(p),
+                                      float(sigma), int(bc), int(geom), lo, hi, vptr, int(device))
+        else:
+            rc = self._l.fe_mf_create_slab(C.byref(self._ctx), int(ncells[0]), int(ncells[1]), int(ncells[2]), int(p),
+                                           float(sigma), int(bc), int(geom), lo, hi, vptr, int(z_open), int(device))
         if rc != FE_MF_OK:
             raise FeMfError(rc, self._l.fe_mf_last_error(None).decode())
         self.ndofs = int(self._l.fe_mf_ndofs(self._ctx))
@@ -207,6 +215,18 @@ def fill_uniform(out, seed: int, offset: int = 0, stream=None):
     if rc != FE_MF_OK:
         raise FeMfError(rc, "fe_fill_uniform failed")
     return out
+
+
+def halo_add(dst, src, stream=None):
+    """dst += src on the device (fe_mf_halo_add): the receiving side of the P^(t)T step of a decomposed apply."""
+    import torch
+    assert isinstance(dst, torch.Tensor) and dst.is_cuda and dst.dtype == torch.float64 and dst.is_contiguous()
+    assert isinstance(src, torch.Tensor) and src.is_cuda and src.dtype == torch.float64 and src.is_contiguous()
+    assert dst.numel() == src.numel()
+    rc = lib().fe_mf_halo_add(dst.data_ptr(), src.data_ptr(), dst.numel(), _stream_ptr(stream))
+    if rc != FE_MF_OK:
+        raise FeMfError(rc, "fe_mf_halo_add failed")
+    return dst
 
 
 def probe_peaks(device: int = 0):

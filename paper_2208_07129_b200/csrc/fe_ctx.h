@@ -15,6 +15,7 @@
 
 struct fe_mf_ctx {
   int ncx, ncy, ncz, p, n, bc, geom;
+  int zopen = 0;            // NEXT-4: bit 0 / 1 = the low / high z face is a cut plane of a decomposed mesh (fe_mf_create_slab)
   int ndx, ndy, ndz;
   long long ndof, ncells;
   double sigma;

@@ -47,10 +47,13 @@ bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int 
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
   if (trim && (c->ndx < 3 || c->ndy < 3 || c->ndz < 3)) return false;
-  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)(c->ndx - trim), (cuuint64_t)(c->ndy - trim), (cuuint64_t)(c->ndz - trim)};
+  // nodes dropped at the low / high end of each direction; a cut plane of a slab (NEXT-4) is not a boundary
+  const int lo = (trim == 2) ? 1 : 0, hi = trim ? 1 : 0;
+  const int loz = (c->zopen & 1) ? 0 : lo, hiz = (c->zopen & 2) ? 0 : hi;
+  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)(c->ndx - lo - hi), (cuuint64_t)(c->ndy - lo - hi), (cuuint64_t)(c->ndz - loz - hiz)};
   const cuuint64_t strides[3] = {(cuuint64_t)nvec * 8, (cuuint64_t)nvec * 8 * c->ndx, (cuuint64_t)nvec * 8 * c->ndx * c->ndy};
   if (strides[2] >= ((cuuint64_t)1 << 40)) return false;
-  if (trim == 2) base = (const char*)base + (strides[0] + strides[1] + strides[2]);
+  base = (const char*)base + (lo * strides[0] + lo * strides[1] + loz * strides[2]);
   const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)(c->n + padx), (cuuint32_t)c->n, (cuuint32_t)c->n};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
@@ -117,6 +120,7 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.ndx = c->ndx; P.ndy = c->ndy; P.ndz = c->ndz;
   P.nvec = nvec; P.bv = bv; P.nvb = (nvec + bv - 1) / bv;
   P.dirichlet = (c->bc == FE_BC_DIRICHLET) ? 1 : 0;
+  P.zopen = c->zopen;
   P.geom_mode = c->geom_mode;
   P.nsm = c->nsm;
   P.geom_stride = c->geom_stride;
@@ -216,7 +220,7 @@ extern "C" int fe_mf_apply_axpby(fe_mf_ctx* ctx, double alpha, const double* W_d
   ctx->last_launches = 0;
   const size_t count = (size_t)ctx->ndof * nvec;
   const int kind = pick_kernel(ctx, nvec, W_dev, Z_dev);
-  if (kind_adds_identity(ctx, kind) && gamma != 0.0 && ctx->bc == FE_BC_PERIODIC) {
+  if (kind_adds_identity(ctx, kind) && gamma != 0.0 && ctx->bc == FE_BC_PERIODIC && !ctx->zopen) {
     // the kernel adds gamma W itself (IDENT): the separate pass only has to scale Z (or zero it)
     if (beta == 0.0) {
       FE_CUDA(ctx, cudaMemsetAsync(Z_dev, 0, count * sizeof(double), st));
@@ -270,6 +274,7 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
                               double a0, void* cuda_stream) {
   int rc = check_io(ctx, X_dev, Y_dev, nvec);
   if (rc) return rc;
+  if (ctx->zopen) return fail(ctx, FE_MF_EUNSUPPORTED, "fe_cheb_filter on a slab context: every step needs a halo exchange (use fe_mf_apply_axpby per step)");
   if (m < 1) return fail(ctx, FE_MF_EINVAL, "m must be >= 1");
   if (!(b > a)) return fail(ctx, FE_MF_EINVAL, "need b > a (inverted or empty damping interval)");
   if (!(a0 < a)) return fail(ctx, FE_MF_EINVAL, "need a0 < a");
@@ -412,6 +417,12 @@ extern "C" int fe_fill_uniform(double* out_dev, long long count, unsigned long l
   if (!out_dev || count < 0) return FE_MF_EINVAL;
   if (count == 0) return FE_MF_OK;
   return fe_host::launch_fill_uniform(out_dev, count, seed, offset, (cudaStream_t)cuda_stream) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
+}
+
+extern "C" int fe_mf_halo_add(double* dst_dev, const double* src_dev, long long count, void* cuda_stream) {
+  if (!dst_dev || !src_dev || count < 0) return FE_MF_EINVAL;
+  if (count == 0) return FE_MF_OK;
+  return fe_host::launch_axpby(dst_dev, src_dev, 1.0, 1.0, (size_t)count, (cudaStream_t)cuda_stream) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
 }
 
 extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {

@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
     bool live = (v0 + beta) < P.nvec;
     if (P.dirichlet) {
-      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) live = false;
     } else {
       if (ix >= P.ndx) ix -= P.ndx;
       if (iy >= P.ndy) iy -= P.ndy;
@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(256) fe_apply_general(const ApplyParams P) {
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
     bool live = (v0 + beta) < P.nvec;
     if (P.dirichlet) {
-      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) live = false;
     } else {
       if (ix >= P.ndx) ix -= P.ndx;
       if (iy >= P.ndy) iy -= P.ndy;
@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(256) fe_apply_general_oi(const ApplyParams P, 
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
     bool live = (v0 + beta) < P.nvec;
     if (P.dirichlet) {
-      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) live = false;
     } else {
       if (ix >= P.ndx) ix -= P.ndx;
       if (iy >= P.ndy) iy -= P.ndy;
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(256) fe_apply_general_oi(const ApplyParams P, 
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
     bool live = (v0 + beta) < P.nvec;
     if (P.dirichlet) {
-      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) live = false;
     } else {
       if (ix >= P.ndx) ix -= P.ndx;
       if (iy >= P.ndy) iy -= P.ndy;

@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
     const int vv = CELLS ? beta % P.nvec : v0 + beta;
     bool live = CELLS ? (ex < P.ncx && beta < (BV / P.nvec) * P.nvec) : (vv < P.nvec);
     if (P.dirichlet) {
-      if (iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+      if (iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) live = false;
     } else {
       if (iy >= P.ndy) iy -= P.ndy;
       if (iz >= P.ndz) iz -= P.ndz;
@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(NT, MINB) fe_apply_cart(const ApplyParams P) {
       for (int i = 0; i < N; ++i) {
         int iz = ez * PDEG + i;
         bool ok = true;
-        if (P.dirichlet) { if (iz == 0 || iz == P.ndz - 1) ok = false; }
+        if (P.dirichlet) { if (fe_z_masked(P, iz)) ok = false; }
         else if (iz >= P.ndz) iz -= P.ndz;
         if (ok) atomicAdd(dst + plane * iz * P.nvec, P.alpha * y[i]);
       }

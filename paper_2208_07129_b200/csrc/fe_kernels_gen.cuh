@@ -92,7 +92,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
-    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
+    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && !P.zopen && ez == P.ncz - 1;
     const bool special = dirichlet ? (ex == 0 || ex == P.ncx - 1 || ey == 0 || ey == P.ncy - 1 || ez == 0 || ez == P.ncz - 1)
                                    : (wx || wy || wz);
     if (!perq && tid < 7) GS[tid] = __ldg(P.geom + (P.geom_mode == 1 ? (size_t)cell * 7 : 0) + tid);   // visible after the barriers below
@@ -113,7 +113,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
         const int i2 = l % N, i3 = l / N;
         if (dirichlet) {
           const int iy = ey * PDEG + i2, iz = ez * PDEG + i3;
-          if (iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) {
+          if (iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) {
 #pragma unroll
             for (int i = 0; i < N; ++i) x[i] = {0.0, 0.0};
           }
@@ -309,7 +309,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
         const int i2 = l % N, i3 = l / N;
         int iy = ey * PDEG + i2, iz = ez * PDEG + i3;
         if (dirichlet) {
-          if (iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) {
+          if (iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) {
 #pragma unroll
             for (int i = 0; i < N; ++i) y[i] = {0.0, 0.0};
           }

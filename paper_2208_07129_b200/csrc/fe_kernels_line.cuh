@@ -33,6 +33,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
   const int tid = threadIdx.x;
   const bool dirichlet = P.dirichlet != 0;
   const int org = dirichlet ? -1 : 0;   // see fe_apply_cart_plane: interior input map on Dirichlet meshes
+  const int orgz = (dirichlet && !(P.zopen & 1)) ? -1 : 0;
   const double g2x = 2.0 * P.ug[0], g2y = 2.0 * P.ug[3], g4y = 4.0 * P.ug[3], g4z = 4.0 * P.ug[5], gm = P.ug[6];
 
   if (tid == 0) {
@@ -49,7 +50,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     mbar_expect_tx(bar, TL::BYTES);
-    tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + org);
+    tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + orgz);
   }
   uint32_t parity = 0;
   int rot = (blockIdx.x / P.nsm) & 3;
@@ -61,9 +62,10 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
-    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
+    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && !P.zopen && ez == P.ncz - 1;
     const bool special = wx || wy || wz;
-    const bool dlow = dirichlet && (ex == 0 || ey == 0 || ez == 0);
+    const bool zlow = ez == 0 && !(P.zopen & 1);
+    const bool dlow = dirichlet && (ex == 0 || ey == 0 || zlow);
     mbar_wait(bar, parity);
     parity ^= 1u;
     if (special) {
@@ -161,7 +163,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
         mbar_expect_tx(bar, TL::BYTES);
-        tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + org);
+        tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + orgz);
       }
     }
     // ph5: Ns^T along x, in place
@@ -211,7 +213,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
 #pragma unroll
           for (int i = 0; i < N; ++i) x[i] = {0.0, 0.0};
         }
-        if (ez == 0) x[0] = {0.0, 0.0};
+        if (zlow) x[0] = {0.0, 0.0};
       }
       sts_line2<N>(B + base + b2, stride, x);
     }

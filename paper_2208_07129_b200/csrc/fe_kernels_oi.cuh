@@ -206,7 +206,7 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
         int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
         const bool in = (k + 1) * 256 <= TOT || t < TOT;
         if (P.dirichlet) {
-          const bool bnd = ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1;
+          const bool bnd = ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz);
           if (in && bnd) B0[t] = 0.0;
         } else {
           const bool wrapped = ix >= P.ndx || iy >= P.ndy || iz >= P.ndz;
@@ -229,7 +229,7 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
       const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
       int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
       bool live = ((k + 1) * 256 <= TOT || t < TOT) && (v0 + beta) < P.nvec;
-      const bool bnd = ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1;
+      const bool bnd = ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz);
       live = live && !(P.dirichlet && bnd);
       ix = ix >= P.ndx ? ix - P.ndx : ix;   // periodic wrap (never taken on a Dirichlet mesh)
       iy = iy >= P.ndy ? iy - P.ndy : iy;
@@ -316,7 +316,7 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
         const int i1 = I % N, i2 = (I / N) % N, i3 = I / (N * N);
         int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
         if (P.dirichlet) {
-          if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) B0[t] = 0.0;
+          if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) B0[t] = 0.0;
         } else {
           const bool wrapped = ix >= P.ndx || iy >= P.ndy || iz >= P.ndz;
           ix = ix >= P.ndx ? ix - P.ndx : ix;
@@ -341,7 +341,7 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
     int ix = ex * PDEG + i1, iy = ey * PDEG + i2, iz = ez * PDEG + i3;
     bool live = (v0 + beta) < P.nvec;
     if (P.dirichlet) {
-      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || iz == 0 || iz == P.ndz - 1) live = false;
+      if (ix == 0 || ix == P.ndx - 1 || iy == 0 || iy == P.ndy - 1 || fe_z_masked(P, iz)) live = false;
     } else {
       if (ix >= P.ndx) ix -= P.ndx;
       if (iy >= P.ndy) iy -= P.ndy;

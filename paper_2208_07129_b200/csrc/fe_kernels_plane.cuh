@@ -189,6 +189,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   // node per direction (clipped); the low boundary faces are zeroed in registers in P4 (Y rows stay 0).
   const bool dirichlet = P.dirichlet != 0;
   const int org = dirichlet ? -1 : 0;
+  const int orgz = (dirichlet && !(P.zopen & 1)) ? -1 : 0;   // a slab's low cut plane is inside the input map
   const double g2x = 2.0 * P.ug[0], g2y = 2.0 * P.ug[3], g4y = 4.0 * P.ug[3], g4z = 4.0 * P.ug[5], gm = P.ug[6];
   if (tid == 0) {
     mbar_init(bar, 1);
@@ -200,7 +201,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     mbar_expect_tx(bar, TL::BYTES);
-    tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + org);
+    tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + orgz);
   }
   uint32_t parity = 0;
   // Items are handed out dynamically (the first one is blockIdx.x): co-resident blocks do not run at the same
@@ -209,9 +210,10 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     const int vb = item % P.nvb, cell = item / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
-    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && ez == P.ncz - 1;
+    const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && !P.zopen && ez == P.ncz - 1;
     const bool special = wx || wy || wz;
-    const bool dlow = dirichlet && (ex == 0 || ey == 0 || ez == 0);
+    const bool zlow = ez == 0 && !(P.zopen & 1);   // the low z face is a Dirichlet boundary (not a cut plane)
+    const bool dlow = dirichlet && (ex == 0 || ey == 0 || zlow);
     // the next item: consumed later, latency hidden (asm volatile: the compiler must not schedule anything that
     // depends on the result up here)
     unsigned nxt_raw = 0;
@@ -343,7 +345,7 @@ FE_ZLOOP_PRAGMA
         const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
         mbar_expect_tx(bar, TL::BYTES);
-        tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + org);
+        tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + orgz);
       }
     }
     // P4: z-lines (i1, i2 = k): Ns^T along z, in place in B
@@ -386,7 +388,7 @@ FE_ZLOOP_PRAGMA
           const bool zl = (ey == 0 && k == 0) || (ex == 0 && i == 0);
 #pragma unroll
           for (int j = 0; j < N; ++j)
-            if (zl || (j == 0 && ez == 0)) x[j] = 0.0;
+            if (zl || (j == 0 && zlow)) x[j] = 0.0;
         }
 #pragma unroll
         for (int j = 0; j < N; ++j) b[j * S3] = x[j];

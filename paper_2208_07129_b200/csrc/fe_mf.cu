@@ -106,16 +106,18 @@ void cell_vertices(const fe_mf_ctx* c, const double* verts, const double lo[3], 
 
 }  // namespace
 
-extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
-                            const double box_lo[3], const double box_hi[3], const double* vertices_host,
-                            int cuda_device) {
+static int create_impl(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
+                       const double box_lo[3], const double box_hi[3], const double* vertices_host,
+                       int cuda_device, int zopen) {
   if (!out) return fail(nullptr, FE_MF_EINVAL, "out is NULL");
   *out = nullptr;
   if (ncx < 1 || ncy < 1 || ncz < 1) return fail(nullptr, FE_MF_EINVAL, "cells per direction must be >= 1");
   if (p < 1 || p > 8) return fail(nullptr, FE_MF_EINVAL, "p must be in 1..8");
   if (bc != FE_BC_PERIODIC && bc != FE_BC_DIRICHLET) return fail(nullptr, FE_MF_EINVAL, "unknown bc");
   if (geom != FE_GEOM_AFFINE && geom != FE_GEOM_QPOINT) return fail(nullptr, FE_MF_EINVAL, "unknown geom");
-  if (bc == FE_BC_PERIODIC && (ncx < 2 || ncy < 2 || ncz < 2))
+  if (zopen < 0 || zopen > 3 || (bc == FE_BC_PERIODIC && zopen != 0 && zopen != 3))
+    return fail(nullptr, FE_MF_EINVAL, "z_open must be 0..3; a periodic slab is cut at both z faces (3)");
+  if (bc == FE_BC_PERIODIC && (ncx < 2 || ncy < 2 || (ncz < 2 && !zopen)))
     return fail(nullptr, FE_MF_EINVAL, "periodic needs >= 2 cells per direction");
   if (!vertices_host) {
     if (!box_lo || !box_hi) return fail(nullptr, FE_MF_EINVAL, "box_lo/box_hi are NULL");
@@ -135,7 +137,8 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   if (!c) return fail(nullptr, FE_MF_ENOMEM, "out of host memory");
   c->ncx = ncx; c->ncy = ncy; c->ncz = ncz; c->p = p; c->n = p + 1; c->bc = bc; c->geom = geom;
   const int add = (bc == FE_BC_DIRICHLET) ? 1 : 0;
-  c->ndx = ncx * p + add; c->ndy = ncy * p + add; c->ndz = ncz * p + add;
+  c->zopen = zopen;
+  c->ndx = ncx * p + add; c->ndy = ncy * p + add; c->ndz = ncz * p + (zopen ? 1 : add);   // a slab carries its top (ghost) plane
   c->ndof = (long long)c->ndx * c->ndy * c->ndz;
   c->ncells = (long long)ncx * ncy * ncz;
   c->sigma = sigma; c->device = cuda_device; c->nsm = prop.multiProcessorCount;
@@ -233,6 +236,18 @@ extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, d
   }
   *out = c;
   return FE_MF_OK;
+}
+
+extern "C" int fe_mf_create(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
+                            const double box_lo[3], const double box_hi[3], const double* vertices_host,
+                            int cuda_device) {
+  return create_impl(out, ncx, ncy, ncz, p, sigma, bc, geom, box_lo, box_hi, vertices_host, cuda_device, 0);
+}
+
+extern "C" int fe_mf_create_slab(fe_mf_ctx** out, int ncx, int ncy, int ncz, int p, double sigma, int bc, int geom,
+                                 const double box_lo[3], const double box_hi[3], const double* vertices_host,
+                                 int z_open, int cuda_device) {
+  return create_impl(out, ncx, ncy, ncz, p, sigma, bc, geom, box_lo, box_hi, vertices_host, cuda_device, z_open);
 }
 
 extern "C" long long fe_mf_ndofs(const fe_mf_ctx* ctx) { return ctx ? ctx->ndof : -1; }
@@ -460,6 +475,7 @@ int build_mass_diagonal(fe_mf_ctx* c) {
 
 extern "C" int fe_mf_set_mass_scaling(fe_mf_ctx* ctx, int on) {
   if (!ctx) return FE_MF_EINVAL;
+  if (ctx->zopen) return fail(ctx, FE_MF_EUNSUPPORTED, "mass scaling on a slab context: diag(M) at a cut plane needs the neighbour's cells");
   DeviceGuard guard(ctx->device);
   if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");
   FE_CUDA(ctx, cudaDeviceSynchronize());
@@ -478,6 +494,7 @@ extern "C" int fe_mf_set_mass_scaling(fe_mf_ctx* ctx, int on) {
 
 extern "C" int fe_mf_mass_diagonal(fe_mf_ctx* ctx, double* out_host) {
   if (!ctx) return FE_MF_EINVAL;
+  if (ctx->zopen) return fail(ctx, FE_MF_EUNSUPPORTED, "mass diagonal of a slab context: a cut plane needs the neighbour's cells");
   if (!out_host) return fail(ctx, FE_MF_EINVAL, "out_host is NULL");
   DeviceGuard guard(ctx->device);
   if (!guard.ok) return fail(ctx, FE_MF_ECUDA, "cudaSetDevice failed");

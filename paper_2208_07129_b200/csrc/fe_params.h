@@ -19,6 +19,9 @@ struct ApplyParams {
   int bv;                         // vectors per block
   int nvb;                        // ceil(nvec / bv)
   int dirichlet;                  // 1: boundary nodes read as 0 / not written
+  int zopen;                      // z-slab of a decomposed mesh: bit 0 / bit 1 = the low / high z face is
+                                  // a CUT plane, not a boundary: no Dirichlet mask there and no periodic wrap in z (a periodic
+                                  // slab has both bits set and ndz = ncz p + 1: its top plane is the ghost plane)
   int geom_mode;                  // 0 uniform (ug), 1 per-cell constants, 2 per-q-point
   int nsm;                        // SM count (persistent kernels)
   long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
@@ -30,6 +33,13 @@ struct ApplyParams {
                                   // the mass factor is ug[6] * kappa_Q, ug[6] then holding det J without sigma
                                   // (general kernel, and the Cartesian kernels instantiated with EIG)
 };
+
+#if defined(__CUDACC__)
+// the z planes that the Dirichlet constraint masks (the physical boundary; a cut plane of a slab is not one)
+__host__ __device__ inline bool fe_z_masked(const ApplyParams& P, int iz) {
+  return (iz == 0 && !(P.zopen & 1)) || (iz == P.ndz - 1 && !(P.zopen & 2));
+}
+#endif
 
 // n_q != n_p Gauss points per direction
 struct OiParams {

@@ -1,0 +1,206 @@
+"""Domain-decomposed apply (section 3.2.5 / Alg. 5) on z-slabs.
+
+    V = sum_t P^(t)T A^(t) P^(t) U
+
+One task t per process (one process per GPU, `torch.distributed` for the point-to-point exchange: NCCL between GPUs),
+or several tasks in ONE process on one device (`SlabGroup`: the exchange is a device copy), which is how the path is
+run and checked on a single B200.  A task owns the cell layers z0 <= ez < z1 and the node planes z0 p <= iz < z1 p; its
+local multivector is its owned planes followed by its top plane, the ghost plane, so that both messages
+of a task are CONTIGUOUS blocks of the multivector and nothing is packed:
+
+    P^(t):    the owner of the ghost plane (task t+1) sends its first owned plane of U          -> ghost plane of U^(t)
+    A^(t):    fe_mf_apply on the slab context (fe_mf_create_slab): the fused kernels, cut planes open
+    P^(t)T:   task t sends the ghost plane of V^(t) to task t+1, which ADDS it to its first plane (fe_mf_halo_add)
+
+This module is argument marshalling and message ordering only; the arithmetic is in libfe_mf.so.  The local operator
+and the halo add are injected (`ops`), so that the message pattern can be exercised without a GPU (tests/
+test_dd_gloo.py runs it over gloo with the CPU oracle standing in for the two device calls).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Callable, List, Optional, Sequence, Tuple
+
+
+def slab_layers(ncz: int, nslabs: int) -> List[Tuple[int, int]]:
+    """Cell layers [z0, z1) of each task: as even as possible, the first ncz % nslabs tasks take one more."""
+    if nslabs < 1 or nslabs > ncz:
+        raise ValueError("need 1 <= nslabs <= ncz")
+    base, rem = divmod(ncz, nslabs)
+    out, z = [], 0
+    for t in range(nslabs):
+        n = base + (1 if t < rem else 0)
+        out.append((z, z + n))
+        z += n
+    return out
+
+
+@dataclass(frozen=True)
+class SlabPlan:
+    """Bookkeeping of one task: sizes are in node PLANES of the local multivector (a plane = nd_x nd_y nvec doubles)."""
+    rank: int
+    nslabs: int
+    z0: int
+    z1: int
+    p: int
+    periodic: bool
+    plane_nodes: int                 # nd_x * nd_y
+
+    @property
+    def nplanes(self) -> int:        # planes of the local multivector (owned + the top plane)
+        return (self.z1 - self.z0) * self.p + 1
+
+    @property
+    def has_ghost(self) -> bool:     # the top plane belongs to the next task (else it is the Dirichlet boundary plane)
+        return self.periodic or self.rank < self.nslabs - 1
+
+    @property
+    def up(self) -> Optional[int]:   # owner of the ghost plane
+        if not self.has_ghost:
+            return None
+        return (self.rank + 1) % self.nslabs
+
+    @property
+    def down(self) -> Optional[int]:  # the task whose ghost plane is this task's first plane
+        if self.periodic:
+            return (self.rank - 1) % self.nslabs
+        return self.rank - 1 if self.rank > 0 else None
+
+    @property
+    def z_open(self) -> int:
+        """fe_mf_create_slab's mask: bit 0 / 1 = low / high z face is a cut plane."""
+        if self.periodic:
+            return 3
+        return (1 if self.rank > 0 else 0) | (2 if self.rank < self.nslabs - 1 else 0)
+
+    @property
+    def n_owned_planes(self) -> int:
+        return self.nplanes - 1 if self.has_ghost else self.nplanes
+
+
+def make_plan(ncells: Sequence[int], p: int, periodic: bool, nslabs: int, rank: int) -> SlabPlan:
+    z0, z1 = slab_layers(ncells[2], nslabs)[rank]
+    add = 0 if periodic else 1
+    return SlabPlan(rank, nslabs, z0, z1, p, periodic, (ncells[0] * p + add) * (ncells[1] * p + add))
+
+
+def slab_geometry(w, plan: SlabPlan):
+    """(ncells, box_lo, box_hi, vertices) of the slab of workload w (paper_2208_07129_b200.inputs.Workload)."""
+    from . import inputs
+    ncz = w.ncells[2]
+    hz = (w.box_hi[2] - w.box_lo[2]) / ncz
+    lo = (w.box_lo[0], w.box_lo[1], w.box_lo[2] + hz * plan.z0)
+    hi = (w.box_hi[0], w.box_hi[1], w.box_lo[2] + hz * plan.z1)
+    verts = inputs.workload_vertices(w)
+    if verts is not None:
+        verts = verts[plan.z0:plan.z1 + 1].copy()
+    return (w.ncells[0], w.ncells[1], plan.z1 - plan.z0), lo, hi, verts
+
+
+@dataclass
+class LocalOps:
+    """The two device calls of a task: V_loc = A^(t) U_loc, and dst += src."""
+    apply: Callable
+    halo_add: Callable
+
+
+def device_ops(w, plan: SlabPlan, device: int = 0):
+    """LocalOps backed by libfe_mf.so (fe_mf_create_slab / fe_mf_apply / fe_mf_halo_add)."""
+    from . import binding
+    nc, lo, hi, verts = slab_geometry(w, plan)
+    op = binding.FeMf(nc, w.p, w.sigma, w.bc, w.geom, lo, hi, verts, device, z_open=plan.z_open)
+    return LocalOps(apply=lambda U, V, nvec: op.apply(U, V, nvec), halo_add=binding.halo_add), op
+
+
+def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, scratch=None):
+    """One task of the decomposed apply with torch.distributed point-to-point messages (dist = torch.distributed).
+    U_loc / V_loc: flat tensors of nplanes * plane_nodes * nvec doubles; the ghost plane of U_loc is overwritten.
+    `scratch`: one plane, receives the neighbour's ghost plane of V."""
+    pe = plan.plane_nodes * nvec
+    own = plan.n_owned_planes * pe
+    if plan.nslabs == 1:                       # a single periodic task is its own neighbour
+        if plan.has_ghost:
+            U_loc[own:own + pe].copy_(U_loc[:pe])
+        ops.apply(U_loc, V_loc, nvec)
+        if plan.has_ghost:
+            ops.halo_add(V_loc[:pe], V_loc[own:own + pe])
+        return V_loc
+    # P^(t): first owned plane of U goes down, the ghost plane comes from above
+    reqs = []
+    if plan.down is not None:
+        reqs.append(dist.isend(U_loc[:pe], plan.down))
+    if plan.up is not None:
+        reqs.append(dist.irecv(U_loc[own:own + pe], plan.up))
+    for r in reqs:
+        r.wait()
+    ops.apply(U_loc, V_loc, nvec)
+    # P^(t)T: ghost plane of V goes up, the neighbour's comes from below and is added into the first plane
+    if scratch is None:
+        scratch = V_loc.new_empty(pe)
+    reqs = []
+    if plan.up is not None:
+        reqs.append(dist.isend(V_loc[own:own + pe], plan.up))
+    if plan.down is not None:
+        reqs.append(dist.irecv(scratch[:pe], plan.down))
+    for r in reqs:
+        r.wait()
+    if plan.down is not None:
+        ops.halo_add(V_loc[:pe], scratch[:pe])
+    return V_loc
+
+
+class SlabGroup:
+    """All tasks of a decomposed mesh in ONE process on one device: the messages become device copies.  This is the
+    form the path takes on a single GPU (tests, bench); with one process per GPU use dd_apply_rank."""
+
+    def __init__(self, w, nslabs: int, device: int = 0, make_ops: Optional[Callable] = None):
+        from . import inputs
+        periodic = w.bc == inputs.BC_PERIODIC
+        self.w, self.nslabs = w, nslabs
+        self.plans = [make_plan(w.ncells, w.p, periodic, nslabs, t) for t in range(nslabs)]
+        self.ops, self.ctxs = [], []
+        for pl in self.plans:
+            if make_ops is None:
+                o, ctx = device_ops(w, pl, device)
+                self.ctxs.append(ctx)
+            else:
+                o = make_ops(w, pl)
+            self.ops.append(o)
+
+    def scatter(self, X, nvec: int):
+        """Global multivector (flat, nd_z planes) -> list of local multivectors (owned planes + ghost plane left unset)."""
+        out = []
+        for pl in self.plans:
+            pe = pl.plane_nodes * nvec
+            U = X.new_empty(pl.nplanes * pe)
+            first = pl.z0 * pl.p
+            U[:pl.n_owned_planes * pe].copy_(X[first * pe:(first + pl.n_owned_planes) * pe])
+            out.append(U)
+        return out
+
+    def gather(self, V_locs, nvec: int, out):
+        """Owned planes of every task -> global multivector."""
+        for pl, V in zip(self.plans, V_locs):
+            pe = pl.plane_nodes * nvec
+            first = pl.z0 * pl.p
+            out[first * pe:(first + pl.n_owned_planes) * pe].copy_(V[:pl.n_owned_planes * pe])
+        return out
+
+    def apply(self, U_locs, V_locs, nvec: int):
+        """V^(t) for every task, ghost planes exchanged and added: on return the owned planes of V_locs hold A U."""
+        plans = self.plans
+        for pl, U in zip(plans, U_locs):                      # P^(t)
+            if pl.has_ghost:
+                pe = pl.plane_nodes * nvec
+                own = pl.n_owned_planes * pe
+                U[own:own + pe].copy_(U_locs[pl.up][:pe])
+        for o, U, V in zip(self.ops, U_locs, V_locs):         # A^(t)
+            o.apply(U, V, nvec)
+        # P^(t)T: every first plane is final after the local applies only in its OWN task's sum, so the adds are
+        # independent of one another (a task's ghost plane is never another add's destination)
+        for pl, V in zip(plans, V_locs):
+            if pl.has_ghost:
+                pe = pl.plane_nodes * nvec
+                own = pl.n_owned_planes * pe
+                self.ops[pl.up].halo_add(V_locs[pl.up][:pe], V[own:own + pe])
+        return V_locs

@@ -1,0 +1,115 @@
+"""world_size-2 and -3 gloo tests of the decomposed apply's host logic (paper_2208_07129_b200/
+dd.py): slab bookkeeping, neighbour ranks, the order of the point-to-point messages of PAPER.md:742-790 (Alg. 5) and
+the halo add.  The two DEVICE calls of a task (local apply, halo add) are replaced by the CPU oracle / a tensor add
+-- injected through dd.LocalOps -- so that the message pattern runs here without a GPU; the same dd_apply_rank drives
+NCCL messages between GPUs.  The single-process form (dd.SlabGroup) is exercised with the same stand-ins."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from oracle import dd_oracle as ddo
+from oracle import fe_oracle as orc
+from paper_2208_07129_b200 import dd, inputs
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close(); return p
+
+
+def _workload(bc):
+    return inputs.Workload("dd_host", 3, (2, 2, 5), bc, inputs.GEOM_AFFINE, 0.7, (0.0, 0.0, 0.0), (1.0, 1.5, 2.5), 3, 4321)
+
+
+def _oracle_ops(w, plan):
+    """Stand-ins for fe_mf_apply on a slab context and fe_mf_halo_add (host logic tests only)."""
+    bc = "periodic" if w.bc == inputs.BC_PERIODIC else "dirichlet"
+    op = orc.Operator(orc.Mesh(w.ncells, w.p, bc, w.box_lo, w.box_hi), w.sigma)
+
+    def apply(U, V, nvec):
+        V.copy_(torch.from_numpy(ddo.slab_apply(op, plan.z0, plan.z1, U.numpy().reshape(-1, nvec).copy()).reshape(-1)))
+
+    return dd.LocalOps(apply=apply, halo_add=lambda dst, src: dst.add_(src))
+
+
+def _worker(rank, world, port, bc, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = _workload(bc)
+        nvec = w.nvec
+        plan = dd.make_plan(w.ncells, w.p, bc == inputs.BC_PERIODIC, world, rank)
+        X = inputs.multivector(w.seed, w.ndof, nvec)                       # every rank can generate the global block
+        pe = plan.plane_nodes * nvec
+        U = torch.full((plan.nplanes * pe,), float("nan"), dtype=torch.float64)
+        first = plan.z0 * plan.p
+        U[:plan.n_owned_planes * pe] = torch.from_numpy(X.reshape(-1)[first * pe:(first + plan.n_owned_planes) * pe].copy())
+        V = torch.full_like(U, float("nan"))
+        dd.dd_apply_rank(plan, _oracle_ops(w, plan), U, V, nvec, dist)
+        q.put((rank, plan.z0, plan.z1, plan.n_owned_planes, V[:plan.n_owned_planes * pe].numpy().copy()))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("world", [2, 3])
+def test_decomposed_apply_over_gloo(bc, world):
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, bc, q)) for r in range(world)]
+    for p in procs: p.start()
+    res = sorted((q.get(timeout=180) for _ in range(world)), key=lambda r: r[0])
+    for p in procs: p.join(timeout=60)
+    assert all(p.exitcode == 0 for p in procs)
+    w = _workload(bc)
+    bcs = "periodic" if bc == inputs.BC_PERIODIC else "dirichlet"
+    Y = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma).apply(inputs.multivector(w.seed, w.ndof, w.nvec))
+    plane = w.nd[0] * w.nd[1] * w.nvec
+    covered = 0
+    for rank, z0, z1, nown, Vown in res:
+        first = z0 * w.p
+        ref = Y.reshape(-1)[first * plane:(first + nown) * plane]
+        assert np.abs(Vown - ref).max() <= 1e-13 * np.abs(Y).max(), (rank, z0, z1)
+        covered += nown
+    assert covered == w.nd[2]                                              # the owned planes partition the mesh
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("nslabs", [1, 2, 4, 5])
+def test_slab_group_single_process(bc, nslabs):
+    """dd.SlabGroup (all tasks in one process: the single-GPU form) with the oracle stand-ins: scatter, exchange,
+    local applies, halo adds, gather = the single-domain apply."""
+    w = _workload(bc)
+    nvec = w.nvec
+    grp = dd.SlabGroup(w, nslabs, make_ops=_oracle_ops)
+    X = inputs.multivector(w.seed, w.ndof, nvec)
+    Xt = torch.from_numpy(X.reshape(-1).copy())
+    U = grp.scatter(Xt, nvec)
+    V = [torch.full_like(u, float("nan")) for u in U]
+    grp.apply(U, V, nvec)
+    out = grp.gather(V, nvec, torch.full_like(Xt, float("nan")))
+    bcs = "periodic" if bc == inputs.BC_PERIODIC else "dirichlet"
+    Y = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma).apply(X)
+    assert np.abs(out.numpy().reshape(Y.shape) - Y).max() <= 1e-13 * np.abs(Y).max()
+
+
+def test_plan_bookkeeping():
+    """Neighbours, cut-plane masks and sizes of every task."""
+    for periodic in (True, False):
+        for ns in (1, 2, 3):
+            plans = [dd.make_plan((2, 3, 6), 4, periodic, ns, t) for t in range(ns)]
+            assert sum(pl.n_owned_planes for pl in plans) == (6 * 4 if periodic else 6 * 4 + 1)
+            for t, pl in enumerate(plans):
+                assert pl.nplanes == (pl.z1 - pl.z0) * 4 + 1
+                if periodic:
+                    assert pl.z_open == 3 and pl.up == (t + 1) % ns and pl.down == (t - 1) % ns and pl.has_ghost
+                else:
+                    assert pl.z_open == ((1 if t > 0 else 0) | (2 if t < ns - 1 else 0))
+                    assert pl.up == (t + 1 if t < ns - 1 else None) and pl.down == (t - 1 if t > 0 else None)
+                    assert pl.has_ghost == (t < ns - 1)
+    assert dd.slab_layers(7, 3) == [(0, 3), (3, 5), (5, 7)]
