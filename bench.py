@@ -231,7 +231,7 @@ def run_ours(args):
         dt = time.perf_counter() - t0
         dt = sharding.max_over_ranks(dt, dist, "cuda")
         e2e = {"value": world * count * n_e2e / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": count * 8,
-               "d2h_bytes_per_step": count * 8, "steps": n_e2e, "api": "fe_mf_apply_host (pinned host buffers)"}
+               "d2h_bytes_per_step": count * 8, "steps": n_e2e, "api": "fe_mf_apply_host (pinned host buffers; z-slab pipeline: contiguous H2D / kernel item ranges / contiguous D2H on three streams)", "launches_per_step": op.last_launch_count()}
         y_host_check = float((Yh.cuda() - Y).abs().max().item())
         e2e["max_abs_diff_vs_device_path"] = y_host_check
 

@@ -142,9 +142,12 @@ int fe_cheb_filter(fe_mf_ctx *ctx, double *X_dev, double *Y_dev, int nvec, int m
 
 /*
  * fe_mf_apply_host -- end-to-end convenience: same as fe_mf_apply but X_host / Y_host are HOST
- * buffers (pinned memory recommended).  The library stages column blocks through an internal
- * device workspace (H2D copy, kernels, D2H copy, overlapped on two internal streams, each with its own
- * work counter) and returns after Y_host is complete.  Errors as fe_mf_apply plus ENOMEM.
+ * buffers (pinned memory recommended).  Large calls on the TMA kernels are pipelined over z-slabs of the mesh: a
+ * range of node planes is one contiguous block of the (z-major) multivector on both sides of the bus, so slab k+1
+ * is copied in and slab k-1 copied out at the full pinned rate while the kernel runs on the cell layers of slab k
+ * (three internal streams; device workspace = the whole X and Y).  Other calls stage column blocks (strided
+ * copies) through a smaller workspace on two internal streams, each with its own work counter.  Returns after
+ * Y_host is complete.  Errors as fe_mf_apply plus ENOMEM.
  */
 int fe_mf_apply_host(fe_mf_ctx *ctx, const double *X_host, double *Y_host, int nvec);
 
@@ -214,7 +217,7 @@ int fe_mf_last_launch_count(const fe_mf_ctx *ctx);
 /* Select a kernel variant (0 = default: chosen from degree, geometry and nvec).  For tests and profiling only:
  * 1 general fallback kernel (with n_q != n_p: loads and atomics on every cell instead of TMA), 2 one-vector-per-thread
  * Cartesian kernel (LDG/RED), 7 full-metric TMA kernel on a Cartesian mesh, 8 plane kernel (p = 6), 10 / 11 line
- * kernel with 16 / 8 vectors per block.  Returns EINVAL if unknown. */
+ * kernel with 16 / 8 vectors per block; 22 / 23 fe_mf_apply_host in column chunks only / in z-slabs whatever the size.  Returns EINVAL if unknown. */
 int fe_mf_set_variant(fe_mf_ctx *ctx, int variant);
 
 /* Message of the last failing call on ctx; with ctx == NULL, of the last failing fe_mf_create on

@@ -54,8 +54,8 @@ struct fe_mf_ctx {
   std::unordered_map<const void*, long long> kstate;
   // fe_mf_apply_host workspace
   double* ws_x = nullptr; double* ws_y = nullptr; size_t ws_elems = 0;
-  cudaStream_t hs[2] = {nullptr, nullptr};
-  cudaEvent_t hev[2] = {nullptr, nullptr};
+  cudaStream_t hs[3] = {nullptr, nullptr, nullptr};   // column-chunk path: two streams; slab path: H2D, kernels, D2H
+  std::vector<cudaEvent_t> hev;                       // slab path: one "slab is on the device" and one "chunk is done" event per chunk
   std::string err;
 };
 

@@ -10,7 +10,8 @@
 //   kind 1  fe_apply_general     anything else (nvec = 1, odd nvec with a full metric): plain contractions
 //   kind 11 fe_apply_oi / fe_apply_general_oi   n_q != n_p points per direction
 // fe_mf_set_variant forces a kind for tests and profiling: 1 -> kind 1, 2 -> kind 2, 7 -> kind 6 on a Cartesian
-// mesh, 8 -> plane, 10 -> line with 16-vector blocks, 11 -> line with 8-vector blocks.
+// mesh, 8 -> plane, 10 -> line with 16-vector blocks, 11 -> line with 8-vector blocks; 22 / 23 -> fe_mf_apply_host always in
+// column chunks / in z-slabs whatever the size.
 #include <cstring>
 
 #include "fe_ctx.h"
@@ -125,6 +126,7 @@ fe::ApplyParams make_params(const fe_mf_ctx* c, const double* W, double* Z, doub
   P.nsm = c->nsm;
   P.geom_stride = c->geom_stride;
   P.item_ctr = fe_host::item_counter(c);
+  P.item0 = 0; P.item_count = 0;
   P.idw = 0.0;
   P.dscale = c->mass_scaled ? c->dscale_dev : nullptr;
   P.kappa = c->kappa_dev;
@@ -139,11 +141,13 @@ bool kind_adds_identity(const fe_mf_ctx* c, int kind) { return (kind == 8 && c->
 
 // Z += alpha * A * W  (Z already initialised); idw != 0 (only if kind_adds_identity): Z += alpha A W + idw W in one
 // launch.  Counts launches into c->last_launches.
-int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st, double idw = 0.0) {
+int launch_accumulate(fe_mf_ctx* c, double alpha, const double* W, double* Z, int nvec, cudaStream_t st, double idw = 0.0,
+                      int item0 = 0, int item_count = 0) {
   const int kind = pick_kernel(c, nvec, W, Z);
   const int bv = kernel_bv(c, kind, nvec);
   fe::ApplyParams P = make_params(c, W, Z, alpha, nvec, bv);
   P.idw = idw;
+  P.item0 = item0; P.item_count = item_count;   // persistent kernels only (kinds 6, 8, 9): a range of cell layers
   if (c->ncells * (long long)P.nvb > 2147483647LL) return fail(c, FE_MF_EINVAL, "grid too large");
   cudaError_t e = cudaErrorInvalidValue;
   CUtensorMap tw, tz;
@@ -358,11 +362,100 @@ extern "C" int fe_cheb_filter(fe_mf_ctx* ctx, double* X_dev, double* Y_dev, int 
   return FE_MF_OK;
 }
 
+namespace {
+
+// fe_mf_apply_host, pipelined over z-SLABS of the mesh (the persistent TMA kernels only: they take item ranges).
+// The multivector is z-major, so a range of node planes is ONE contiguous block on both sides of the bus: the copies
+// run at the full pinned rate (55 GB/s each way measured on the box, 49 GB/s with both directions busy), whereas a
+// column chunk is a strided 2-D copy of 128-byte rows (the column-chunk path below: 29 GB/s each way).  Chunk k =
+// cell layers lay[k] .. lay[k+1]: its kernel (an item range of the one persistent kernel) needs the node planes up to
+// lay[k+1] p, starts when their copy has landed, and leaves planes lay[k] p .. lay[k+1] p - 1 of Y final (the top
+// plane also receives from chunk k+1; on a periodic mesh plane 0 also from the last chunk, so it travels last).
+// Three internal streams: H2D, kernels, D2H.  Needs the whole X and Y on the device (2 ndof nvec doubles).
+int apply_host_slabs(fe_mf_ctx* ctx, const double* X_host, double* Y_host, int nvec, int nchunks) {
+  const size_t total = (size_t)ctx->ndof * nvec;
+  if (ctx->ws_elems < total) {
+    if (ctx->ws_x) cudaFree(ctx->ws_x);
+    if (ctx->ws_y) cudaFree(ctx->ws_y);
+    ctx->ws_x = ctx->ws_y = nullptr; ctx->ws_elems = 0;
+    if (cudaMalloc(&ctx->ws_x, total * sizeof(double)) != cudaSuccess || cudaMalloc(&ctx->ws_y, total * sizeof(double)) != cudaSuccess) {
+      if (ctx->ws_x) cudaFree(ctx->ws_x);
+      ctx->ws_x = nullptr; (void)cudaGetLastError();
+      return FE_MF_ENOMEM;   // the caller falls back to the column-chunk path
+    }
+    ctx->ws_elems = total;
+  }
+  for (cudaStream_t& s_ : ctx->hs)
+    if (!s_) FE_CUDA(ctx, cudaStreamCreateWithFlags(&s_, cudaStreamNonBlocking));
+  while ((int)ctx->hev.size() < 2 * nchunks) {
+    cudaEvent_t ev;
+    FE_CUDA(ctx, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    ctx->hev.push_back(ev);
+  }
+  cudaStream_t sin = ctx->hs[0], sk = ctx->hs[1], sout = ctx->hs[2];
+  double *dx = ctx->ws_x, *dy = ctx->ws_y;
+  const size_t plane = (size_t)ctx->ndx * ctx->ndy * nvec;
+  const bool periodic = ctx->bc == FE_BC_PERIODIC && !ctx->zopen;
+  const int kind = pick_kernel(ctx, nvec, dx, dy);
+  const int bv = kernel_bv(ctx, kind, nvec);
+  const long long layer_items = (long long)ctx->ncx * ctx->ncy * ((nvec + bv - 1) / bv);
+  FE_CUDA(ctx, cudaMemsetAsync(dy, 0, total * sizeof(double), sk));
+  int first_in = 0, launches = 0, rc = FE_MF_OK;
+  for (int k = 0; k < nchunks && rc == FE_MF_OK; ++k) {
+    const int l0 = (int)((long long)ctx->ncz * k / nchunks), l1 = (int)((long long)ctx->ncz * (k + 1) / nchunks);
+    int last_in = l1 * ctx->p;                             // top node plane the chunk's cells read
+    if (last_in > ctx->ndz - 1) last_in = ctx->ndz - 1;    // periodic: the top plane of the last layer is plane 0, copied first
+    if (last_in >= first_in) {
+      FE_CUDA(ctx, cudaMemcpyAsync(dx + (size_t)first_in * plane, X_host + (size_t)first_in * plane,
+                                   (size_t)(last_in - first_in + 1) * plane * sizeof(double), cudaMemcpyHostToDevice, sin));
+      first_in = last_in + 1;
+    }
+    FE_CUDA(ctx, cudaEventRecord(ctx->hev[2 * k], sin));
+    FE_CUDA(ctx, cudaStreamWaitEvent(sk, ctx->hev[2 * k], 0));
+    ctx->ctrl_slot = 1;
+    ctx->last_launches = 0;
+    rc = launch_accumulate(ctx, 1.0, dx, dy, nvec, sk, 0.0, (int)(l0 * layer_items), (int)((l1 - l0) * layer_items));
+    ctx->ctrl_slot = 0;
+    if (rc) break;
+    launches += ctx->last_launches;
+    FE_CUDA(ctx, cudaEventRecord(ctx->hev[2 * k + 1], sk));
+    FE_CUDA(ctx, cudaStreamWaitEvent(sout, ctx->hev[2 * k + 1], 0));
+    // planes final after this chunk: lay[k] p .. lay[k+1] p - 1 (the last chunk: up to the end); periodic plane 0 waits
+    int o0 = l0 * ctx->p, o1 = (k == nchunks - 1) ? ctx->ndz - 1 : l1 * ctx->p - 1;
+    if (periodic && k == 0) o0 = 1;
+    if (o1 >= o0)
+      FE_CUDA(ctx, cudaMemcpyAsync(Y_host + (size_t)o0 * plane, dy + (size_t)o0 * plane, (size_t)(o1 - o0 + 1) * plane * sizeof(double),
+                                   cudaMemcpyDeviceToHost, sout));
+    if (periodic && k == nchunks - 1)
+      FE_CUDA(ctx, cudaMemcpyAsync(Y_host, dy, plane * sizeof(double), cudaMemcpyDeviceToHost, sout));
+  }
+  for (cudaStream_t s_ : ctx->hs) FE_CUDA(ctx, cudaStreamSynchronize(s_));
+  if (rc) return rc;
+  ctx->last_launches = launches;
+  return FE_MF_OK;
+}
+
+}  // namespace
+
 extern "C" int fe_mf_apply_host(fe_mf_ctx* ctx, const double* X_host, double* Y_host, int nvec) {
   if (!ctx) return FE_MF_EINVAL;
   if (!X_host || !Y_host) return fail(ctx, FE_MF_EINVAL, "null host pointer");
   if (nvec < 1) return fail(ctx, FE_MF_EINVAL, "nvec must be >= 1");
   DeviceGuard guard(ctx->device);
+  {
+    // large outputs on the persistent TMA kernels: z-slab pipeline with contiguous copies (variant 22 switches it off)
+    const int kind = pick_kernel(ctx, nvec, nullptr, nullptr);
+    const size_t bytes = (size_t)ctx->ndof * nvec * sizeof(double);
+    int nchunks = ctx->ncz < 12 ? ctx->ncz : 12;
+    const long long layer_items = (long long)ctx->ncx * ctx->ncy * ((nvec + kernel_bv(ctx, kind, nvec) - 1) / kernel_bv(ctx, kind, nvec));
+    const bool force = ctx->variant == 23;   // tests: the slab pipeline on meshes of any size
+    while (!force && nchunks > 1 && (long long)(ctx->ncz / nchunks) * layer_items < 2LL * 2 * ctx->nsm) --nchunks;   // >= 2 items per resident block
+    if ((kind == 6 || kind == 8 || kind == 9) && ctx->variant != 22 &&
+        (force ? nchunks >= 2 : (nchunks >= 3 && bytes >= ((size_t)32 << 20)))) {
+      const int rc = apply_host_slabs(ctx, X_host, Y_host, nvec, nchunks);
+      if (rc != FE_MF_ENOMEM) return rc;
+    }
+  }
   // column chunks: copies of chunk k+1 / k-1 overlap the kernels of chunk k on two streams
   // (at least 16 columns = 128-byte rows per chunk: strided host copies with 64-byte rows ran at half the rate;
   // measured on config 2: 1 chunk 42 ms, 2 chunks of 16 columns 30 ms, 4 chunks of 8 columns 43 ms)
@@ -385,8 +478,8 @@ extern "C" int fe_mf_apply_host(fe_mf_ctx* ctx, const double* X_host, double* Y_
     }
     ctx->ws_elems = per * nbuf;
   }
-  for (int i = 0; i < 2; ++i)
-    if (!ctx->hs[i]) FE_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->hs[i], cudaStreamNonBlocking));
+  for (cudaStream_t& s_ : ctx->hs)
+    if (!s_) FE_CUDA(ctx, cudaStreamCreateWithFlags(&s_, cudaStreamNonBlocking));
   int launches = 0, rc = FE_MF_OK;
   for (int k = 0; k < nchunks && rc == FE_MF_OK; ++k) {
     const int c0 = k * cw, w = (c0 + cw <= nvec) ? cw : (nvec - c0);
@@ -448,7 +541,7 @@ extern "C" int fe_mf_last_launch_count(const fe_mf_ctx* ctx) { return ctx ? ctx-
 
 extern "C" int fe_mf_set_variant(fe_mf_ctx* ctx, int variant) {
   if (!ctx) return FE_MF_EINVAL;
-  const bool known = variant == 0 || variant == 1 || variant == 2 || variant == 7 || variant == 8 || variant == 10 || variant == 11;
+  const bool known = variant == 0 || variant == 1 || variant == 2 || variant == 7 || variant == 8 || variant == 10 || variant == 11 || variant == 22 || variant == 23;
   if (!known) return fail(ctx, FE_MF_EINVAL, "unknown kernel variant");
   ctx->variant = variant;
   return FE_MF_OK;

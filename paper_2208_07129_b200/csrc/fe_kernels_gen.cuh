@@ -73,7 +73,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
 
   int item = blockIdx.x;
   if (tid == 0 && item < nitems) {
-    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     mbar_expect_tx(bar, TL::BYTES);
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG, ey * PDEG, ez * PDEG);
@@ -89,7 +89,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     unsigned nxt_raw = 0;
     if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
     const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
-    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && !P.zopen && ez == P.ncz - 1;
@@ -234,7 +234,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
       const int nxt = (int)(gridDim.x + nxt_raw);
       if (nxt < nitems) {
         mbar_expect_tx(gbar, GBYTES);
-        bulk_load(GS, P.geom + (size_t)(nxt / P.nvb) * P.geom_stride, GBYTES, gbar);
+        bulk_load(GS, P.geom + (size_t)((nxt + P.item0) / P.nvb) * P.geom_stride, GBYTES, gbar);
       }
     }
     // ph5: R += Ds_x^T S0 -> A
@@ -254,7 +254,7 @@ fe_apply_gen_tma(const __grid_constant__ CUtensorMap tmW, const __grid_constant_
     if (tid == 0) {
       const int nxt = (int)(gridDim.x + nxt_raw);
       if (nxt < nitems) {
-        const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
+        const int nvb_ = (nxt + P.item0) % P.nvb, ncell = (nxt + P.item0) / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
         mbar_expect_tx(bar, TL::BYTES);
         tma_load_4d(B, &tmW, bar, nvb_ * BV, nex * PDEG, ney * PDEG, nez * PDEG);

@@ -47,7 +47,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
   __syncthreads();
   int item = blockIdx.x;
   if (tid == 0 && item < nitems) {
-    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     mbar_expect_tx(bar, TL::BYTES);
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + orgz);
@@ -59,7 +59,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     unsigned nxt_raw = 0;
     if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
     const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
-    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && !P.zopen && ez == P.ncz - 1;
@@ -160,7 +160,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
       const int nxt = (int)(gridDim.x + nxt_raw);
       *s_next = nxt;
       if (nxt < nitems) {
-        const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
+        const int nvb_ = (nxt + P.item0) % P.nvb, ncell = (nxt + P.item0) / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
         mbar_expect_tx(bar, TL::BYTES);
         tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + orgz);

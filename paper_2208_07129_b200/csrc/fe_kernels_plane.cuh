@@ -130,11 +130,18 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
                                                  bool wx, bool wy, bool wz) {
   constexpr int N = PDEG + 1, HB = BV / 2, FACE = N * N * HB;
   const long long nvec = P.nvec;
+  constexpr int IT = (FACE + NT - 1) / NT;
 #pragma unroll
   for (int f = 0; f < 3; ++f) {
     if (!(f == 0 ? wx : (f == 1 ? wy : wz))) continue;
-#pragma unroll 1
-    for (int r = tid; r < FACE; r += NT) {
+    // all the loads of a thread are issued before the first store (one L2 round trip per face instead of IT)
+    double2 val[IT];
+    double2* dst[IT];
+#pragma unroll
+    for (int it = 0; it < IT; ++it) {
+      const int r = tid + it * NT;
+      dst[it] = nullptr;
+      if (r >= FACE) continue;
       const int b2 = (r % HB) * 2, a = (r / HB) % N, b = r / (HB * N);
       int i1, i2, i3;
       if (f == 0) { i1 = N - 1; i2 = a; i3 = b; }
@@ -148,11 +155,17 @@ __device__ __forceinline__ void plane_wrap_fixup(double* tile, const ApplyParams
       const long long g = ((long long)ix + (long long)P.ndx * ((long long)iy + (long long)P.ndy * iz)) * nvec + v0 + b2;
       double2* s = reinterpret_cast<double2*>(tile + ((i3 * N + i2) * (N + PADX) + i1) * BV + b2);
       if (!OUT) {
-        *s = __ldg(reinterpret_cast<const double2*>(P.W + g));
+        val[it] = __ldg(reinterpret_cast<const double2*>(P.W + g));
+        dst[it] = s;
       } else {
         const double2 d = *s;
         atomicAdd(P.Z + g, d.x); atomicAdd(P.Z + g + 1, d.y);
       }
+    }
+    if (!OUT) {
+#pragma unroll
+      for (int it = 0; it < IT; ++it)
+        if (dst[it]) *dst[it] = val[it];
     }
   }
 }
@@ -198,7 +211,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   __syncthreads();
   int item = blockIdx.x;
   if (tid == 0 && item < nitems) {
-    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     mbar_expect_tx(bar, TL::BYTES);
     tma_load_4d(A, &tmW, bar, vb * BV, ex * PDEG + org, ey * PDEG + org, ez * PDEG + orgz);
@@ -207,7 +220,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   // Items are handed out dynamically (the first one is blockIdx.x): co-resident blocks do not run at the same
   // speed (the warp arbiter favours one of them), and a static round-robin would leave the slow ones behind.
   while (item < nitems) {
-    const int vb = item % P.nvb, cell = item / P.nvb;
+    const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);
     const int v0 = vb * BV;
     const bool wx = !dirichlet && ex == P.ncx - 1, wy = !dirichlet && ey == P.ncy - 1, wz = !dirichlet && !P.zopen && ez == P.ncz - 1;
@@ -342,7 +355,7 @@ FE_ZLOOP_PRAGMA
       const int nxt = (int)(gridDim.x + nxt_raw);
       *s_next = nxt;
       if (nxt < nitems) {
-        const int nvb_ = nxt % P.nvb, ncell = nxt / P.nvb;
+        const int nvb_ = (nxt + P.item0) % P.nvb, ncell = (nxt + P.item0) / P.nvb;
         const int nex = ncell % P.ncx, ney = (ncell / P.ncx) % P.ncy, nez = ncell / (P.ncx * P.ncy);
         mbar_expect_tx(bar, TL::BYTES);
         tma_load_4d(A, &tmW, bar, nvb_ * BV, nex * PDEG + org, ney * PDEG + org, nez * PDEG + orgz);

@@ -6,7 +6,7 @@ static cudaError_t launch_line_v(fe_mf_ctx* c, const fe::ApplyParams& prm, const
   constexpr int PADX = line_padx(PDEG, C::BV);
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV, PADX>::PITCH + 64;
   auto kern = fe::fe_apply_cart_line<PDEG, C::BV, C::NT, C::MINB, PADX, IDENT, EIG>;
-  const long long nitems = c->ncells * prm.nvb;
+  const long long nitems = prm.item_count ? prm.item_count : c->ncells * prm.nvb;
   long long grid = 0;
   cudaError_t e = persistent_grid(c, kern, C::NT, SMEM, nitems, grid);
   if (e == cudaSuccess) e = reset_counter(c, st);

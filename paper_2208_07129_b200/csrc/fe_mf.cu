@@ -272,8 +272,8 @@ extern "C" void fe_mf_destroy(fe_mf_ctx* ctx) {
   { double* b[] = {ctx->oi_N, ctx->oi_D, ctx->oi_w, ctx->oi_geom}; for (double* q : b) if (q) cudaFree(q); }
   if (ctx->ws_x) cudaFree(ctx->ws_x);
   if (ctx->ws_y) cudaFree(ctx->ws_y);
-  for (int i = 0; i < 2; ++i) if (ctx->hs[i]) cudaStreamDestroy(ctx->hs[i]);
-  for (int i = 0; i < 2; ++i) if (ctx->hev[i]) cudaEventDestroy(ctx->hev[i]);
+  for (cudaStream_t s_ : ctx->hs) if (s_) cudaStreamDestroy(s_);
+  for (cudaEvent_t ev : ctx->hev) if (ev) cudaEventDestroy(ev);
   delete ctx;
 }
 

@@ -26,6 +26,8 @@ struct ApplyParams {
   int nsm;                        // SM count (persistent kernels)
   long long geom_stride;          // doubles per cell in geom (per-q-point: 7 n^3 rounded up to even; per-cell: 7)
   int* item_ctr;                  // persistent kernels: work counter (0 at launch); item = gridDim.x + atomicAdd after the first
+  int item0, item_count;          // persistent kernels: the launch processes items item0 .. item0 + item_count - 1 of the
+                                  // ncells * nvb items (cell-major: a range of cell layers); item_count = 0: all of them
   double idw;                     // Cartesian kernels with IDENT: Z += alpha A W + idw W
   const double* dscale;           // nullptr, or d = diag(M)^-1/2 [ndof] of the GLL-lumped mass matrix: Z += alpha d.(A (d.W))
                                   // (Eq. B.1; full-metric kernels only)

@@ -26,7 +26,7 @@ static cudaError_t launch_gen_p(fe_mf_ctx* c, const fe::ApplyParams& prm, const 
   constexpr int NN = (PDEG + 1) * (PDEG + 1) * (PDEG + 1);
   constexpr size_t SMEM = (size_t)3 * fe::DenseTile<PDEG, C::BV>::PITCH + ((size_t)7 * NN * 8 + 15) / 16 * 16 + 64;
   auto kern = fe::fe_apply_gen_tma<PDEG, C::BV, C::NT, C::MINB, MSC>;
-  const long long nitems = c->ncells * prm.nvb;
+  const long long nitems = prm.item_count ? prm.item_count : c->ncells * prm.nvb;
   long long grid = 0;
   cudaError_t e = persistent_grid(c, kern, C::NT, SMEM, nitems, grid);
   if (e == cudaSuccess) e = reset_counter(c, st);

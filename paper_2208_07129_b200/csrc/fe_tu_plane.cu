@@ -19,7 +19,7 @@ static cudaError_t launch_plane_v(fe_mf_ctx* c, const fe::ApplyParams& prm, cons
   constexpr size_t SMEM = (size_t)2 * fe::DenseTile<PDEG, C::BV>::PITCH + 64;
   auto kern = fe::fe_apply_cart_plane<PDEG, C::BV, C::NT, C::MINB, IDENT, EIG>;
   long long grid = 0;
-  const long long nitems = c->ncells * prm.nvb;
+  const long long nitems = prm.item_count ? prm.item_count : c->ncells * prm.nvb;
   cudaError_t e = persistent_grid(c, kern, C::NT, SMEM, nitems, grid);
   if (e == cudaSuccess) e = reset_counter(c, st);
   if (e != cudaSuccess) return e;

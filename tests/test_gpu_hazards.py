@@ -178,3 +178,35 @@ def test_chebyshev_narrow_interval_does_not_underflow(env, a, b, a0, m):
     assert np.isfinite(F).all()
     assert np.isfinite(Xd.cpu().numpy()).all()
     assert relerr(F, Fo) <= TOL
+
+
+@pytest.mark.parametrize("p,bc,geom,nc,nvec", [
+    (6, inputs.BC_DIRICHLET, inputs.GEOM_AFFINE, (3, 2, 7), 32),     # plane kernel
+    (6, inputs.BC_PERIODIC, inputs.GEOM_AFFINE, (2, 3, 14), 16),     # plane kernel, 12 slabs of 1-2 layers, periodic plane 0 last
+    (7, inputs.BC_PERIODIC, inputs.GEOM_AFFINE, (2, 2, 5), 10),      # line kernel, vector tail
+    (4, inputs.BC_DIRICHLET, inputs.GEOM_AFFINE, (3, 3, 2), 8),      # two slabs
+    (8, inputs.BC_PERIODIC, inputs.GEOM_QPOINT, (2, 2, 4), 6),       # full-metric kernel
+    (5, inputs.BC_DIRICHLET, inputs.GEOM_QPOINT, (2, 3, 6), 8),
+])
+def test_apply_host_z_slab_pipeline(env, p, bc, geom, nc, nvec):
+    """fe_mf_apply_host pipelined over z-slabs (contiguous copies; chunk k's kernel is an item range of the persistent
+    kernel and starts when its planes have landed; its planes of Y leave when it is done): variant 23 forces it on
+    small meshes.  Repeated, from a NaN-filled host output; the column-chunk path (variant 22) must agree."""
+    torch, orc, binding = env
+    w = inputs.Workload(f"host_slabs_p{p}", p, nc, bc, geom, 0.8, (0.0, 0.0, 0.0), (1.0, 1.5, 2.0), nvec, 7700 + p,
+                        perturb=0.1 if geom == inputs.GEOM_QPOINT else 0.0)
+    X = inputs.multivector(w.seed, w.ndof, nvec)
+    Yo = orc.Operator(oracle_mesh(orc, w), w.sigma).apply(X)
+    op = binding.FeMf.from_workload(w)
+    Xh = torch.from_numpy(X).contiguous().pin_memory()
+    Yh = torch.empty_like(Xh).pin_memory()
+    op.set_variant(23)
+    for rep in range(20):
+        Yh.fill_(float("nan"))
+        op.apply_host(Xh, Yh, nvec)
+        assert relerr(Yh.numpy(), Yo) <= TOL
+    assert op.last_launch_count() == min(nc[2], 12)
+    op.set_variant(22)
+    Yh.fill_(float("nan"))
+    op.apply_host(Xh, Yh, nvec)
+    assert relerr(Yh.numpy(), Yo) <= TOL
