@@ -133,6 +133,25 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+PROBE_SRC = os.path.join(CSRC, "probe_pipes.cu")
+PROBE_BIN = os.path.join(OBJ, "probe_pipes")
+
+
+def build_probe(force: bool = False, verbose: bool = False) -> str:
+    """The stand-alone box probe (DFMA vs DMMA, LDS vs DFMA; profiles/r2_probe_pipes.md): csrc/build/probe_pipes."""
+    if not force and os.path.exists(PROBE_BIN) and os.path.getmtime(PROBE_BIN) >= os.path.getmtime(PROBE_SRC):
+        return PROBE_BIN
+    os.makedirs(OBJ, exist_ok=True)
+    cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", PROBE_BIN, PROBE_SRC]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or res.returncode != 0:
+        sys.stderr.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed building probe_pipes")
+    return PROBE_BIN
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
     print(build_chfsi(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build_probe(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -89,3 +89,23 @@ def test_product_does_not_import_oracle():
                 assert "import oracle" not in txt and "from oracle" not in txt, f
     orc = open(os.path.join(ROOT, "oracle", "fe_oracle.py")).read()
     assert "paper_2208_07129_b200" not in orc.replace("`paper_2208_07129_b200/csrc`", "")
+
+
+def test_roofline_counts():
+    """The work model of paper_2208_07129_b200/roofline.py (pure counting): the even-odd count per DoF*vector quoted in
+    SURVEY.md 8(d) / DESIGN.md section 6, the rectangular count of the n_q != n_p rule reducing to it at n_q = n_p, and the
+    non-even-odd total 24 n^4 + 16 n^3 flops per cell and vector of PAPER.md:203."""
+    from paper_2208_07129_b200 import roofline
+    assert abs(roofline.work_per_dof_vec(6, True)[0] - 107.07) < 0.01       # Cartesian-diagonal metric, p = 6
+    assert abs(roofline.work_per_dof_vec(6, False)[0] - 116.6) < 0.01
+    assert abs(roofline.work_per_dof_vec(8, False)[0] - 122.45) < 0.01
+    for p in range(1, 9):
+        for diag in (True, False):
+            a = roofline.work_per_dof_vec(p, diag)
+            b = roofline.work_per_dof_vec_oi(p, p + 1, diag)
+            assert abs(a[0] - b[0]) < 1e-12 and abs(a[1] - b[1]) < 1e-12
+        n = p + 1
+        fma, other = roofline.fp64_instr_per_cell_vec(p, False, even_odd=False)
+        assert 2 * fma + other == 24 * n ** 4 + 16 * n ** 3
+    assert roofline.work_per_dof_vec_oi(8, 11, False)[0] > 1.7 * roofline.work_per_dof_vec(8, False)[0]
+    assert roofline.bytes_per_dof_vec(6, False, 16) == 16.0 and roofline.bytes_per_dof_vec(6, False, 16, chebyshev=True) == 24.0
