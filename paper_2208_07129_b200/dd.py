@@ -149,6 +149,60 @@ def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, 
     return V_loc
 
 
+TAG_U, TAG_V = 11, 12   # ghost values of U travel down, ghost rows of V travel up: two message kinds between a pair of tasks
+
+
+def dd_apply_rank_batches(plan: SlabPlan, ops: LocalOps, U_list, V_list, nvec: int, dist, scratch_list=None):
+    """Algorithm 5: the multivector comes in n_b batches (one local multivector per batch, `nvec` columns
+    each); while batch i_b is applied, the ghost exchange of batch i_b + 1 (Alg. 5 l.3-4, finished at l.8-9) and the halo
+    add of batch i_b - 1 (l.5-6, finished at l.10-11) are in flight.  Messages between a pair of tasks are posted in
+    the same order on both sides (U of the next batch first, then V of the previous one) and carry distinct tags."""
+    nb = len(U_list)
+    pe = plan.plane_nodes * nvec
+    own = plan.n_owned_planes * pe
+    if plan.nslabs == 1:
+        for U, V in zip(U_list, V_list):
+            dd_apply_rank(plan, ops, U, V, nvec, dist)
+        return V_list
+    if scratch_list is None:
+        scratch_list = [V_list[0].new_empty(pe) for _ in range(2)]
+
+    def start_u(i):       # P^(t) for batch i
+        r = []
+        if plan.down is not None:
+            r.append(dist.isend(U_list[i][:pe], plan.down, tag=TAG_U))
+        if plan.up is not None:
+            r.append(dist.irecv(U_list[i][own:own + pe], plan.up, tag=TAG_U))
+        return r
+
+    def start_v(i):       # P^(t)T for batch i
+        r = []
+        if plan.up is not None:
+            r.append(dist.isend(V_list[i][own:own + pe], plan.up, tag=TAG_V))
+        if plan.down is not None:
+            r.append(dist.irecv(scratch_list[i & 1][:pe], plan.down, tag=TAG_V))
+        return r
+
+    def finish_v(i, reqs):
+        for r in reqs:
+            r.wait()
+        if plan.down is not None:
+            ops.halo_add(V_list[i][:pe], scratch_list[i & 1][:pe])
+
+    for r in start_u(0):                                  # Alg. 5 l.1
+        r.wait()
+    for ib in range(nb):                                  # l.2
+        ru = start_u(ib + 1) if ib + 1 < nb else []       # l.3-4
+        rv = start_v(ib - 1) if ib > 0 else []            # l.5-6
+        ops.apply(U_list[ib], V_list[ib], nvec)           # l.7
+        for r in ru:                                      # l.8-9
+            r.wait()
+        if ib > 0:                                        # l.10-11
+            finish_v(ib - 1, rv)
+    finish_v(nb - 1, start_v(nb - 1))                     # l.12
+    return V_list
+
+
 class SlabGroup:
     """All tasks of a decomposed mesh in ONE process on one device: the messages become device copies.  This is the
     form the path takes on a single GPU (tests, bench); with one process per GPU use dd_apply_rank."""

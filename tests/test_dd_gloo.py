@@ -36,6 +36,50 @@ def _oracle_ops(w, plan):
     return dd.LocalOps(apply=apply, halo_add=lambda dst, src: dst.add_(src))
 
 
+def _worker_batches(rank, world, port, bc, q):
+    """Alg. 5: three batches of the multivector, exchange of batch i+1 / halo add of batch i-1 in flight during batch i."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = _workload(bc)
+        nvec, nb = w.nvec, 3
+        plan = dd.make_plan(w.ncells, w.p, bc == inputs.BC_PERIODIC, world, rank)
+        pe = plan.plane_nodes * nvec
+        first = plan.z0 * plan.p
+        Us, Vs = [], []
+        for b in range(nb):
+            X = inputs.multivector(w.seed + 10 * b, w.ndof, nvec)
+            U = torch.full((plan.nplanes * pe,), float("nan"), dtype=torch.float64)
+            U[:plan.n_owned_planes * pe] = torch.from_numpy(X.reshape(-1)[first * pe:(first + plan.n_owned_planes) * pe].copy())
+            Us.append(U); Vs.append(torch.full_like(U, float("nan")))
+        dd.dd_apply_rank_batches(plan, _oracle_ops(w, plan), Us, Vs, nvec, dist)
+        q.put((rank, plan.z0, plan.n_owned_planes, [V[:plan.n_owned_planes * pe].numpy().copy() for V in Vs]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("world", [2, 3])
+def test_decomposed_apply_batches_overlap_over_gloo(bc, world):
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker_batches, args=(r, world, port, bc, q)) for r in range(world)]
+    for p in procs: p.start()
+    res = sorted((q.get(timeout=240) for _ in range(world)), key=lambda r: r[0])
+    for p in procs: p.join(timeout=60)
+    assert all(p.exitcode == 0 for p in procs)
+    w = _workload(bc)
+    bcs = "periodic" if bc == inputs.BC_PERIODIC else "dirichlet"
+    op = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma)
+    plane = w.nd[0] * w.nd[1] * w.nvec
+    for b in range(3):
+        Y = op.apply(inputs.multivector(w.seed + 10 * b, w.ndof, w.nvec))
+        for rank, z0, nown, Vs in res:
+            ref = Y.reshape(-1)[z0 * w.p * plane:(z0 * w.p + nown) * plane]
+            assert np.abs(Vs[b] - ref).max() <= 1e-13 * np.abs(Y).max(), (b, rank)
+
+
 def _worker(rank, world, port, bc, q):
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
