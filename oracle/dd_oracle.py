@@ -21,6 +21,13 @@ matrices: no kernels, no fusion.  Pins (tests/test_oracle_dd.py): every global n
 count is one node plane; sum_t P^(t)T V^(t) reproduces fe_oracle.Operator.apply for any number of slabs on periodic,
 Dirichlet and perturbed meshes (an exact identity up to summation order); with the ghost exchange or the halo add
 left out the identity fails at the cut planes.
+
+Mixed-precision boundary payload ("the boundary data communicated is recast as FP32 floats"): with
+`fp32_payload` every value that crosses a task boundary -- the ghost rows of U on their way in, the ghost rows of V^(t)
+on their way back -- is rounded to IEEE binary32 (round to nearest even) and widened again; everything a task computes
+stays FP64.  A single task exchanges nothing, so nothing is rounded.  Pins: the deviation from the exact apply lives
+only in the cell layer under a cut plane, on the cut plane itself it is the rounding error of the exact ghost row when
+U is FP32-representable, and it is of the size of the FP32 unit roundoff.
 """
 from __future__ import annotations
 
@@ -83,9 +90,15 @@ def slab_apply(op, z0: int, z1: int, U_loc: np.ndarray) -> np.ndarray:
     return V
 
 
-def dd_apply(op, X: np.ndarray, nslabs: int, exchange_ghosts: bool = True, halo_add: bool = True) -> np.ndarray:
-    """V = sum_t P^(t)T V^(t), V^(t) = A^(t) P^(t) U.  The two switches exist for the pins only (what breaks without
-    each communication step)."""
+def round_fp32(a: np.ndarray) -> np.ndarray:
+    """The FP32 payload of PAPER.md:752: FP64 -> binary32 (round to nearest even) -> FP64."""
+    return np.asarray(a, dtype=np.float64).astype(np.float32).astype(np.float64)
+
+
+def dd_apply(op, X: np.ndarray, nslabs: int, exchange_ghosts: bool = True, halo_add: bool = True,
+             fp32_payload: bool = False) -> np.ndarray:
+    """V = sum_t P^(t)T V^(t), V^(t) = A^(t) P^(t) U.  exchange_ghosts / halo_add exist for the pins only (what breaks
+    without each communication step); fp32_payload: the communicated rows travel as FP32."""
     m = op.mesh
     X = np.asarray(X, dtype=np.float64)
     V = np.zeros_like(X)
@@ -94,7 +107,11 @@ def dd_apply(op, X: np.ndarray, nslabs: int, exchange_ghosts: bool = True, halo_
         U_loc = X[rows].copy()                                   # P^(t) U: owned rows + received ghost rows
         if not exchange_ghosts:
             U_loc[n_owned:] = 0.0
+        elif fp32_payload and nslabs > 1:
+            U_loc[n_owned:] = round_fp32(U_loc[n_owned:])        # the ghost rows arrived as FP32
         V_loc = slab_apply(op, z0, z1, U_loc)
+        if fp32_payload and nslabs > 1:
+            V_loc[n_owned:] = round_fp32(V_loc[n_owned:])        # the ghost rows leave as FP32
         if halo_add:
             np.add.at(V, rows, V_loc)                            # P^(t)T: owned rows stay, ghost rows go to their owner
         else:

@@ -69,3 +69,56 @@ def test_decomposed_apply_on_the_perturbed_mesh():
     Y = op.apply(X)
     for ns in (2, 3):
         assert np.abs(ddo.dd_apply(op, X, ns) - Y).max() <= 1e-14 * np.abs(Y).max()
+
+
+@pytest.mark.parametrize("bc", ["periodic", "dirichlet"])
+def test_fp32_payload_deviates_only_under_the_cut_planes(bc):
+    """PAPER.md:752 (FP32 boundary payload).  What the mathematics fixes: (i) a single task exchanges nothing: no
+    deviation; (ii) the deviation from the exact apply is confined to the cell layer under each cut plane (rounded ghost
+    values of U enter only the cells that touch the ghost plane; rounded ghost rows of V land on the cut plane);
+    (iii) it has the size of the FP32 unit roundoff 2^-24, not of FP64 and not O(1); (iv) when U is itself
+    FP32-representable the inbound rounding is the identity: the deviation then sits on the cut planes only and there it
+    is exactly fl32(g) - g for the ghost row g of the exact local product, computed here from slab_apply directly."""
+    p, nc, ns = 3, (2, 2, 5), 2
+    mesh = orc.Mesh(nc, p, bc)
+    op = orc.Operator(mesh, 0.7)
+    rng = np.random.default_rng(5)
+    X = rng.uniform(-1, 1, (mesh.ndof, 2))
+    Y = ddo.dd_apply(op, X, ns)
+    scale = np.abs(Y).max()
+    assert np.array_equal(ddo.dd_apply(op, X, 1, fp32_payload=True), ddo.dd_apply(op, X, 1))          # (i)
+    D = ddo.dd_apply(op, X, ns, fp32_payload=True) - Y
+    plane = mesh.nd[0] * mesh.nd[1]
+    ndz = mesh.nd[2]
+    layers = ddo.slab_layers(nc[2], ns)
+    allowed = np.zeros(ndz, dtype=bool)
+    cuts = []
+    for (z0, z1) in layers:
+        if bc == "dirichlet" and z1 == nc[2]:
+            continue                                                   # the physical boundary is not a cut
+        cuts.append((z0, z1))
+        for iz in range((z1 - 1) * p, z1 * p + 1):
+            allowed[iz % ndz] = True
+    dev = np.abs(D).reshape(ndz, plane * 2).max(axis=1)
+    assert np.all(dev[~allowed] == 0.0)                                                                # (ii)
+    assert dev[allowed].min() > 0.0
+    assert 1e-10 * scale < dev.max() < 100 * 2.0 ** -24 * scale                                        # (iii)
+    # (iv)
+    X32 = ddo.round_fp32(X)
+    Y32 = ddo.dd_apply(op, X32, ns)
+    D32 = ddo.dd_apply(op, X32, ns, fp32_payload=True) - Y32
+    on_cut = np.zeros(ndz, dtype=bool)
+    expect = np.zeros_like(Y32)
+    for (z0, z1) in cuts:
+        on_cut[(z1 * p) % ndz] = True
+        rows, n_owned = ddo.slab_rows(mesh, z0, z1)
+        g = ddo.slab_apply(op, z0, z1, X32[rows].copy())[n_owned:]
+        expect[rows[n_owned:]] += ddo.round_fp32(g) - g
+    dev32 = np.abs(D32).reshape(ndz, plane * 2).max(axis=1)
+    assert np.all(dev32[~on_cut] == 0.0) and np.all(dev32[on_cut] > 0.0)
+    assert np.abs(D32 - expect).max() <= 4e-16 * scale
+    if bc == "dirichlet":                                              # boundary rows stay exactly zero
+        ix, iy, iz = np.meshgrid(*[np.arange(n) for n in mesh.nd], indexing="ij")
+        bnd = (ix == 0) | (ix == mesh.nd[0] - 1) | (iy == 0) | (iy == mesh.nd[1] - 1) | (iz == 0) | (iz == ndz - 1)
+        rows = (ix + mesh.nd[0] * (iy + mesh.nd[1] * iz))[bnd]
+        assert np.all(ddo.dd_apply(op, X, ns, fp32_payload=True)[rows] == 0.0)
