@@ -82,6 +82,12 @@ int fe_mf_create(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double sigma
  *   neighbouring slab at every step).
  * fe_mf_halo_add: dst_dev[k] += src_dev[k], k < count (DEVICE pointers, stream-ordered): the P^(t)T step on the
  *   receiving side -- the neighbour's ghost plane of V added into the owner's first plane.
+ * fe_mf_halo_pack_f32 / fe_mf_halo_unpack_f32: the mixed-precision boundary payload of PAPER.md:752 ("the boundary data
+ *   communicated is recast as FP32 floats").  pack: dst_dev[k] = (float) src_dev[k], round to nearest even, on the
+ *   sending side; unpack on the receiving side: dst_dev[k] = (double) src_dev[k] (add = 0: ghost values of U) or
+ *   dst_dev[k] += (double) src_dev[k] (add = 1: ghost rows of V).  DEVICE pointers, count elements, stream-ordered;
+ *   dst and src must not overlap.  Everything a task computes stays FP64: only the message is FP32 (half the bytes).
+ * Errors of the three halo calls: EINVAL (null pointer, count < 0, add not 0 / 1), ECUDA (launch failure).
  * The exchange itself is point-to-point (two neighbours per slab): paper_2208_07129_b200/dd.py drives it with
  * torch.distributed send / recv (NCCL between GPUs; the plane to send is a contiguous block of the multivector).
  */
@@ -89,6 +95,8 @@ int fe_mf_create_slab(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double 
                       const double box_lo[3], const double box_hi[3], const double *vertices_host, int z_open,
                       int cuda_device);
 int fe_mf_halo_add(double *dst_dev, const double *src_dev, long long count, void *cuda_stream);
+int fe_mf_halo_pack_f32(float *dst_dev, const double *src_dev, long long count, void *cuda_stream);
+int fe_mf_halo_unpack_f32(double *dst_dev, const float *src_dev, long long count, int add, void *cuda_stream);
 
 /* nd_x*nd_y*nd_z including Dirichlet boundary nodes; -1 if ctx is NULL. */
 long long fe_mf_ndofs(const fe_mf_ctx *ctx);

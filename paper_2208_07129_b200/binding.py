@@ -28,6 +28,8 @@ SYMBOLS = {
     "fe_mf_create_slab": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int, _D, C.c_int, C.c_int,
                                     _PD, _PD, C.c_void_p, C.c_int, C.c_int]),
     "fe_mf_halo_add": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]),
+    "fe_mf_halo_pack_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]),
+    "fe_mf_halo_unpack_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, C.c_void_p]),
     "fe_mf_ndofs": (C.c_longlong, [C.c_void_p]),
     "fe_mf_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "fe_mf_apply_axpby": (C.c_int, [C.c_void_p, _D, C.c_void_p, _D, _D, C.c_void_p, C.c_int, C.c_void_p]),
@@ -226,6 +228,30 @@ def halo_add(dst, src, stream=None):
     rc = lib().fe_mf_halo_add(dst.data_ptr(), src.data_ptr(), dst.numel(), _stream_ptr(stream))
     if rc != FE_MF_OK:
         raise FeMfError(rc, "fe_mf_halo_add failed")
+    return dst
+
+
+def halo_pack_f32(dst, src, stream=None):
+    """dst (float32) <- src (float64), round to nearest (fe_mf_halo_pack_f32): the sending side of the FP32 payload."""
+    import torch
+    assert isinstance(dst, torch.Tensor) and dst.is_cuda and dst.dtype == torch.float32 and dst.is_contiguous()
+    assert isinstance(src, torch.Tensor) and src.is_cuda and src.dtype == torch.float64 and src.is_contiguous()
+    assert dst.numel() == src.numel()
+    rc = lib().fe_mf_halo_pack_f32(dst.data_ptr(), src.data_ptr(), dst.numel(), _stream_ptr(stream))
+    if rc != FE_MF_OK:
+        raise FeMfError(rc, "fe_mf_halo_pack_f32 failed")
+    return dst
+
+
+def halo_unpack_f32(dst, src, add: bool, stream=None):
+    """dst (float64) <- src (float32), or dst += src (fe_mf_halo_unpack_f32): the receiving side of the FP32 payload."""
+    import torch
+    assert isinstance(dst, torch.Tensor) and dst.is_cuda and dst.dtype == torch.float64 and dst.is_contiguous()
+    assert isinstance(src, torch.Tensor) and src.is_cuda and src.dtype == torch.float32 and src.is_contiguous()
+    assert dst.numel() == src.numel()
+    rc = lib().fe_mf_halo_unpack_f32(dst.data_ptr(), src.data_ptr(), dst.numel(), 1 if add else 0, _stream_ptr(stream))
+    if rc != FE_MF_OK:
+        raise FeMfError(rc, "fe_mf_halo_unpack_f32 failed")
     return dst
 
 

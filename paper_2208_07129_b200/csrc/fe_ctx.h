@@ -134,6 +134,8 @@ cudaError_t launch_scale2(double* A, double* B, double sa, double sb, int swap, 
                           int ndx, int ndy, int ndz, int nvec, cudaStream_t st);
 cudaError_t launch_swap(double* A, double* B, size_t count, cudaStream_t st);
 cudaError_t launch_fill_uniform(double* out, long long count, unsigned long long seed, long long offset, cudaStream_t st);
+cudaError_t launch_halo_pack_f32(float* dst, const double* src, size_t count, cudaStream_t st);
+cudaError_t launch_halo_unpack_f32(double* dst, const float* src, size_t count, int add, cudaStream_t st);
 // fe_tu_gen.cu: full symmetric metric (per-q-point or per-cell geometry), TMA tiles
 cudaError_t launch_gen(fe_mf_ctx* c, const fe::ApplyParams& P, const CUtensorMap& tw, const CUtensorMap& tz, cudaStream_t st);
 int gen_bv(const fe_mf_ctx* c, int nvec);

@@ -518,6 +518,18 @@ extern "C" int fe_mf_halo_add(double* dst_dev, const double* src_dev, long long 
   return fe_host::launch_axpby(dst_dev, src_dev, 1.0, 1.0, (size_t)count, (cudaStream_t)cuda_stream) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
 }
 
+extern "C" int fe_mf_halo_pack_f32(float* dst_dev, const double* src_dev, long long count, void* cuda_stream) {
+  if (!dst_dev || !src_dev || count < 0) return FE_MF_EINVAL;
+  if (count == 0) return FE_MF_OK;
+  return fe_host::launch_halo_pack_f32(dst_dev, src_dev, (size_t)count, (cudaStream_t)cuda_stream) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
+}
+
+extern "C" int fe_mf_halo_unpack_f32(double* dst_dev, const float* src_dev, long long count, int add, void* cuda_stream) {
+  if (!dst_dev || !src_dev || count < 0 || (add != 0 && add != 1)) return FE_MF_EINVAL;
+  if (count == 0) return FE_MF_OK;
+  return fe_host::launch_halo_unpack_f32(dst_dev, src_dev, (size_t)count, add, (cudaStream_t)cuda_stream) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
+}
+
 extern "C" int fe_mf_batch_width(const fe_mf_ctx* ctx, int nvec) {
   if (!ctx || nvec < 1) return -1;
   const int kind = pick_kernel(ctx, nvec, nullptr, nullptr);

@@ -74,6 +74,23 @@ __global__ void fe_swap_kernel(double* __restrict__ A, double* __restrict__ B, s
   for (size_t k = i; k < count; k += stride) { double a = A[k]; A[k] = B[k]; B[k] = a; }
 }
 
+// NEXT-4, the FP32 boundary payload: the plane that crosses a task boundary is recast as binary32
+// (round to nearest even) on the sending side ...
+__global__ void fe_halo_pack_f32_kernel(float* __restrict__ dst, const double* __restrict__ src, size_t count) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t k = i; k < count; k += stride) dst[k] = __double2float_rn(src[k]);
+}
+// ... and widened on the receiving side: dst <- src (add = 0: ghost values of U) or dst += src (add = 1: ghost rows of V)
+__global__ void fe_halo_unpack_f32_kernel(double* __restrict__ dst, const float* __restrict__ src, size_t count, int add) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t k = i; k < count; k += stride) {
+    const double v = (double)src[k];
+    dst[k] = add ? dst[k] + v : v;
+  }
+}
+
 // Input generator; not part of the operator.
 __global__ void fe_fill_uniform_kernel(double* __restrict__ out, long long count, unsigned long long seed,
                                        long long offset) {

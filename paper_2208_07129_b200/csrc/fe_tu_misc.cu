@@ -126,6 +126,14 @@ cudaError_t launch_swap(double* A, double* B, size_t count, cudaStream_t st) {
   fe::fe_swap_kernel<<<stream_grid(count), 256, 0, st>>>(A, B, count);
   return cudaGetLastError();
 }
+cudaError_t launch_halo_pack_f32(float* dst, const double* src, size_t count, cudaStream_t st) {
+  fe::fe_halo_pack_f32_kernel<<<stream_grid(count), 256, 0, st>>>(dst, src, count);
+  return cudaGetLastError();
+}
+cudaError_t launch_halo_unpack_f32(double* dst, const float* src, size_t count, int add, cudaStream_t st) {
+  fe::fe_halo_unpack_f32_kernel<<<stream_grid(count), 256, 0, st>>>(dst, src, count, add);
+  return cudaGetLastError();
+}
 cudaError_t launch_fill_uniform(double* out, long long count, unsigned long long seed, long long offset, cudaStream_t st) {
   fe::fe_fill_uniform_kernel<<<stream_grid((size_t)count), 256, 0, st>>>(out, count, seed, offset);
   return cudaGetLastError();

@@ -12,6 +12,11 @@ of a task are CONTIGUOUS blocks of the multivector and nothing is packed:
     A^(t):    fe_mf_apply on the slab context (fe_mf_create_slab): the fused kernels, cut planes open
     P^(t)T:   task t sends the ghost plane of V^(t) to task t+1, which ADDS it to its first plane (fe_mf_halo_add)
 
+With `fp32_payload` the plane that crosses a task boundary travels as FP32 ("the boundary data communicated
+is recast as FP32 floats"): fe_mf_halo_pack_f32 on the sending side into a message buffer of half the bytes,
+fe_mf_halo_unpack_f32 on the receiving side (overwrite for U, add for V); everything a task computes stays FP64.  A
+single task exchanges nothing, so nothing is rounded.
+
 This module is argument marshalling and message ordering only; the arithmetic is in libfe_mf.so.  The local operator
 and the halo add are injected (`ops`), so that the message pattern can be exercised without a GPU (tests/
 test_dd_gloo.py runs it over gloo with the CPU oracle standing in for the two device calls).
@@ -99,9 +104,12 @@ def slab_geometry(w, plan: SlabPlan):
 
 @dataclass
 class LocalOps:
-    """The two device calls of a task: V_loc = A^(t) U_loc, and dst += src."""
+    """The device calls of a task: V_loc = A^(t) U_loc; dst += src; and, for the FP32 payload only, pack_f32(dst32, src64)
+    and unpack_f32(dst64, src32, add)."""
     apply: Callable
     halo_add: Callable
+    pack_f32: Optional[Callable] = None
+    unpack_f32: Optional[Callable] = None
 
 
 def device_ops(w, plan: SlabPlan, device: int = 0):
@@ -109,13 +117,21 @@ def device_ops(w, plan: SlabPlan, device: int = 0):
     from . import binding
     nc, lo, hi, verts = slab_geometry(w, plan)
     op = binding.FeMf(nc, w.p, w.sigma, w.bc, w.geom, lo, hi, verts, device, z_open=plan.z_open)
-    return LocalOps(apply=lambda U, V, nvec: op.apply(U, V, nvec), halo_add=binding.halo_add), op
+    return LocalOps(apply=lambda U, V, nvec: op.apply(U, V, nvec), halo_add=binding.halo_add,
+                    pack_f32=binding.halo_pack_f32, unpack_f32=binding.halo_unpack_f32), op
 
 
-def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, scratch=None):
+def _buffers32(like, pe: int, count: int):
+    import torch
+    return [torch.empty(pe, dtype=torch.float32, device=like.device) for _ in range(count)]
+
+
+def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, scratch=None, fp32_payload: bool = False,
+                  scratch32=None):
     """One task of the decomposed apply with torch.distributed point-to-point messages (dist = torch.distributed).
     U_loc / V_loc: flat tensors of nplanes * plane_nodes * nvec doubles; the ghost plane of U_loc is overwritten.
-    `scratch`: one plane, receives the neighbour's ghost plane of V."""
+    `scratch`: one plane, receives the neighbour's ghost plane of V.  fp32_payload: the planes travel as FP32
+    (`scratch32`: two float32 planes, the send and the receive buffer)."""
     pe = plan.plane_nodes * nvec
     own = plan.n_owned_planes * pe
     if plan.nslabs == 1:                       # a single periodic task is its own neighbour
@@ -125,38 +141,47 @@ def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, 
         if plan.has_ghost:
             ops.halo_add(V_loc[:pe], V_loc[own:own + pe])
         return V_loc
+    if fp32_payload:
+        s32, r32 = scratch32 if scratch32 is not None else _buffers32(U_loc, pe, 2)
     # P^(t): first owned plane of U goes down, the ghost plane comes from above
     reqs = []
     if plan.down is not None:
-        reqs.append(dist.isend(U_loc[:pe], plan.down))
+        reqs.append(dist.isend(ops.pack_f32(s32, U_loc[:pe]) if fp32_payload else U_loc[:pe], plan.down))
     if plan.up is not None:
-        reqs.append(dist.irecv(U_loc[own:own + pe], plan.up))
+        reqs.append(dist.irecv(r32 if fp32_payload else U_loc[own:own + pe], plan.up))
     for r in reqs:
         r.wait()
+    if fp32_payload and plan.up is not None:
+        ops.unpack_f32(U_loc[own:own + pe], r32, False)
     ops.apply(U_loc, V_loc, nvec)
     # P^(t)T: ghost plane of V goes up, the neighbour's comes from below and is added into the first plane
-    if scratch is None:
+    if scratch is None and not fp32_payload:
         scratch = V_loc.new_empty(pe)
     reqs = []
     if plan.up is not None:
-        reqs.append(dist.isend(V_loc[own:own + pe], plan.up))
+        reqs.append(dist.isend(ops.pack_f32(s32, V_loc[own:own + pe]) if fp32_payload else V_loc[own:own + pe], plan.up))
     if plan.down is not None:
-        reqs.append(dist.irecv(scratch[:pe], plan.down))
+        reqs.append(dist.irecv(r32 if fp32_payload else scratch[:pe], plan.down))
     for r in reqs:
         r.wait()
     if plan.down is not None:
-        ops.halo_add(V_loc[:pe], scratch[:pe])
+        if fp32_payload:
+            ops.unpack_f32(V_loc[:pe], r32, True)
+        else:
+            ops.halo_add(V_loc[:pe], scratch[:pe])
     return V_loc
 
 
 TAG_U, TAG_V = 11, 12   # ghost values of U travel down, ghost rows of V travel up: two message kinds between a pair of tasks
 
 
-def dd_apply_rank_batches(plan: SlabPlan, ops: LocalOps, U_list, V_list, nvec: int, dist, scratch_list=None):
+def dd_apply_rank_batches(plan: SlabPlan, ops: LocalOps, U_list, V_list, nvec: int, dist, scratch_list=None,
+                          fp32_payload: bool = False):
     """Algorithm 5: the multivector comes in n_b batches (one local multivector per batch, `nvec` columns
     each); while batch i_b is applied, the ghost exchange of batch i_b + 1 (Alg. 5 l.3-4, finished at l.8-9) and the halo
     add of batch i_b - 1 (l.5-6, finished at l.10-11) are in flight.  Messages between a pair of tasks are posted in
-    the same order on both sides (U of the next batch first, then V of the previous one) and carry distinct tags."""
+    the same order on both sides (U of the next batch first, then V of the previous one) and carry distinct tags.
+    fp32_payload: the planes travel as FP32; the U and the V message of a step have their own send / receive buffers."""
     nb = len(U_list)
     pe = plan.plane_nodes * nvec
     own = plan.n_owned_planes * pe
@@ -164,39 +189,50 @@ def dd_apply_rank_batches(plan: SlabPlan, ops: LocalOps, U_list, V_list, nvec: i
         for U, V in zip(U_list, V_list):
             dd_apply_rank(plan, ops, U, V, nvec, dist)
         return V_list
-    if scratch_list is None:
+    if fp32_payload:
+        su32, ru32, sv32, rv32 = _buffers32(U_list[0], pe, 4)
+    elif scratch_list is None:
         scratch_list = [V_list[0].new_empty(pe) for _ in range(2)]
 
     def start_u(i):       # P^(t) for batch i
         r = []
         if plan.down is not None:
-            r.append(dist.isend(U_list[i][:pe], plan.down, tag=TAG_U))
+            r.append(dist.isend(ops.pack_f32(su32, U_list[i][:pe]) if fp32_payload else U_list[i][:pe], plan.down, tag=TAG_U))
         if plan.up is not None:
-            r.append(dist.irecv(U_list[i][own:own + pe], plan.up, tag=TAG_U))
+            r.append(dist.irecv(ru32 if fp32_payload else U_list[i][own:own + pe], plan.up, tag=TAG_U))
         return r
+
+    def finish_u(i, reqs):
+        for r in reqs:
+            r.wait()
+        if fp32_payload and plan.up is not None:
+            ops.unpack_f32(U_list[i][own:own + pe], ru32, False)
 
     def start_v(i):       # P^(t)T for batch i
         r = []
         if plan.up is not None:
-            r.append(dist.isend(V_list[i][own:own + pe], plan.up, tag=TAG_V))
+            out = ops.pack_f32(sv32, V_list[i][own:own + pe]) if fp32_payload else V_list[i][own:own + pe]
+            r.append(dist.isend(out, plan.up, tag=TAG_V))
         if plan.down is not None:
-            r.append(dist.irecv(scratch_list[i & 1][:pe], plan.down, tag=TAG_V))
+            r.append(dist.irecv(rv32 if fp32_payload else scratch_list[i & 1][:pe], plan.down, tag=TAG_V))
         return r
 
     def finish_v(i, reqs):
         for r in reqs:
             r.wait()
         if plan.down is not None:
-            ops.halo_add(V_list[i][:pe], scratch_list[i & 1][:pe])
+            if fp32_payload:
+                ops.unpack_f32(V_list[i][:pe], rv32, True)
+            else:
+                ops.halo_add(V_list[i][:pe], scratch_list[i & 1][:pe])
 
-    for r in start_u(0):                                  # Alg. 5 l.1
-        r.wait()
+    finish_u(0, start_u(0))                               # Alg. 5 l.1
     for ib in range(nb):                                  # l.2
         ru = start_u(ib + 1) if ib + 1 < nb else []       # l.3-4
         rv = start_v(ib - 1) if ib > 0 else []            # l.5-6
         ops.apply(U_list[ib], V_list[ib], nvec)           # l.7
-        for r in ru:                                      # l.8-9
-            r.wait()
+        if ib + 1 < nb:                                   # l.8-9
+            finish_u(ib + 1, ru)
         if ib > 0:                                        # l.10-11
             finish_v(ib - 1, rv)
     finish_v(nb - 1, start_v(nb - 1))                     # l.12
@@ -240,14 +276,22 @@ class SlabGroup:
             out[first * pe:(first + pl.n_owned_planes) * pe].copy_(V[:pl.n_owned_planes * pe])
         return out
 
-    def apply(self, U_locs, V_locs, nvec: int):
-        """V^(t) for every task, ghost planes exchanged and added: on return the owned planes of V_locs hold A U."""
+    def apply(self, U_locs, V_locs, nvec: int, fp32_payload: bool = False):
+        """V^(t) for every task, ghost planes exchanged and added: on return the owned planes of V_locs hold A U.
+        fp32_payload: every plane that crosses a task boundary goes through an FP32 message buffer (pack / unpack)."""
         plans = self.plans
+        fp32 = fp32_payload and self.nslabs > 1
+        if fp32:
+            (m32,) = _buffers32(U_locs[0], plans[0].plane_nodes * nvec, 1)
         for pl, U in zip(plans, U_locs):                      # P^(t)
             if pl.has_ghost:
                 pe = pl.plane_nodes * nvec
                 own = pl.n_owned_planes * pe
-                U[own:own + pe].copy_(U_locs[pl.up][:pe])
+                if fp32:
+                    self.ops[pl.up].pack_f32(m32, U_locs[pl.up][:pe])
+                    self.ops[pl.rank].unpack_f32(U[own:own + pe], m32, False)
+                else:
+                    U[own:own + pe].copy_(U_locs[pl.up][:pe])
         for o, U, V in zip(self.ops, U_locs, V_locs):         # A^(t)
             o.apply(U, V, nvec)
         # P^(t)T: every first plane is final after the local applies only in its OWN task's sum, so the adds are
@@ -256,5 +300,9 @@ class SlabGroup:
             if pl.has_ghost:
                 pe = pl.plane_nodes * nvec
                 own = pl.n_owned_planes * pe
-                self.ops[pl.up].halo_add(V_locs[pl.up][:pe], V[own:own + pe])
+                if fp32:
+                    self.ops[pl.rank].pack_f32(m32, V[own:own + pe])
+                    self.ops[pl.up].unpack_f32(V_locs[pl.up][:pe], m32, True)
+                else:
+                    self.ops[pl.up].halo_add(V_locs[pl.up][:pe], V[own:own + pe])
         return V_locs

@@ -33,10 +33,14 @@ def _oracle_ops(w, plan):
     def apply(U, V, nvec):
         V.copy_(torch.from_numpy(ddo.slab_apply(op, plan.z0, plan.z1, U.numpy().reshape(-1, nvec).copy()).reshape(-1)))
 
-    return dd.LocalOps(apply=apply, halo_add=lambda dst, src: dst.add_(src))
+    def unpack_f32(dst, src, add):
+        return dst.add_(src.double()) if add else dst.copy_(src.double())
+
+    return dd.LocalOps(apply=apply, halo_add=lambda dst, src: dst.add_(src),
+                       pack_f32=lambda dst, src: dst.copy_(src.to(torch.float32)), unpack_f32=unpack_f32)
 
 
-def _worker_batches(rank, world, port, bc, q):
+def _worker_batches(rank, world, port, bc, q, fp32=False):
     """Alg. 5: three batches of the multivector, exchange of batch i+1 / halo add of batch i-1 in flight during batch i."""
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -52,19 +56,19 @@ def _worker_batches(rank, world, port, bc, q):
             U = torch.full((plan.nplanes * pe,), float("nan"), dtype=torch.float64)
             U[:plan.n_owned_planes * pe] = torch.from_numpy(X.reshape(-1)[first * pe:(first + plan.n_owned_planes) * pe].copy())
             Us.append(U); Vs.append(torch.full_like(U, float("nan")))
-        dd.dd_apply_rank_batches(plan, _oracle_ops(w, plan), Us, Vs, nvec, dist)
+        dd.dd_apply_rank_batches(plan, _oracle_ops(w, plan), Us, Vs, nvec, dist, fp32_payload=fp32)
         q.put((rank, plan.z0, plan.n_owned_planes, [V[:plan.n_owned_planes * pe].numpy().copy() for V in Vs]))
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("bc,fp32", [(inputs.BC_PERIODIC, False), (inputs.BC_DIRICHLET, False), (inputs.BC_PERIODIC, True)])
 @pytest.mark.parametrize("world", [2, 3])
-def test_decomposed_apply_batches_overlap_over_gloo(bc, world):
+def test_decomposed_apply_batches_overlap_over_gloo(bc, fp32, world):
     port = _free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    procs = [ctx.Process(target=_worker_batches, args=(r, world, port, bc, q)) for r in range(world)]
+    procs = [ctx.Process(target=_worker_batches, args=(r, world, port, bc, q, fp32)) for r in range(world)]
     for p in procs: p.start()
     res = sorted((q.get(timeout=240) for _ in range(world)), key=lambda r: r[0])
     for p in procs: p.join(timeout=60)
@@ -74,13 +78,14 @@ def test_decomposed_apply_batches_overlap_over_gloo(bc, world):
     op = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma)
     plane = w.nd[0] * w.nd[1] * w.nvec
     for b in range(3):
-        Y = op.apply(inputs.multivector(w.seed + 10 * b, w.ndof, w.nvec))
+        Xb = inputs.multivector(w.seed + 10 * b, w.ndof, w.nvec)
+        Y = ddo.dd_apply(op, Xb, world, fp32_payload=True) if fp32 else op.apply(Xb)
         for rank, z0, nown, Vs in res:
             ref = Y.reshape(-1)[z0 * w.p * plane:(z0 * w.p + nown) * plane]
             assert np.abs(Vs[b] - ref).max() <= 1e-13 * np.abs(Y).max(), (b, rank)
 
 
-def _worker(rank, world, port, bc, q):
+def _worker(rank, world, port, bc, q, fp32=False):
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -93,26 +98,34 @@ def _worker(rank, world, port, bc, q):
         first = plan.z0 * plan.p
         U[:plan.n_owned_planes * pe] = torch.from_numpy(X.reshape(-1)[first * pe:(first + plan.n_owned_planes) * pe].copy())
         V = torch.full_like(U, float("nan"))
-        dd.dd_apply_rank(plan, _oracle_ops(w, plan), U, V, nvec, dist)
+        dd.dd_apply_rank(plan, _oracle_ops(w, plan), U, V, nvec, dist, fp32_payload=fp32)
         q.put((rank, plan.z0, plan.z1, plan.n_owned_planes, V[:plan.n_owned_planes * pe].numpy().copy()))
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("bc,fp32", [(inputs.BC_PERIODIC, False), (inputs.BC_DIRICHLET, False), (inputs.BC_DIRICHLET, True),
+                                     (inputs.BC_PERIODIC, True)])
 @pytest.mark.parametrize("world", [2, 3])
-def test_decomposed_apply_over_gloo(bc, world):
+def test_decomposed_apply_over_gloo(bc, fp32, world):
+    """fp32: the planes travel as FP32; the result is then the oracle's fp32_payload result (the same
+    roundings at the same places), which differs from the exact apply at the FP32 level."""
     port = _free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    procs = [ctx.Process(target=_worker, args=(r, world, port, bc, q)) for r in range(world)]
+    procs = [ctx.Process(target=_worker, args=(r, world, port, bc, q, fp32)) for r in range(world)]
     for p in procs: p.start()
     res = sorted((q.get(timeout=180) for _ in range(world)), key=lambda r: r[0])
     for p in procs: p.join(timeout=60)
     assert all(p.exitcode == 0 for p in procs)
     w = _workload(bc)
     bcs = "periodic" if bc == inputs.BC_PERIODIC else "dirichlet"
-    Y = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma).apply(inputs.multivector(w.seed, w.ndof, w.nvec))
+    op = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    Y = op.apply(X)
+    if fp32:
+        Yexact, Y = Y, ddo.dd_apply(op, X, world, fp32_payload=True)
+        assert np.abs(Y - Yexact).max() > 1e-10 * np.abs(Y).max()
     plane = w.nd[0] * w.nd[1] * w.nvec
     covered = 0
     for rank, z0, z1, nown, Vown in res:
@@ -123,9 +136,10 @@ def test_decomposed_apply_over_gloo(bc, world):
     assert covered == w.nd[2]                                              # the owned planes partition the mesh
 
 
+@pytest.mark.parametrize("fp32", [False, True])
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
 @pytest.mark.parametrize("nslabs", [1, 2, 4, 5])
-def test_slab_group_single_process(bc, nslabs):
+def test_slab_group_single_process(bc, nslabs, fp32):
     """dd.SlabGroup (all tasks in one process: the single-GPU form) with the oracle stand-ins: scatter, exchange,
     local applies, halo adds, gather = the single-domain apply."""
     w = _workload(bc)
@@ -135,10 +149,11 @@ def test_slab_group_single_process(bc, nslabs):
     Xt = torch.from_numpy(X.reshape(-1).copy())
     U = grp.scatter(Xt, nvec)
     V = [torch.full_like(u, float("nan")) for u in U]
-    grp.apply(U, V, nvec)
+    grp.apply(U, V, nvec, fp32_payload=fp32)
     out = grp.gather(V, nvec, torch.full_like(Xt, float("nan")))
     bcs = "periodic" if bc == inputs.BC_PERIODIC else "dirichlet"
-    Y = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma).apply(X)
+    op = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma)
+    Y = ddo.dd_apply(op, X, nslabs, fp32_payload=True) if fp32 else op.apply(X)
     assert np.abs(out.numpy().reshape(Y.shape) - Y).max() <= 1e-13 * np.abs(Y).max()
 
 
