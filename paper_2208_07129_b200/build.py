@@ -4,8 +4,8 @@
 
 Produces paper_2208_07129_b200/csrc/libfe_mf.so (git-ignored; it travels with gpurun snapshots) and, beside it,
 libfe_chfsi.so (include/fe_chfsi.h: the subspace iteration around the operator; links libfe_mf.so, cuBLAS, cuSOLVER).
-libfe_mf.so is several translation units (one per kernel family, fe_tu_*.cu, plus the host code) compiled in
-parallel and linked without relocatable device code.
+libfe_mf.so is several translation units (one per kernel family, fe_tu_*.cu, plus the host code and the constraint
+matrices of include/fe_constraints.h) compiled in parallel and linked without relocatable device code.
 """
 from __future__ import annotations
 
@@ -27,6 +27,7 @@ UNITS = {
     "fe_mf.cu": HOST_DEPS + ["fe_tables.h"],
     "fe_dispatch.cu": HOST_DEPS,
     "fe_probe.cu": [FE_MF_H],
+    "fe_constraints.cu": [os.path.join("..", "..", "include", "fe_constraints.h"), FE_MF_H],
     "fe_tu_misc.cu": KERNEL_DEPS + ["fe_kernels_stream.cuh"],
     "fe_tu_gen.cu": KERNEL_DEPS + ["fe_kernels_gen.cuh"],
     "fe_tu_plane.cu": KERNEL_DEPS + ["fe_kernels_plane.cuh"],

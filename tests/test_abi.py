@@ -109,3 +109,48 @@ def test_roofline_counts():
         assert 2 * fma + other == 24 * n ** 4 + 16 * n ** 3
     assert roofline.work_per_dof_vec_oi(8, 11, False)[0] > 1.7 * roofline.work_per_dof_vec(8, False)[0]
     assert roofline.bytes_per_dof_vec(6, False, 16) == 16.0 and roofline.bytes_per_dof_vec(6, False, 16, chebyshev=True) == 24.0
+
+
+def test_constraints_header_symbols_and_validation_without_gpu(built_lib):
+    """include/fe_constraints.h: libfe_mf.so exports what the header declares, the
+    binding's table matches, the host-side validation of the sets (closed sets, index ranges, offsets) answers EINVAL
+    before any device is touched, and valid sets without a device fail with ECUDA (no CPU fallback)."""
+    import torch
+    from paper_2208_07129_b200 import binding, constraints
+    lib = ctypes.CDLL(built_lib)
+    syms = header_symbols("fe_constraints.h")
+    assert "fe_constraints_create" in syms and "fe_constraints_distribute_transpose" in syms
+    for name in syms:
+        assert hasattr(lib, name), name
+    assert sorted(constraints.SYMBOLS) == syms
+    L = constraints.lib()
+    LL = ctypes.c_longlong
+
+    def create(ndof, m_ptr, masters, s_ptr, slaves, weights):
+        h = ctypes.c_void_p()
+        arr = lambda v: (LL * max(len(v), 1))(*v)      # noqa: E731
+        w = (ctypes.c_double * max(len(weights), 1))(*weights)
+        rc = L.fe_constraints_create(ctypes.byref(h), ndof, len(m_ptr) - 1, arr(m_ptr), arr(masters), arr(s_ptr), arr(slaves),
+                                     w, None, 0)
+        return rc, h, L.fe_constraints_last_error(None)
+
+    rc, h, msg = create(5, [0, 1, 2], [1, 2], [0, 1, 2], [2, 3], [1.0, 1.0])          # slave 2 is a master of set 1
+    assert rc == binding.FE_MF_EINVAL and b"not closed" in msg and not h.value
+    rc, h, msg = create(5, [0, 1, 2], [1, 0], [0, 1, 2], [2, 2], [1.0, 1.0])          # slave 2 twice
+    assert rc == binding.FE_MF_EINVAL and b"two sets" in msg
+    rc, h, msg = create(5, [0, 1], [7], [0, 1], [2], [1.0])                           # master out of range
+    assert rc == binding.FE_MF_EINVAL and b"out of range" in msg
+    rc, h, msg = create(5, [0, 1], [1], [0, 1], [-1], [1.0])
+    assert rc == binding.FE_MF_EINVAL and b"out of range" in msg
+    rc, h, msg = create(5, [1, 1], [1], [0, 1], [2], [])                              # offsets must start at 0
+    assert rc == binding.FE_MF_EINVAL
+    rc, h, msg = create(0, [0], [], [0], [], [])
+    assert rc == binding.FE_MF_EINVAL
+    assert L.fe_constraints_distribute(None, None, 1, 0, None) == binding.FE_MF_EINVAL
+    assert L.fe_constraints_distribute_transpose(None, None, 1, None) == binding.FE_MF_EINVAL
+    assert L.fe_constraints_counts(None, None, None, None) == binding.FE_MF_EINVAL
+    L.fe_constraints_destroy(None)
+    if not torch.cuda.is_available():
+        with pytest.raises(binding.FeMfError) as e:
+            constraints.Constraints(5, [([1], [2], [[1.0]], None)])
+        assert e.value.code == binding.FE_MF_ECUDA
