@@ -117,6 +117,18 @@ long long fe_mf_ndofs(const fe_mf_ctx *ctx);
 int fe_mf_apply(fe_mf_ctx *ctx, const double *X_dev, double *Y_dev, int nvec, void *cuda_stream);
 
 /*
+ * fe_mf_apply_bcv -- the same product on the paper's Batched Contiguous Vector layout (section 3.2.1,
+ * Fig. 1): the nvec vectors in n_b = ceil(nvec / b) batches, batch i_b holding vectors i_b b .. i_b b + b_i - 1
+ * (b_i = b, the last batch nvec - (n_b - 1) b) as a contiguous [ndofs][b_i] block, vector index innermost, at offset
+ * ndofs * i_b * b doubles:   element (J, beta)  ->  ndofs * b * (beta / b) + J * b_i + beta % b.
+ * With b >= nvec this is fe_mf_apply's layout.  One kernel launch (plus the zero fill) per batch, all on cuda_stream
+ * (Eq. 17's sum over i_b); b is the caller's choice -- fe_mf_batch_width(ctx, b) tells how many vectors a thread block of
+ * the kernel chosen for that width takes.  X_dev / Y_dev: DEVICE, ndofs*nvec doubles each, must not overlap.
+ * Errors: EINVAL (null pointers, b < 1, nvec < 1, overlap), ECUDA.
+ */
+int fe_mf_apply_bcv(fe_mf_ctx *ctx, const double *X_dev, double *Y_dev, int b, int nvec, void *cuda_stream);
+
+/*
  * fe_mf_apply_axpby -- the fused form of Eq. (B.1) without mass scaling:
  *     Z <- alpha * A * W  +  beta * Z  +  gamma * W
  * W_dev read-only, Z_dev updated in place, no aliasing.  This is the one step the Chebyshev

@@ -458,6 +458,24 @@ class Operator:
 # --------------------------------------------------------------------------------------
 
 
+def to_bcv(X: np.ndarray, b: int) -> np.ndarray:
+    """Batched Contiguous Vector layout (section 3.2.1, Fig. 1): "stores the nodal values of a batch of b
+    vectors contiguously for all nodes in n_b = ceil(n_v / b) contiguous batches".  X [ndof][nvec] -> flat array, batch
+    after batch, each batch [ndof][b_i] with the vector index innermost (the last batch holds the remaining vectors)."""
+    X = np.asarray(X, dtype=np.float64)
+    return np.concatenate([np.ascontiguousarray(X[:, v0:v0 + b]).reshape(-1) for v0 in range(0, X.shape[1], b)])
+
+
+def from_bcv(flat: np.ndarray, ndof: int, nvec: int, b: int) -> np.ndarray:
+    """Inverse of to_bcv."""
+    flat = np.asarray(flat, dtype=np.float64).reshape(-1)
+    X = np.empty((ndof, nvec))
+    for v0 in range(0, nvec, b):
+        bi = min(b, nvec - v0)
+        X[:, v0:v0 + bi] = flat[ndof * v0:ndof * (v0 + bi)].reshape(ndof, bi)
+    return X
+
+
 def chebyshev_filter(apply, X: np.ndarray, m: int, a: float, b: float, a0: float) -> np.ndarray:
     """Scaled Chebyshev filter of degree m damping [a, b], a0 = lower spectral bound.
     Temporaries named as in the paper: e, c, sigma, sigma1, gamma, alpha1, alpha2."""

@@ -32,6 +32,7 @@ SYMBOLS = {
     "fe_mf_halo_unpack_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, C.c_void_p]),
     "fe_mf_ndofs": (C.c_longlong, [C.c_void_p]),
     "fe_mf_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
+    "fe_mf_apply_bcv": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "fe_mf_apply_axpby": (C.c_int, [C.c_void_p, _D, C.c_void_p, _D, _D, C.c_void_p, C.c_int, C.c_void_p]),
     "fe_mf_accumulate": (C.c_int, [C.c_void_p, _D, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "fe_cheb_filter": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, _D, _D, _D, C.c_void_p]),
@@ -135,6 +136,11 @@ class FeMf:
     def apply(self, X, Y, nvec: int, stream=None):
         _check_tensor(X, self.ndofs, nvec, "X"); _check_tensor(Y, self.ndofs, nvec, "Y")
         self._raise(self._l.fe_mf_apply(self._ctx, X.data_ptr(), Y.data_ptr(), int(nvec), _stream_ptr(stream)))
+
+    def apply_bcv(self, X, Y, b: int, nvec: int, stream=None):
+        """The apply on the paper's BCV layout (fe_mf_apply_bcv): batches of b vectors, each a contiguous [ndofs][b] block."""
+        _check_tensor(X, self.ndofs, nvec, "X"); _check_tensor(Y, self.ndofs, nvec, "Y")
+        self._raise(self._l.fe_mf_apply_bcv(self._ctx, X.data_ptr(), Y.data_ptr(), int(b), int(nvec), _stream_ptr(stream)))
 
     def apply_axpby(self, alpha: float, W, beta: float, gamma: float, Z, nvec: int, stream=None):
         _check_tensor(W, self.ndofs, nvec, "W"); _check_tensor(Z, self.ndofs, nvec, "Z")

@@ -252,6 +252,27 @@ extern "C" int fe_mf_apply(fe_mf_ctx* ctx, const double* X_dev, double* Y_dev, i
   return fe_mf_apply_axpby(ctx, 1.0, X_dev, 0.0, 0.0, Y_dev, nvec, cuda_stream);
 }
 
+// BCV layout (Fig. 1): n_b = ceil(nvec / b) batches, batch i_b = the [ndof][b_i] block of vectors
+// i_b b .. i_b b + b_i - 1 stored contiguously at offset ndof * i_b * b.  Each batch is a multivector of the simple
+// layout, so the batched apply is one fe_mf_apply per batch on the same stream (Eq. 17's sum over i_b).
+extern "C" int fe_mf_apply_bcv(fe_mf_ctx* ctx, const double* X_dev, double* Y_dev, int b, int nvec, void* cuda_stream) {
+  if (!ctx) return FE_MF_EINVAL;
+  if (!X_dev || !Y_dev) return fail(ctx, FE_MF_EINVAL, "null device pointer");
+  if (b < 1 || nvec < 1) return fail(ctx, FE_MF_EINVAL, "b and nvec must be >= 1");
+  const size_t total = (size_t)ctx->ndof * nvec;
+  if (X_dev < Y_dev + total && Y_dev < X_dev + total) return fail(ctx, FE_MF_EINVAL, "X and Y must not overlap");
+  int launches = 0;
+  for (int v0 = 0; v0 < nvec; v0 += b) {
+    const int bi = (v0 + b <= nvec) ? b : (nvec - v0);
+    const size_t off = (size_t)ctx->ndof * v0;
+    const int rc = fe_mf_apply(ctx, X_dev + off, Y_dev + off, bi, cuda_stream);
+    if (rc) return rc;
+    launches += ctx->last_launches;
+  }
+  ctx->last_launches = launches;
+  return FE_MF_OK;
+}
+
 namespace {
 
 // The scale factors s_k of the one-launch-per-step form of the recurrence (see fe_cheb_filter): s_0 = s_1 = 1,

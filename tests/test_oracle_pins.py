@@ -405,3 +405,21 @@ def test_generator():
     assert np.array_equal(inputs.multivector(9, 50, 4, rows=[3, 17]), X[[3, 17]])
     cfg = inputs.configs()
     assert [cfg[i].ndof for i in (1, 2, 3, 4, 5)] == [32768, 3048625, 2097152, 11239424, 884736]
+
+
+def test_bcv_layout_is_the_index_formula_of_fig_1():
+    """PAPER.md:280-286 (Fig. 1): batch i_b = floor(beta / b) holds b_i vectors of all nodes contiguously, the vector index
+    innermost: element (J, beta) sits at ndof * b * i_b + J * b_i + beta mod b.  Checked element by element with a
+    ragged last batch; b >= nvec is the plain [ndof][nvec] layout; the inverse restores X."""
+    ndof, nvec = 7, 11
+    X = np.arange(ndof * nvec, dtype=np.float64).reshape(ndof, nvec)
+    for b in (1, 2, 4, 8, 11, 16):
+        flat = orc.to_bcv(X, b)
+        assert flat.shape == (ndof * nvec,)
+        for J in range(ndof):
+            for beta in range(nvec):
+                ib = beta // b
+                bi = min(b, nvec - ib * b)
+                assert flat[ndof * b * ib + J * bi + beta % b] == X[J, beta]
+        assert np.array_equal(orc.from_bcv(flat, ndof, nvec, b), X)
+    assert np.array_equal(orc.to_bcv(X, 16), X.reshape(-1))
