@@ -44,6 +44,7 @@ struct Guard {
 constexpr int kThreads = 256;
 constexpr int kVecBlock = 32;
 
+// [device-code-begin]  (tests/test_host_emulation.py compiles the lines up to the end marker for the host and runs them on threads)
 struct SetArrays {
   const long long* m_ptr; const long long* s_ptr; const long long* w_ptr;
   const long long* masters; const long long* slaves;
@@ -91,6 +92,8 @@ __global__ void fe_constraints_transpose_kernel(SetArrays A, double* V, int nvec
     V[A.slaves[s0 + s] * (long long)nvec + v0 + beta] = 0.0;
   }
 }
+
+// [device-code-end]
 
 template <typename T>
 cudaError_t upload(T*& dst, const T* src, size_t count) {
