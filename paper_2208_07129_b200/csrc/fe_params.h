@@ -36,7 +36,7 @@ struct ApplyParams {
                                   // (general kernel, and the Cartesian kernels instantiated with EIG)
 };
 
-#if defined(__CUDACC__)
+#if defined(__CUDACC__) || defined(FE_HOST_EMULATION)   // FE_HOST_EMULATION: tests/host/shim (device code on host threads)
 // the z planes that the Dirichlet constraint masks (the physical boundary; a cut plane of a slab is not one)
 __host__ __device__ inline bool fe_z_masked(const ApplyParams& P, int iz) {
   return (iz == 0 && !(P.zopen & 1)) || (iz == P.ndz - 1 && !(P.zopen & 2));

@@ -17,9 +17,17 @@ inline thread_local EmulDim3 blockIdx, threadIdx, blockDim, gridDim;
 inline std::barrier<>* emul_barrier = nullptr;
 inline std::mutex emul_atomic_mutex;
 
+#define FE_HOST_EMULATION 1
 #define __global__
 #define __device__
 #define __host__
+#define __constant__
+#define __shared__                       // "extern __shared__ double smem[]" becomes a plain extern array the test program defines
+#define __forceinline__ inline
+#define __launch_bounds__(...)
+#define __grid_constant__
+template <typename T>
+inline T __ldg(const T* p) { return *p; }
 #define __syncthreads() emul_barrier->arrive_and_wait()
 using std::min;
 using std::max;

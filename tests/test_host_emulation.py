@@ -42,3 +42,113 @@ def test_stream_kernels_on_host_threads(tmp_path):
     assert len(rows) == 8 * 5
     for name, count, bad in rows:
         assert int(bad) == 0, (name, count, bad)
+
+
+# ---- the apply kernels that need neither TMA nor inline PTX, against the oracle -------------------------------------
+import numpy as np  # noqa: E402
+
+from oracle import dd_oracle as ddo  # noqa: E402
+from oracle import fe_oracle as orc  # noqa: E402
+from paper_2208_07129_b200 import inputs  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def emul_apply(tmp_path_factory):
+    tmp = tmp_path_factory.mktemp("emul_apply")
+    exe = str(tmp / "emul_apply")
+    subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-ffp-contract=off", "-Wno-unknown-pragmas", "-I", os.path.join(HOST, "shim"),
+                    "-o", exe, os.path.join(HOST, "emul_apply.cpp")], check=True)
+
+    def run(kernel, p, nc, bc, zopen, geom_mode, nvec, sigma, lo, hi, X, verts=None):
+        xf, yf, vf = str(tmp / "x.bin"), str(tmp / "y.bin"), str(tmp / "v.bin")
+        np.ascontiguousarray(X, dtype=np.float64).tofile(xf)
+        cmd = [exe, kernel, str(p), *map(str, nc), str(bc), str(zopen), str(geom_mode), str(nvec), repr(float(sigma)),
+               *[repr(float(v)) for v in lo], *[repr(float(v)) for v in hi], xf, yf]
+        if verts is not None:
+            np.ascontiguousarray(verts, dtype=np.float64).tofile(vf)
+            cmd.append(vf)
+        subprocess.run(cmd, check=True, timeout=600)
+        return np.fromfile(yf, dtype=np.float64).reshape(-1, nvec)
+
+    return run
+
+
+def _relerr(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def _sheared_vertices(nc, lo, hi):
+    """Vertices of an AFFINE image of the uniform grid (parallelepiped cells: J constant, full symmetric metric)."""
+    g = [np.linspace(lo[d], hi[d], nc[d] + 1) for d in range(3)]
+    Z, Yc, Xc = np.meshgrid(g[2], g[1], g[0], indexing="ij")
+    A = np.array([[1.0, 0.25, -0.1], [0.05, 0.9, 0.2], [-0.15, 0.1, 1.1]])
+    pts = np.stack([Xc, Yc, Z], axis=-1) @ A.T
+    return pts                                                    # [(ncz+1)][(ncy+1)][(ncx+1)][3]
+
+
+GENERAL_CASES = [
+    # p, cells, bc, geometry, nvec
+    (2, (2, 3, 2), "periodic", "box", 3),          # bv = 2: a vector tail
+    (3, (2, 2, 3), "dirichlet", "box", 5),
+    (2, (3, 2, 2), "periodic", "perturbed", 2),    # per-q-point metric (config 3's recipe)
+    (3, (2, 2, 2), "dirichlet", "perturbed", 1),
+    (2, (2, 2, 3), "dirichlet", "sheared", 4),     # per-cell constant, full symmetric metric
+    (5, (2, 2, 2), "periodic", "box", 2),
+]
+
+
+@pytest.mark.parametrize("p,nc,bc,geometry,nvec", GENERAL_CASES)
+def test_general_kernel_on_host_threads_matches_the_oracle(emul_apply, p, nc, bc, geometry, nvec):
+    lo, hi, sigma = (0.0, -1.0, 0.5), (1.0, 0.5, 2.0), 0.7
+    verts, mode = None, 0
+    if geometry == "perturbed":
+        verts, mode = inputs.perturbed_vertices(nc, lo, hi, 0.12, 77 + p), 2
+    elif geometry == "sheared":
+        verts, mode = _sheared_vertices(nc, lo, hi), 1
+    mesh = orc.Mesh(nc, p, bc, lo, hi, vertices=verts)
+    X = inputs.multivector(500 + p, mesh.ndof, nvec)
+    Y = emul_apply("general", p, nc, 0 if bc == "periodic" else 1, 0, mode, nvec, sigma, lo, hi, X, verts)
+    assert _relerr(Y, orc.Operator(mesh, sigma).apply(X)) <= 1e-12
+
+
+CART_CASES = [
+    # kernel, p, cells, bc, nvec
+    ("cart", 2, (2, 3, 2), "periodic", 8),
+    ("cart", 3, (2, 2, 3), "dirichlet", 11),       # a tail block of 3 vectors; even n: padded x-lines
+    ("cart", 4, (3, 2, 2), "periodic", 5),
+    ("cart", 5, (2, 2, 2), "dirichlet", 8),        # NT = TASKS / 2: two tasks per thread
+    ("cart", 6, (2, 2, 2), "periodic", 9),
+    ("cells", 3, (5, 2, 2), "periodic", 1),        # 8 cells of an x-row per block, ragged last group
+    ("cells", 4, (5, 2, 2), "dirichlet", 2),
+    ("cells", 6, (3, 2, 2), "periodic", 3),        # 2 cells x 3 vectors per block, 2 idle slots
+]
+
+
+@pytest.mark.parametrize("kernel,p,nc,bc,nvec", CART_CASES)
+def test_even_odd_cartesian_kernel_on_host_threads_matches_the_oracle(emul_apply, kernel, p, nc, bc, nvec):
+    """Also a check of the even-odd half tables of csrc/fe_eo_tables.h (Ns, Ns^T, Ds^T Ds / 2) end to end."""
+    lo, hi, sigma = (0.0, 0.0, 0.0), (1.0, 1.5, 0.8), 0.6
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    X = inputs.multivector(600 + p, mesh.ndof, nvec)
+    Y = emul_apply(kernel, p, nc, 0 if bc == "periodic" else 1, 0, 0, nvec, sigma, lo, hi, X)
+    assert _relerr(Y, orc.Operator(mesh, sigma).apply(X)) <= 1e-12
+
+
+@pytest.mark.parametrize("kernel,nvec", [("general", 3), ("cart", 8), ("cells", 2)])
+@pytest.mark.parametrize("bc", ["periodic", "dirichlet"])
+def test_slab_flags_of_the_fallback_kernels_on_host_threads(emul_apply, kernel, nvec, bc):
+    """NEXT-4: z_open bits (cut planes: no Dirichlet mask, no periodic wrap in z) in the kernels that mask through
+    fe_z_masked, against the oracle's local operator of every task of a 3-slab decomposition."""
+    p, nc, lo, hi, sigma = 3, (2, 2, 4), (0.0, 0.0, 0.0), (1.0, 1.0, 2.0), 0.9
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    op = orc.Operator(mesh, sigma)
+    X = inputs.multivector(700, mesh.ndof, nvec)
+    hz = (hi[2] - lo[2]) / nc[2]
+    layers = ddo.slab_layers(nc[2], 3)
+    for t, (z0, z1) in enumerate(layers):
+        rows, _ = ddo.slab_rows(mesh, z0, z1)
+        U = X[rows].copy()
+        zopen = 3 if bc == "periodic" else ((1 if t > 0 else 0) | (2 if t < len(layers) - 1 else 0))
+        Y = emul_apply(kernel, p, (nc[0], nc[1], z1 - z0), 0 if bc == "periodic" else 1, zopen, 0, nvec, sigma,
+                       (lo[0], lo[1], lo[2] + hz * z0), (hi[0], hi[1], lo[2] + hz * z1), U)
+        assert _relerr(Y, ddo.slab_apply(op, z0, z1, U)) <= 1e-12, (t, zopen)
