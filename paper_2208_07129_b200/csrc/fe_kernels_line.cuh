@@ -38,7 +38,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
 
   if (tid == 0) {
     mbar_init(bar, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_init_fence();
   }
   if (PADX) {   // the pad node of every x-row of the result tile is reduced into Z too: it must stay zero
     for (int e = tid; e < N * N * BV; e += NT) B[(e / BV) * TL::XP + N * BV + e % BV] = 0.0;
@@ -57,7 +57,7 @@ fe_apply_cart_line(const __grid_constant__ CUtensorMap tmW, const __grid_constan
   // items are handed out dynamically after the first one (co-resident blocks do not run at the same speed)
   for (; item < nitems; rot = (rot + 1) & 3) {
     unsigned nxt_raw = 0;
-    if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
+    if (tid == 0) nxt_raw = item_counter_next(P.item_ctr);
     const int rot_tid = ROTATE ? ((((tid >> 5) + NW - rot) % NW) << 5) + (tid & 31) : tid;
     const int vb = (item + P.item0) % P.nvb, cell = (item + P.item0) / P.nvb;
     const int ex = cell % P.ncx, ey = (cell / P.ncx) % P.ncy, ez = cell / (P.ncx * P.ncy);

@@ -191,7 +191,7 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
   if (tma) {
     if (tid == 0) {
       mbar_init(&bar, 1);
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      mbar_init_fence();
       mbar_expect_tx(&bar, TOT * 8);
       tma_load_4d(B0, &tmW, &bar, v0, ex * PDEG, ey * PDEG, ez * PDEG);
     }

@@ -206,7 +206,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
   const double g2x = 2.0 * P.ug[0], g2y = 2.0 * P.ug[3], g4y = 4.0 * P.ug[3], g4z = 4.0 * P.ug[5], gm = P.ug[6];
   if (tid == 0) {
     mbar_init(bar, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_init_fence();
   }
   __syncthreads();
   int item = blockIdx.x;
@@ -230,7 +230,7 @@ fe_apply_cart_plane(const __grid_constant__ CUtensorMap tmW, const __grid_consta
     // the next item: consumed later, latency hidden (asm volatile: the compiler must not schedule anything that
     // depends on the result up here)
     unsigned nxt_raw = 0;
-    if (tid == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(nxt_raw) : "l"(P.item_ctr) : "memory");
+    if (tid == 0) nxt_raw = item_counter_next(P.item_ctr);
     mbar_wait(bar, parity);
     parity ^= 1u;
     if (special) {

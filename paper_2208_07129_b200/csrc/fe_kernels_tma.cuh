@@ -12,6 +12,9 @@
 
 namespace fe {
 
+// The PTX wrappers.  FE_TMA_WRAPPERS_PROVIDED: tests/host/shim/cuda.h supplies host stand-ins with the same names and
+// semantics (tests/test_host_emulation.py runs the kernels on CPU threads); never defined in a CUDA build.
+#ifndef FE_TMA_WRAPPERS_PROVIDED
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -50,6 +53,16 @@ __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commi
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// after mbar_init, before the barrier is used by the async proxy
+__device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// the dynamic item counter: returns the old value (asm volatile: the compiler must not move it, nor anything that
+// depends on the result, across the surrounding code)
+__device__ __forceinline__ unsigned item_counter_next(int* ctr) {
+  unsigned old;
+  asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
+  return old;
+}
+#endif  // FE_TMA_WRAPPERS_PROVIDED
 
 // PADX = 1: the box carries one extra node per x-row (the first node of the next cell's interior, never used).
 // With 8 vectors per block a node is 64 bytes, and for even n all x-lines of a dense tile start a multiple of
