@@ -40,22 +40,17 @@ EncodeTiledFn encode_tiled_fn() {
   return fn;
 }
 
-// 4-D FP64 tensor map of a multivector [z][y][x][beta] with box (bv, n, n, n).
-// Dirichlet meshes (Cartesian kernels): trim = 2 -> the map covers nodes 1 .. nd-2 in every direction, origin at
-// node (1,1,1), so that boundary nodes are out of bounds (zero on load; box coordinates shift by -1); trim = 1 ->
-// nodes 0 .. nd-2, origin unchanged (the last node is clipped on reduce).
+// 4-D FP64 tensor map of a multivector [z][y][x][beta] with box (bv, n, n, n): the numbers come from fe::tensor_map_desc
+// (fe_params.h: trimming for Dirichlet meshes, cut planes of slabs, the pad node of the 8-vector line kernels)
 bool make_tensor_map(CUtensorMap* tm, const fe_mf_ctx* c, const void* base, int nvec, int bv, int trim = 0, int padx = 0) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
-  if (trim && (c->ndx < 3 || c->ndy < 3 || c->ndz < 3)) return false;
-  // nodes dropped at the low / high end of each direction; a cut plane of a slab (NEXT-4) is not a boundary
-  const int lo = (trim == 2) ? 1 : 0, hi = trim ? 1 : 0;
-  const int loz = (c->zopen & 1) ? 0 : lo, hiz = (c->zopen & 2) ? 0 : hi;
-  const cuuint64_t dims[4] = {(cuuint64_t)nvec, (cuuint64_t)(c->ndx - lo - hi), (cuuint64_t)(c->ndy - lo - hi), (cuuint64_t)(c->ndz - loz - hiz)};
-  const cuuint64_t strides[3] = {(cuuint64_t)nvec * 8, (cuuint64_t)nvec * 8 * c->ndx, (cuuint64_t)nvec * 8 * c->ndx * c->ndy};
-  if (strides[2] >= ((cuuint64_t)1 << 40)) return false;
-  base = (const char*)base + (lo * strides[0] + lo * strides[1] + loz * strides[2]);
-  const cuuint32_t box[4] = {(cuuint32_t)bv, (cuuint32_t)(c->n + padx), (cuuint32_t)c->n, (cuuint32_t)c->n};
+  fe::TensorMapDesc d;
+  if (!fe::tensor_map_desc(d, c->ndx, c->ndy, c->ndz, c->n, c->zopen, nvec, bv, trim, padx)) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)d.dims[0], (cuuint64_t)d.dims[1], (cuuint64_t)d.dims[2], (cuuint64_t)d.dims[3]};
+  const cuuint64_t strides[3] = {(cuuint64_t)d.strides[0], (cuuint64_t)d.strides[1], (cuuint64_t)d.strides[2]};
+  base = (const char*)base + d.base_offset;
+  const cuuint32_t box[4] = {(cuuint32_t)d.box[0], (cuuint32_t)d.box[1], (cuuint32_t)d.box[2], (cuuint32_t)d.box[3]};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,

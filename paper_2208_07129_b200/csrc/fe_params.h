@@ -43,6 +43,35 @@ __host__ __device__ inline bool fe_z_masked(const ApplyParams& P, int iz) {
 }
 #endif
 
+// The 4-D FP64 tensor map of a multivector [z][y][x][beta] with box (bv, n + padx, n, n), as plain numbers (host code
+// hands them to cuTensorMapEncodeTiled: fe_dispatch.cu make_tensor_map).
+// Dirichlet meshes (Cartesian kernels): trim = 2 -> the map covers nodes 1 .. nd-2 in every direction, origin at
+// node (1,1,1), so that boundary nodes are out of bounds (zero on load; box coordinates shift by -1); trim = 1 ->
+// nodes 0 .. nd-2, origin unchanged (the last node is clipped on reduce).  A cut plane of a slab (zopen, NEXT-4) is not
+// a boundary: nothing is dropped there.
+struct TensorMapDesc {
+  unsigned long long base_offset;   // bytes from the multivector's first element to the map's origin
+  unsigned long long dims[4];       // elements: beta, x, y, z
+  unsigned long long strides[3];    // bytes: x, y, z
+  unsigned box[4];
+};
+inline bool tensor_map_desc(TensorMapDesc& d, int ndx, int ndy, int ndz, int n, int zopen, int nvec, int bv, int trim, int padx) {
+  if (trim && (ndx < 3 || ndy < 3 || ndz < 3)) return false;
+  const int lo = (trim == 2) ? 1 : 0, hi = trim ? 1 : 0;   // nodes dropped at the low / high end of each direction
+  const int loz = (zopen & 1) ? 0 : lo, hiz = (zopen & 2) ? 0 : hi;
+  d.dims[0] = (unsigned long long)nvec;
+  d.dims[1] = (unsigned long long)(ndx - lo - hi);
+  d.dims[2] = (unsigned long long)(ndy - lo - hi);
+  d.dims[3] = (unsigned long long)(ndz - loz - hiz);
+  d.strides[0] = (unsigned long long)nvec * 8;
+  d.strides[1] = (unsigned long long)nvec * 8 * ndx;
+  d.strides[2] = (unsigned long long)nvec * 8 * ndx * ndy;
+  if (d.strides[2] >= (1ULL << 40)) return false;
+  d.base_offset = lo * d.strides[0] + lo * d.strides[1] + loz * d.strides[2];
+  d.box[0] = (unsigned)bv; d.box[1] = (unsigned)(n + padx); d.box[2] = (unsigned)n; d.box[3] = (unsigned)n;
+  return true;
+}
+
 // n_q != n_p Gauss points per direction
 struct OiParams {
   int nq;                     // Gauss points per direction

@@ -26,6 +26,7 @@ inline std::mutex emul_atomic_mutex;
 #define __forceinline__ inline
 #define __launch_bounds__(...)
 #define __grid_constant__
+#define __align__(n)                     // the test program defines the shared-memory array with the alignment
 template <typename T>
 inline T __ldg(const T* p) { return *p; }
 #define __syncthreads() emul_barrier->arrive_and_wait()

@@ -52,14 +52,15 @@ from oracle import fe_oracle as orc  # noqa: E402
 from paper_2208_07129_b200 import inputs  # noqa: E402
 
 
-@pytest.fixture(scope="module")
-def emul_apply(tmp_path_factory):
-    tmp = tmp_path_factory.mktemp("emul_apply")
-    exe = str(tmp / "emul_apply")
+def _emulator(tmp_path_factory, name):
+    """Compile tests/host/<name>.cpp against the shim; return run(kernel, ..., **options) -> Y [ndof][nvec].  Options
+    (tests/host/emul_common.h): idw=float, layers="l0:l1", kappa=array, dscale=array."""
+    tmp = tmp_path_factory.mktemp(name)
+    exe = str(tmp / name)
     subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-ffp-contract=off", "-Wno-unknown-pragmas", "-I", os.path.join(HOST, "shim"),
-                    "-o", exe, os.path.join(HOST, "emul_apply.cpp")], check=True)
+                    "-o", exe, os.path.join(HOST, name + ".cpp")], check=True)
 
-    def run(kernel, p, nc, bc, zopen, geom_mode, nvec, sigma, lo, hi, X, verts=None):
+    def run(kernel, p, nc, bc, zopen, geom_mode, nvec, sigma, lo, hi, X, verts=None, **options):
         xf, yf, vf = str(tmp / "x.bin"), str(tmp / "y.bin"), str(tmp / "v.bin")
         np.ascontiguousarray(X, dtype=np.float64).tofile(xf)
         cmd = [exe, kernel, str(p), *map(str, nc), str(bc), str(zopen), str(geom_mode), str(nvec), repr(float(sigma)),
@@ -67,10 +68,30 @@ def emul_apply(tmp_path_factory):
         if verts is not None:
             np.ascontiguousarray(verts, dtype=np.float64).tofile(vf)
             cmd.append(vf)
-        subprocess.run(cmd, check=True, timeout=600)
+        else:
+            cmd.append("-")
+        for key, val in options.items():
+            if isinstance(val, np.ndarray):
+                f = str(tmp / (key + ".bin"))
+                np.ascontiguousarray(val, dtype=np.float64).tofile(f)
+                cmd.append(f"{key}={f}")
+            else:
+                cmd.append(f"{key}={val}")
+        res = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+        assert res.returncode == 0, (res.returncode, res.stderr)
         return np.fromfile(yf, dtype=np.float64).reshape(-1, nvec)
 
     return run
+
+
+@pytest.fixture(scope="module")
+def emul_apply(tmp_path_factory):
+    return _emulator(tmp_path_factory, "emul_apply")
+
+
+@pytest.fixture(scope="module")
+def emul_tma(tmp_path_factory):
+    return _emulator(tmp_path_factory, "emul_tma")
 
 
 def _relerr(a, b):
@@ -152,3 +173,150 @@ def test_slab_flags_of_the_fallback_kernels_on_host_threads(emul_apply, kernel, 
         Y = emul_apply(kernel, p, (nc[0], nc[1], z1 - z0), 0 if bc == "periodic" else 1, zopen, 0, nvec, sigma,
                        (lo[0], lo[1], lo[2] + hz * z0), (hi[0], hi[1], lo[2] + hz * z1), U)
         assert _relerr(Y, ddo.slab_apply(op, z0, z1, U)) <= 1e-12, (t, zopen)
+
+
+# ---- the persistent TMA kernels (plane, line, full metric) from their exact source ----------------------------------
+# tests/host/shim/cuda.h: CUtensorMap as plain numbers (from the product's fe::tensor_map_desc), bulk tensor load with zero
+# fill, bulk tensor reduce-add with clipping (aborts on a negative start coordinate or a misaligned tile, as the device
+# faults), mbarrier phases with expected bytes, the dynamic item counter.
+
+TMA_CASES = [
+    # kernel, p, cells, bc, nvec, idw
+    ("plane", 6, (2, 2, 2), "periodic", 16, 0.0),
+    ("plane", 6, (2, 3, 2), "dirichlet", 32, 0.0),       # interior input map, trimmed output map, low-face zeroing
+    ("plane", 6, (2, 2, 2), "periodic", 28, -0.7),       # vector tail of 12; identity term (the Chebyshev step's -c I)
+    ("line16", 2, (3, 2, 2), "dirichlet", 20, 0.0),
+    ("line16", 5, (2, 2, 2), "periodic", 16, 0.0),
+    ("line16", 6, (2, 2, 2), "dirichlet", 16, 0.0),
+    ("line8", 3, (2, 2, 3), "periodic", 6, 0.0),         # even n with 8-vector blocks: the pad node per x-row
+    ("line8", 4, (2, 2, 2), "periodic", 8, 1.3),
+    ("line8", 7, (2, 2, 2), "dirichlet", 8, 0.0),        # config 4's kernel
+]
+
+
+@pytest.mark.parametrize("kernel,p,nc,bc,nvec,idw", TMA_CASES)
+def test_cartesian_tma_kernels_on_host_threads_match_the_oracle(emul_tma, kernel, p, nc, bc, nvec, idw):
+    lo, hi, sigma = (0.0, 0.0, 0.0), (1.0, 1.5, 0.8), 0.6
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    X = inputs.multivector(800 + p, mesh.ndof, nvec)
+    Y = emul_tma(kernel, p, nc, 0 if bc == "periodic" else 1, 0, 0, nvec, sigma, lo, hi, X, idw=idw)
+    assert _relerr(Y, orc.Operator(mesh, sigma).apply(X) + idw * X) <= 1e-12
+
+
+GEN_CASES = [
+    # p, cells, bc, geometry, nvec
+    (2, (2, 3, 2), "periodic", "box", 4),                # a Cartesian mesh on the full-metric kernel (variant 7)
+    (3, (2, 2, 3), "dirichlet", "box", 6),
+    (2, (3, 2, 2), "periodic", "perturbed", 8),
+    (3, (2, 2, 2), "dirichlet", "perturbed", 2),
+    (5, (2, 2, 2), "periodic", "perturbed", 10),
+    (3, (2, 2, 2), "periodic", "sheared", 4),            # one full symmetric metric per cell
+    (8, (2, 2, 2), "periodic", "perturbed", 6),          # config 3's kernel: 4-vector blocks, 192 threads, a tail of 2
+]
+
+
+@pytest.mark.parametrize("p,nc,bc,geometry,nvec", GEN_CASES)
+def test_full_metric_tma_kernel_on_host_threads_matches_the_oracle(emul_tma, p, nc, bc, geometry, nvec):
+    lo, hi, sigma = (0.0, -1.0, 0.5), (1.0, 0.5, 2.0), 0.7
+    verts, mode = None, 0
+    if geometry == "perturbed":
+        verts, mode = inputs.perturbed_vertices(nc, lo, hi, 0.12, 77 + p), 2
+    elif geometry == "sheared":
+        verts, mode = _sheared_vertices(nc, lo, hi), 1
+    mesh = orc.Mesh(nc, p, bc, lo, hi, vertices=verts)
+    X = inputs.multivector(500 + p, mesh.ndof, nvec)
+    Y = emul_tma("gen", p, nc, 0 if bc == "periodic" else 1, 0, mode, nvec, sigma, lo, hi, X, verts)
+    assert _relerr(Y, orc.Operator(mesh, sigma).apply(X)) <= 1e-12
+
+
+@pytest.mark.parametrize("kernel,p,nvec", [("plane", 6, 16), ("line16", 5, 16), ("line8", 3, 8), ("gen", 3, 4)])
+@pytest.mark.parametrize("bc", ["periodic", "dirichlet"])
+def test_slab_flags_of_the_tma_kernels_on_host_threads(emul_tma, kernel, p, nvec, bc):
+    """NEXT-4: the z_open bits in the tensor maps (per-direction trimming), the low-face zeroing, the wrap fix-ups:
+    every task of a 3-slab decomposition against the oracle's local operator."""
+    nc, lo, hi, sigma = (2, 2, 4), (0.0, 0.0, 0.0), (1.0, 1.0, 2.0), 0.9
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    op = orc.Operator(mesh, sigma)
+    X = inputs.multivector(700, mesh.ndof, nvec)
+    hz = (hi[2] - lo[2]) / nc[2]
+    layers = ddo.slab_layers(nc[2], 3)
+    for t, (z0, z1) in enumerate(layers):
+        rows, _ = ddo.slab_rows(mesh, z0, z1)
+        U = X[rows].copy()
+        zopen = 3 if bc == "periodic" else ((1 if t > 0 else 0) | (2 if t < len(layers) - 1 else 0))
+        Y = emul_tma(kernel, p, (nc[0], nc[1], z1 - z0), 0 if bc == "periodic" else 1, zopen, 0, nvec, sigma,
+                     (lo[0], lo[1], lo[2] + hz * z0), (hi[0], hi[1], lo[2] + hz * z1), U)
+        assert _relerr(Y, ddo.slab_apply(op, z0, z1, U)) <= 1e-12, (t, zopen)
+
+
+EIG_CASES = [
+    # kernel, p, cells, bc, nvec, idw
+    ("plane", 6, (2, 2, 2), "periodic", 16, 0.0),
+    ("plane", 6, (2, 2, 3), "dirichlet", 16, 0.0),
+    ("plane", 6, (2, 2, 2), "periodic", 16, -0.4),       # the filter step on H~: EIG + identity term
+    ("line8", 4, (2, 3, 2), "periodic", 8, 0.0),
+    ("line16", 5, (2, 2, 2), "dirichlet", 16, 0.0),
+    ("line8", 7, (2, 2, 2), "periodic", 4, 0.9),
+]
+
+
+@pytest.mark.parametrize("kernel,p,nc,bc,nvec,idw", EIG_CASES)
+def test_eigenproblem_operator_on_the_cartesian_tma_kernels_on_host_threads(emul_tma, kernel, p, nc, bc, nvec, idw):
+    """NEXT-1: H~ = M^-1/2 (K + M^kappa) M^-1/2 on a uniform box: kappa per quadrature point, the mass
+    scaling inside the interpolation tables (MAT_NSS of csrc/fe_eo_tables.h) and in the metric constants."""
+    lo, hi = (0.0, 0.0, 0.0), (1.0, 1.5, 0.8)
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    X = inputs.multivector(900 + p, mesh.ndof, nvec)
+    kap = np.asarray(inputs.kappa_points(1234 + p, int(np.prod(nc)), (p + 1) ** 3))
+    d = 1.0 / np.sqrt(orc.lumped_mass_diagonal(mesh))
+    Y = emul_tma(kernel, p, nc, 0 if bc == "periodic" else 1, 0, 0, nvec, 0.0, lo, hi, X, kappa=kap, dscale=d, idw=idw)
+    assert _relerr(Y, orc.Operator(mesh, 0.0, kappa=kap).apply_mass_scaled(X, d) + idw * X) <= 1e-12
+
+
+@pytest.mark.parametrize("program,kernel,p,nc,bc,nvec", [("tma", "gen", 3, (2, 2, 2), "periodic", 4), ("tma", "gen", 2, (2, 3, 2), "dirichlet", 6),
+                                                         ("apply", "general", 3, (2, 2, 2), "periodic", 3)])
+def test_mass_scaled_operator_on_a_perturbed_mesh_on_host_threads(emul_tma, emul_apply, program, kernel, p, nc, bc, nvec):
+    """d = diag(M)^-1/2 applied at extraction and assembly by the full-metric kernels."""
+    lo, hi, sigma = (0.0, -1.0, 0.5), (1.0, 0.5, 2.0), 0.7
+    verts = inputs.perturbed_vertices(nc, lo, hi, 0.12, 77 + p)
+    mesh = orc.Mesh(nc, p, bc, lo, hi, vertices=verts)
+    X = inputs.multivector(500 + p, mesh.ndof, nvec)
+    d = 1.0 / np.sqrt(orc.lumped_mass_diagonal(mesh))
+    run = emul_tma if program == "tma" else emul_apply
+    Y = run(kernel, p, nc, 0 if bc == "periodic" else 1, 0, 2, nvec, sigma, lo, hi, X, verts, dscale=d)
+    assert _relerr(Y, orc.Operator(mesh, sigma).apply_mass_scaled(X, d)) <= 1e-12
+
+
+def test_kappa_on_a_uniform_box_on_the_general_kernel_on_host_threads(emul_apply):
+    """kappa(x) without mass scaling runs on fe_apply_general (pick_kernel): the mass factor is det J * kappa_Q."""
+    p, nc, lo, hi, nvec = 3, (2, 2, 2), (0.0, 0.0, 0.0), (1.0, 1.5, 0.8), 3
+    mesh = orc.Mesh(nc, p, "periodic", lo, hi)
+    X = inputs.multivector(960, mesh.ndof, nvec)
+    kap = np.asarray(inputs.kappa_points(4321, int(np.prod(nc)), (p + 1) ** 3))
+    Y = emul_apply("general", p, nc, 0, 0, 0, nvec, 0.0, lo, hi, X, kappa=kap)
+    assert _relerr(Y, orc.Operator(mesh, 0.0, kappa=kap).apply(X)) <= 1e-12
+
+
+@pytest.mark.parametrize("kernel,p,nc,bc,nvec", [("plane", 6, (2, 2, 4), "dirichlet", 16), ("line8", 3, (2, 2, 5), "periodic", 8),
+                                                ("gen", 3, (2, 2, 4), "periodic", 4)])
+def test_item_ranges_of_the_persistent_kernels_on_host_threads(emul_tma, kernel, p, nc, bc, nvec):
+    """fe_mf_apply_host's z-slab pipeline launches the persistent kernels on a RANGE of cell layers (item0, item_count):
+    the result is the sum of the contributions of exactly those cells (oracle: the same cells, one by one)."""
+    lo, hi, sigma, l0, l1 = (0.0, 0.0, 0.0), (1.0, 1.5, 0.8), 0.6, 1, 3
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    op = orc.Operator(mesh, sigma)
+    X = inputs.multivector(950 + p, mesh.ndof, nvec)
+    Y = emul_tma(kernel, p, nc, 0 if bc == "periodic" else 1, 0, 0, nvec, sigma, lo, hi, X, layers=f"{l0}:{l1}")
+    Yo = np.zeros_like(X)
+    for ez in range(l0, l1):
+        for ey in range(nc[1]):
+            for ex in range(nc[0]):
+                idx, mask = mesh.cell_dofs(ex, ey, ez)
+                U = X[idx].copy()
+                if mask is not None:
+                    U[mask] = 0.0
+                W = op.cell_apply(ex, ey, ez, U)
+                if mask is not None:
+                    W[mask] = 0.0
+                np.add.at(Yo, idx, W)
+    assert _relerr(Y, Yo) <= 1e-12
