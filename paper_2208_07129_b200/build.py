@@ -24,7 +24,7 @@ HOST_DEPS = ["fe_ctx.h", "fe_params.h", FE_MF_H]
 KERNEL_DEPS = HOST_DEPS + ["fe_kernels.cuh", "fe_kernels_eo.cuh", "fe_kernels_cart2.cuh", "fe_kernels_tma.cuh"]
 # translation unit -> the files it depends on (besides itself)
 UNITS = {
-    "fe_mf.cu": HOST_DEPS + ["fe_tables.h", "fe_eo_tables.h"],
+    "fe_mf.cu": HOST_DEPS + ["fe_tables.h", "fe_eo_tables.h", "fe_oi_tables.h"],
     "fe_dispatch.cu": HOST_DEPS,
     "fe_probe.cu": [FE_MF_H],
     "fe_constraints.cu": [os.path.join("..", "..", "include", "fe_constraints.h"), FE_MF_H],

@@ -11,6 +11,7 @@
 #include "fe_ctx.h"
 #include "fe_tables.h"
 #include "fe_eo_tables.h"
+#include "fe_oi_tables.h"
 
 static thread_local std::string g_create_err = "";
 
@@ -283,27 +284,12 @@ extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
   }
   if (!ctx->nq_oi) return FE_MF_OK;
   const int n = ctx->n;
-  // tables of the nq-point rule in long double: N[q][i] = l_i(xq_q) on the GLL nodes, D~ on the quadrature points
-  long double xi[16], xq[16], w[16], c[16];
-  fe::gll_nodes(ctx->p, xi);
-  fe::gauss_legendre(nq, xq, w);
-  std::vector<double> hN((size_t)nq * n), hD((size_t)nq * nq), hw(nq);
-  for (int q = 0; q < nq; ++q) {
-    hw[q] = (double)w[q];
-    for (int i = 0; i < n; ++i) {
-      long double v = 1.0L;
-      for (int j = 0; j < n; ++j) if (j != i) v *= (xq[q] - xi[j]) / (xi[i] - xi[j]);
-      hN[(size_t)q * n + i] = (double)v;
-    }
-  }
-  for (int r = 0; r < nq; ++r) { c[r] = 1.0L; for (int j = 0; j < nq; ++j) if (j != r) c[r] *= (xq[r] - xq[j]); }
-  for (int q = 0; q < nq; ++q)
-    for (int r = 0; r < nq; ++r) {
-      long double v = 0.0L;
-      if (q != r) v = (c[q] / c[r]) / (xq[q] - xq[r]);
-      else for (int j = 0; j < nq; ++j) if (j != q) v += 1.0L / (xq[q] - xq[j]);
-      hD[(size_t)q * nq + r] = (double)v;
-    }
+  // tables of the nq-point rule (fe_oi_tables.h): N[q][i] = l_i(xq_q) on the GLL nodes, D~ on the quadrature points
+  fe_host::OiTables oit;
+  try { fe_host::make_oi_tables(ctx->p, nq, oit); }
+  catch (...) { ctx->nq_oi = 0; return fail(ctx, FE_MF_ENOMEM, "out of host memory (quadrature tables)"); }
+  const std::vector<double>&hN = oit.N, &hD = oit.D, &hw = oit.w;
+  const long double* xq = oit.xq;
   auto upload = [&](double** dst, const std::vector<double>& src) {
     if (cudaMalloc(dst, src.size() * sizeof(double)) != cudaSuccess) { *dst = nullptr; return false; }
     return cudaMemcpy(*dst, src.data(), src.size() * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess;
@@ -312,24 +298,8 @@ extern "C" int fe_mf_set_quadrature(fe_mf_ctx* ctx, int nq) {
     ctx->nq_oi = 0;
     return fail(ctx, FE_MF_ENOMEM, "table upload failed (quadrature)");
   }
-  if (nq == ctx->p + 3) {   // the compile-time kernel of n_q = n_p + 2 reads its tables from constant memory
-    // even / odd halves [Ne | No | De | Do] (layout: fe_kernels.cuh, c_oi), halved in long double from the symmetrised pair
-    std::vector<double> pack;
-    auto halves = [&](const std::vector<double>& M, int R, int C, double sgn) {
-      const int hR = (R + 1) / 2, hC = (C + 1) / 2;
-      for (int part = 0; part < 2; ++part)
-        for (int o = 0; o < hR; ++o)
-          for (int i = 0; i < hC; ++i) {
-            // the centro-(anti)symmetry is enforced exactly: entry (o, i) is averaged with its image (R-1-o, C-1-i)
-            const long double a = 0.5L * ((long double)M[(size_t)o * C + i] + sgn * (long double)M[(size_t)(R - 1 - o) * C + (C - 1 - i)]);
-            const long double b = 0.5L * ((long double)M[(size_t)o * C + (C - 1 - i)] + sgn * (long double)M[(size_t)(R - 1 - o) * C + i]);
-            pack.push_back((double)(part == 0 ? 0.5L * (a + b) : 0.5L * (a - b)));
-          }
-    };
-    halves(hN, nq, n, 1.0);
-    halves(hD, nq, nq, -1.0);
-    FE_CUDA(ctx, fe_host::upload_tables_oi(pack.data(), pack.size(), (size_t)fe::oi_offset(ctx->p)));
-  }
+  if (nq == ctx->p + 3)   // the compile-time kernel of n_q = n_p + 2 reads its tables (even / odd halves) from constant memory
+    FE_CUDA(ctx, fe_host::upload_tables_oi(oit.pack.data(), oit.pack.size(), (size_t)fe::oi_offset(ctx->p)));
   if (ctx->geom_mode == 2) {   // per-point metric at the nq^3 points (Eq. 7c evaluated at every point of the rule)
     const size_t nn = (size_t)nq * nq * nq;
     ctx->oi_geom_stride = (long long)(7 * nn);

@@ -7,6 +7,7 @@
 //          kappa=FILE     kappa at the quadrature points [cell][n^3] of a uniform box (fe_mf_set_kappa); sigma is then unused
 //          dscale=FILE    d = diag(M)^-1/2 [ndof] (fe_mf_set_mass_scaling): Z = d.(A (d.W)); on a uniform box with kappa the
 //                         Cartesian TMA kernels run their EIG instantiation instead (d inside the tables)
+//          nq=N           N Gauss points per direction instead of p + 1 (emul_oi.cpp; fe_mf_set_quadrature)
 //          layers=l0:l1   only the cells of layers l0 <= ez < l1 (the item ranges of fe_mf_apply_host's z-slab pipeline)
 #pragma once
 #include <cstdio>
@@ -25,7 +26,7 @@ struct EmulSetup {
   int ndx, ndy, ndz;
   long long ndof, ncells;
   double sigma, idw = 0.0, detj0 = 1.0;
-  int layer0 = 0, layer1 = -1;
+  int layer0 = 0, layer1 = -1, nq = 0;
   std::vector<double> X, Y, verts, G, kappa, dscale;
   fe::Tables1D tab;
   fe::EoTab eo[5];
@@ -56,6 +57,7 @@ inline void emul_setup(EmulSetup& s, int argc, char** argv) {
     if (kv.rfind("idw=", 0) == 0) s.idw = atof(kv.c_str() + 4);
     else if (kv.rfind("kappa=", 0) == 0) kappa_path = kv.substr(6);
     else if (kv.rfind("dscale=", 0) == 0) dscale_path = kv.substr(7);
+    else if (kv.rfind("nq=", 0) == 0) s.nq = atoi(kv.c_str() + 3);
     else if (kv.rfind("layers=", 0) == 0) { if (sscanf(kv.c_str() + 7, "%d:%d", &s.layer0, &s.layer1) != 2) exit(2); }
     else { fprintf(stderr, "unknown option %s\n", kv.c_str()); exit(2); }
   }
@@ -69,7 +71,8 @@ inline void emul_setup(EmulSetup& s, int argc, char** argv) {
   s.X = emul_read_bin(argv[17], (size_t)s.ndof * s.nvec);
   s.Y.assign((size_t)s.ndof * s.nvec, 0.0);
   if (s.geom_mode != 0) s.verts = emul_read_bin(argv[19], (size_t)3 * (ncx + 1) * (ncy + 1) * (ncz + 1));
-  if (!kappa_path.empty()) s.kappa = emul_read_bin(kappa_path.c_str(), (size_t)nn * s.ncells);
+  const size_t npts = s.nq ? (size_t)s.nq * s.nq * s.nq : (size_t)nn;   // points per cell of the rule in force
+  if (!kappa_path.empty()) s.kappa = emul_read_bin(kappa_path.c_str(), npts * s.ncells);
   if (!dscale_path.empty()) s.dscale = emul_read_bin(dscale_path.c_str(), (size_t)s.ndof);
   s.tab = fe::make_tables(p);
   fe_host::make_eo_tables(s.tab, s.eo, s.eo2);

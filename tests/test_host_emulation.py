@@ -320,3 +320,45 @@ def test_item_ranges_of_the_persistent_kernels_on_host_threads(emul_tma, kernel,
                     W[mask] = 0.0
                 np.add.at(Yo, idx, W)
     assert _relerr(Y, Yo) <= 1e-12
+
+
+# ---- n_q != n_p Gauss points per direction (NEXT-2) ------------------------------------------------------------------
+
+@pytest.fixture(scope="module")
+def emul_oi(tmp_path_factory):
+    return _emulator(tmp_path_factory, "emul_oi")
+
+
+OI_CASES = [
+    # kernel, p, nq, cells, bc, geometry, nvec
+    ("oi", 2, 5, (2, 3, 2), "periodic", "box", 4),
+    ("oi", 3, 6, (2, 2, 2), "dirichlet", "perturbed", 6),
+    ("oi", 4, 7, (2, 2, 2), "periodic", "perturbed", 5),        # odd nvec: a half-empty last block
+    ("oi", 6, 9, (2, 2, 2), "periodic", "perturbed", 2),        # config 2's degree with the paper's n_q = n_p + 2
+    ("general_oi", 3, 5, (2, 2, 2), "periodic", "perturbed", 3),
+    ("general_oi", 2, 7, (2, 2, 3), "dirichlet", "perturbed", 1),
+    ("general_oi", 4, 7, (2, 2, 2), "periodic", "box", 1),      # n_q = n_p + 2 with one vector: the run-time kernel
+]
+
+
+@pytest.mark.parametrize("kernel,p,nq,nc,bc,geometry,nvec", OI_CASES)
+def test_overintegration_kernels_on_host_threads_match_the_oracle(emul_oi, kernel, p, nq, nc, bc, geometry, nvec):
+    """Rectangular tables from csrc/fe_oi_tables.h (N: n_q x n_p, the collocation derivative on the n_q points, their even /
+    odd halves), per-point geometry at the n_q^3 points; fe_apply_oi in its loads / atomics mode."""
+    lo, hi, sigma = (0.0, -1.0, 0.5), (1.0, 0.5, 2.0), 0.7
+    verts, mode = None, 0
+    if geometry == "perturbed":
+        verts, mode = inputs.perturbed_vertices(nc, lo, hi, 0.12, 77 + p), 2
+    mesh = orc.Mesh(nc, p, bc, lo, hi, vertices=verts)
+    X = inputs.multivector(500 + p, mesh.ndof, nvec)
+    Y = emul_oi(kernel, p, nc, 0 if bc == "periodic" else 1, 0, mode, nvec, sigma, lo, hi, X, verts, nq=nq)
+    assert _relerr(Y, orc.Operator(mesh, sigma, nq=nq).apply(X)) <= 1e-12
+
+
+def test_kappa_at_the_points_of_the_larger_rule_on_host_threads(emul_oi):
+    p, nq, nc, nvec, lo, hi = 3, 6, (2, 2, 2), 4, (0.0, 0.0, 0.0), (1.0, 1.5, 0.8)
+    mesh = orc.Mesh(nc, p, "periodic", lo, hi)
+    X = inputs.multivector(77, mesh.ndof, nvec)
+    kap = np.asarray(inputs.kappa_points(99, 8, nq ** 3))
+    Y = emul_oi("oi", p, nc, 0, 0, 0, nvec, 0.0, lo, hi, X, nq=nq, kappa=kap)
+    assert _relerr(Y, orc.Operator(mesh, 0.0, kappa=kap, nq=nq).apply(X)) <= 1e-12
