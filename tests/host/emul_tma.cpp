@@ -94,12 +94,17 @@ int main(int argc, char** argv) {
   bool ok = true;
   // block sizes: PlaneCfg (fe_tu_plane.cu), LineCfg (fe_tu_line16.cu, fe_tu_line8.cu), GenCfg (fe_tu_gen.cu)
   if (s.kernel == "plane" && p == 6) run_plane(s);
+  else if (s.kernel == "line16" && p == 1) run_line_i<1, 16, 32>(s);
   else if (s.kernel == "line16" && p == 2) run_line_i<2, 16, 96>(s);
+  else if (s.kernel == "line16" && p == 3) run_line_i<3, 16, 128>(s);
   else if (s.kernel == "line16" && p == 5) run_line_i<5, 16, 160>(s);
   else if (s.kernel == "line16" && p == 6) run_line_i<6, 16, 256>(s);
+  else if (s.kernel == "line8" && p == 1) run_line_i<1, 8, 32>(s);
+  else if (s.kernel == "line8" && p == 2) run_line_i<2, 8, 64>(s);
   else if (s.kernel == "line8" && p == 3) run_line_i<3, 8, 64>(s);
   else if (s.kernel == "line8" && p == 4) run_line_i<4, 8, 128>(s);
   else if (s.kernel == "line8" && p == 7) run_line_i<7, 8, 128>(s);
+  else if (s.kernel == "gen" && p == 1) run_gen<1, 8, 32>(s);
   else if (s.kernel == "gen" && p == 2) run_gen<2, 8, 64>(s);
   else if (s.kernel == "gen" && p == 3) run_gen<3, 8, 64>(s);
   else if (s.kernel == "gen" && p == 5) run_gen<5, 8, 160>(s);

@@ -362,3 +362,38 @@ def test_kappa_at_the_points_of_the_larger_rule_on_host_threads(emul_oi):
     kap = np.asarray(inputs.kappa_points(99, 8, nq ** 3))
     Y = emul_oi("oi", p, nc, 0, 0, 0, nvec, 0.0, lo, hi, X, nq=nq, kappa=kap)
     assert _relerr(Y, orc.Operator(mesh, 0.0, kappa=kap, nq=nq).apply(X)) <= 1e-12
+
+
+def test_seeded_random_configurations_on_host_threads(emul_tma, emul_apply):
+    """40 seeded random small configurations over all kernel families (degree, 1-3 cells per direction incl. one-cell-thick
+    Dirichlet meshes, vector counts with and without tails, identity term): the oracle at 1e-12, and none of the aborts
+    of the stand-ins (a reduction that starts at a negative coordinate, a misaligned tile)."""
+    import random
+    rnd = random.Random(20240807)
+    lo, hi, sigma = (0.0, 0.0, 0.0), (1.0, 1.3, 0.7), 0.6
+    degrees = {"plane": [6], "line16": [1, 2, 3, 5, 6], "line8": [1, 2, 3, 4, 7], "gen": [1, 2, 3, 5],
+               "cart": [1, 2, 3, 4, 5, 6], "cells": [1, 2, 3, 4, 6], "general": [1, 2, 3, 4]}
+    for case in range(40):
+        kernel = rnd.choice(sorted(degrees))
+        p = rnd.choice(degrees[kernel])
+        bc = rnd.choice(["periodic", "dirichlet"])
+        nc = tuple(rnd.randint(2 if bc == "periodic" else 1, 3) for _ in range(3))
+        if bc == "dirichlet" and p == 1 and kernel in ("plane", "line16", "line8"):
+            nc = tuple(max(c, 2) for c in nc)              # the trimmed maps need >= 3 nodes per direction (else pick_kernel takes kind 2)
+        if kernel == "cells":
+            nvec = rnd.choice([1, 2, 3])
+        elif kernel in ("general", "cart"):
+            nvec = rnd.choice([1, 2, 3, 5, 8, 9, 11])
+        else:
+            nvec = rnd.choice([2, 4, 6, 8, 10, 14, 16, 18, 20]) if p < 5 else rnd.choice([2, 6, 8, 12, 16])
+        idw = rnd.uniform(-1, 1) if kernel in ("plane", "line16", "line8") and bc == "periodic" and rnd.random() < 0.3 else 0.0
+        mesh = orc.Mesh(nc, p, bc, lo, hi)
+        X = inputs.multivector(3000 + case, mesh.ndof, nvec)
+        run = emul_tma if kernel in ("plane", "line16", "line8", "gen") else emul_apply
+        Y = run(kernel, p, nc, 0 if bc == "periodic" else 1, 0, 0, nvec, sigma, lo, hi, X, **({"idw": idw} if idw else {}))
+        Yo = orc.Operator(mesh, sigma).apply(X) + idw * X
+        scale = np.abs(Yo).max()
+        if scale == 0.0:                                   # every node on the Dirichlet boundary
+            assert np.all(Y == 0.0), (case, kernel, p, nc, bc, nvec)
+        else:
+            assert np.abs(Y - Yo).max() <= 1e-12 * scale, (case, kernel, p, nc, bc, nvec, idw)
