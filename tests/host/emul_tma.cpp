@@ -44,6 +44,7 @@ static void launch(EmulSetup& s, int bv, int nt, size_t smem_bytes, bool cartesi
   const unsigned grid = (unsigned)(nitems < 3 ? nitems : 3);
   const fe::ApplyParams P = s.P;
   emul_launch(grid, 1, (unsigned)nt, [&] { kernel(tw, tz, P, (int)nitems); });
+  fe::emul_check_nothing_pending();
 }
 
 // IDENT / EIG instantiations are chosen the way launch_plane / launch_line_p do: EIG if kappa is set, IDENT if idw != 0

@@ -52,12 +52,12 @@ from oracle import fe_oracle as orc  # noqa: E402
 from paper_2208_07129_b200 import inputs  # noqa: E402
 
 
-def _emulator(tmp_path_factory, name):
+def _emulator(tmp_path_factory, name, flags=()):
     """Compile tests/host/<name>.cpp against the shim; return run(kernel, ..., **options) -> Y [ndof][nvec].  Options
     (tests/host/emul_common.h): idw=float, layers="l0:l1", kappa=array, dscale=array."""
     tmp = tmp_path_factory.mktemp(name)
     exe = str(tmp / name)
-    subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-ffp-contract=off", "-Wno-unknown-pragmas", "-I", os.path.join(HOST, "shim"),
+    subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-ffp-contract=off", "-Wno-unknown-pragmas", *flags, "-I", os.path.join(HOST, "shim"),
                     "-o", exe, os.path.join(HOST, name + ".cpp")], check=True)
 
     def run(kernel, p, nc, bc, zopen, geom_mode, nvec, sigma, lo, hi, X, verts=None, **options):
@@ -89,9 +89,11 @@ def emul_apply(tmp_path_factory):
     return _emulator(tmp_path_factory, "emul_apply")
 
 
-@pytest.fixture(scope="module")
-def emul_tma(tmp_path_factory):
-    return _emulator(tmp_path_factory, "emul_tma")
+@pytest.fixture(scope="module", params=["copies_at_issue", "copies_as_late_as_allowed"])
+def emul_tma(tmp_path_factory, request):
+    """Both legal extremes of the asynchronous bulk copies (tests/host/shim/cuda.h): at issue, and as late as the kernel's
+    own waits allow (-DFE_EMUL_LAZY_TMA): a missing mbarrier wait or bulk-group wait makes the second one go wrong."""
+    return _emulator(tmp_path_factory, "emul_tma", ["-DFE_EMUL_LAZY_TMA"] if request.param == "copies_as_late_as_allowed" else [])
 
 
 def _relerr(a, b):
