@@ -28,6 +28,10 @@ on their way back -- is rounded to IEEE binary32 (round to nearest even) and wid
 stays FP64.  A single task exchanges nothing, so nothing is rounded.  Pins: the deviation from the exact apply lives
 only in the cell layer under a cut plane, on the cut plane itself it is the rounding error of the exact ghost row when
 U is FP32-representable, and it is of the size of the FP32 unit roundoff.
+
+dd_chebyshev_filter: the filter recurrence of fe_oracle.chebyshev_filter with the decomposed apply as its operator.  Pins:
+equal to the single-domain filter for every slab count (1e-12: m steps of summation-order differences, amplified by the
+filter's growth outside [a, b]); with the FP32 payload the deviation stays at the FP32 level times that growth.
 """
 from __future__ import annotations
 
@@ -117,3 +121,14 @@ def dd_apply(op, X: np.ndarray, nslabs: int, exchange_ghosts: bool = True, halo_
         else:
             np.add.at(V, rows[:n_owned], V_loc[:n_owned])
     return V
+
+
+def dd_chebyshev_filter(op, X: np.ndarray, nslabs: int, m: int, a: float, b: float, a0: float,
+                        fp32_payload: bool = False) -> np.ndarray:
+    """The Chebyshev filter (Alg. 6 l.2-17) with EVERY operator application evaluated in decomposed
+    form, V = sum_t P^(t)T A^(t) P^(t) U (the paper's multi-GPU eigenproblem runs): the recurrence is
+    fe_oracle.chebyshev_filter's, line by line; only the operator is replaced.  Without the FP32 payload this equals the
+    single-domain filter up to summation order (pinned in tests/test_oracle_dd.py); with it every step's boundary planes are
+    rounded to binary32 on their way across a cut."""
+    from .fe_oracle import chebyshev_filter
+    return chebyshev_filter(lambda V: dd_apply(op, V, nslabs, fp32_payload=fp32_payload), X, m, a, b, a0)

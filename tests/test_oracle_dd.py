@@ -122,3 +122,25 @@ def test_fp32_payload_deviates_only_under_the_cut_planes(bc):
         bnd = (ix == 0) | (ix == mesh.nd[0] - 1) | (iy == 0) | (iy == mesh.nd[1] - 1) | (iz == 0) | (iz == ndz - 1)
         rows = (ix + mesh.nd[0] * (iy + mesh.nd[1] * iz))[bnd]
         assert np.all(ddo.dd_apply(op, X, ns, fp32_payload=True)[rows] == 0.0)
+
+
+@pytest.mark.parametrize("bc", ["periodic", "dirichlet"])
+def test_decomposed_chebyshev_filter_is_the_single_domain_filter(bc):
+    """Alg. 6 with the decomposed operator: the same polynomial of the same matrix, whatever the number of tasks.  The
+    spectrum bound comes from the oracle's Lanczos; [a, b] covers the upper 60 % of the spectrum (damped), the scaled
+    filter is 1 at a0."""
+    p, nc, m = 3, (2, 2, 4), 7
+    mesh = orc.Mesh(nc, p, bc, (0.0, 0.0, 0.0), (1.0, 1.2, 2.0))
+    op = orc.Operator(mesh, 0.7)
+    X = inputs.multivector(91, mesh.ndof, 3)
+    b = orc.lanczos_upper_bound(op.apply, inputs.uniform_pm1(92, 0, mesh.ndof), 10)
+    a, a0 = 0.4 * b, 0.0
+    Y = orc.chebyshev_filter(op.apply, X, m, a, b, a0)
+    assert np.abs(Y - X).max() > 0.1 * np.abs(X).max()                  # the filter does something
+    for ns in (1, 2, 4):
+        Yd = ddo.dd_chebyshev_filter(op, X, ns, m, a, b, a0)
+        assert np.abs(Yd - Y).max() <= 1e-12 * np.abs(Y).max(), ns
+    Y32 = ddo.dd_chebyshev_filter(op, X, 2, m, a, b, a0, fp32_payload=True)
+    dev = np.abs(Y32 - Y).max() / np.abs(Y).max()
+    assert 1e-10 < dev < 1e-4                                           # FP32 roundoff per step, not FP64, not O(1)
+    assert np.array_equal(ddo.dd_chebyshev_filter(op, X, 1, m, a, b, a0, fp32_payload=True), ddo.dd_chebyshev_filter(op, X, 1, m, a, b, a0))
