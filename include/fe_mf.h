@@ -87,7 +87,12 @@ int fe_mf_create(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double sigma
  *   sending side; unpack on the receiving side: dst_dev[k] = (double) src_dev[k] (add = 0: ghost values of U) or
  *   dst_dev[k] += (double) src_dev[k] (add = 1: ghost rows of V).  DEVICE pointers, count elements, stream-ordered;
  *   dst and src must not overlap.  Everything a task computes stays FP64: only the message is FP32 (half the bytes).
- * Errors of the three halo calls: EINVAL (null pointer, count < 0, add not 0 / 1), ECUDA (launch failure).
+ * fe_mf_axpby: Z_dev[k] = beta Z_dev[k] + gamma W_dev[k], k < count (DEVICE pointers, 8-byte aligned is enough, stream-ordered;
+ *   beta == 0: Z is not read and may hold anything).  The owned-rows update of a decomposed Chebyshev step
+ *   (Alg. 6 l.15: X <- alpha1 V + alpha2 X - c alpha1 Y with V = the decomposed product, dd.py), which a slab
+ *   context cannot fuse into its kernel because the ghost rows of V first travel to their owner.  Z and W must not overlap
+ *   unless they are the same pointer.
+ * Errors of the halo calls and fe_mf_axpby: EINVAL (null pointer, count < 0, add not 0 / 1), ECUDA (launch failure).
  * The exchange itself is point-to-point (two neighbours per slab): paper_2208_07129_b200/dd.py drives it with
  * torch.distributed send / recv (NCCL between GPUs; the plane to send is a contiguous block of the multivector).
  */
@@ -95,6 +100,7 @@ int fe_mf_create_slab(fe_mf_ctx **out, int ncx, int ncy, int ncz, int p, double 
                       const double box_lo[3], const double box_hi[3], const double *vertices_host, int z_open,
                       int cuda_device);
 int fe_mf_halo_add(double *dst_dev, const double *src_dev, long long count, void *cuda_stream);
+int fe_mf_axpby(double *Z_dev, const double *W_dev, double beta, double gamma, long long count, void *cuda_stream);
 int fe_mf_halo_pack_f32(float *dst_dev, const double *src_dev, long long count, void *cuda_stream);
 int fe_mf_halo_unpack_f32(double *dst_dev, const float *src_dev, long long count, int add, void *cuda_stream);
 

@@ -28,6 +28,7 @@ SYMBOLS = {
     "fe_mf_create_slab": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int, _D, C.c_int, C.c_int,
                                     _PD, _PD, C.c_void_p, C.c_int, C.c_int]),
     "fe_mf_halo_add": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]),
+    "fe_mf_axpby": (C.c_int, [C.c_void_p, C.c_void_p, _D, _D, C.c_longlong, C.c_void_p]),
     "fe_mf_halo_pack_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]),
     "fe_mf_halo_unpack_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, C.c_void_p]),
     "fe_mf_ndofs": (C.c_longlong, [C.c_void_p]),
@@ -235,6 +236,18 @@ def halo_add(dst, src, stream=None):
     if rc != FE_MF_OK:
         raise FeMfError(rc, "fe_mf_halo_add failed")
     return dst
+
+
+def axpby(Z, W, beta: float, gamma: float, stream=None):
+    """Z <- beta Z + gamma W on the device (fe_mf_axpby)."""
+    import torch
+    assert isinstance(Z, torch.Tensor) and Z.is_cuda and Z.dtype == torch.float64 and Z.is_contiguous()
+    assert isinstance(W, torch.Tensor) and W.is_cuda and W.dtype == torch.float64 and W.is_contiguous()
+    assert Z.numel() == W.numel()
+    rc = lib().fe_mf_axpby(Z.data_ptr(), W.data_ptr(), float(beta), float(gamma), Z.numel(), _stream_ptr(stream))
+    if rc != FE_MF_OK:
+        raise FeMfError(rc, "fe_mf_axpby failed")
+    return Z
 
 
 def halo_pack_f32(dst, src, stream=None):

@@ -534,6 +534,16 @@ extern "C" int fe_mf_halo_add(double* dst_dev, const double* src_dev, long long 
   return fe_host::launch_axpby(dst_dev, src_dev, 1.0, 1.0, (size_t)count, (cudaStream_t)cuda_stream) == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
 }
 
+extern "C" int fe_mf_axpby(double* Z_dev, const double* W_dev, double beta, double gamma, long long count, void* cuda_stream) {
+  if (!Z_dev || !W_dev || count < 0) return FE_MF_EINVAL;
+  if (count == 0) return FE_MF_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // beta == 0: Z is not read (it may hold anything, NaN included)
+  const cudaError_t e = (beta == 0.0) ? fe_host::launch_scale_copy(Z_dev, W_dev, gamma, (size_t)count, st)
+                                      : fe_host::launch_axpby(Z_dev, W_dev, beta, gamma, (size_t)count, st);
+  return e == cudaSuccess ? FE_MF_OK : FE_MF_ECUDA;
+}
+
 extern "C" int fe_mf_halo_pack_f32(float* dst_dev, const double* src_dev, long long count, void* cuda_stream) {
   if (!dst_dev || !src_dev || count < 0) return FE_MF_EINVAL;
   if (count == 0) return FE_MF_OK;

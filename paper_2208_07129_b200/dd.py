@@ -17,6 +17,9 @@ is recast as FP32 floats"): fe_mf_halo_pack_f32 on the sending side into a messa
 fe_mf_halo_unpack_f32 on the receiving side (overwrite for U, add for V); everything a task computes stays FP64.  A
 single task exchanges nothing, so nothing is rounded.
 
+dd_cheb_filter_rank / SlabGroup.cheb_filter: the Chebyshev filter (Alg. 6) on a decomposed mesh -- every product by the
+exchange above, the three-term update of the owned rows by fe_mf_axpby; the host evaluates the scalar recurrence.
+
 This module is argument marshalling and message ordering only; the arithmetic is in libfe_mf.so.  The local operator
 and the halo add are injected (`ops`), so that the message pattern can be exercised without a GPU (tests/
 test_dd_gloo.py runs it over gloo with the CPU oracle standing in for the two device calls).
@@ -104,12 +107,13 @@ def slab_geometry(w, plan: SlabPlan):
 
 @dataclass
 class LocalOps:
-    """The device calls of a task: V_loc = A^(t) U_loc; dst += src; and, for the FP32 payload only, pack_f32(dst32, src64)
-    and unpack_f32(dst64, src32, add)."""
+    """The device calls of a task: V_loc = A^(t) U_loc; dst += src; for the FP32 payload only, pack_f32(dst32, src64)
+    and unpack_f32(dst64, src32, add); for the Chebyshev filter only, axpby(Z, W, beta, gamma): Z <- beta Z + gamma W."""
     apply: Callable
     halo_add: Callable
     pack_f32: Optional[Callable] = None
     unpack_f32: Optional[Callable] = None
+    axpby: Optional[Callable] = None
 
 
 def device_ops(w, plan: SlabPlan, device: int = 0):
@@ -118,7 +122,7 @@ def device_ops(w, plan: SlabPlan, device: int = 0):
     nc, lo, hi, verts = slab_geometry(w, plan)
     op = binding.FeMf(nc, w.p, w.sigma, w.bc, w.geom, lo, hi, verts, device, z_open=plan.z_open)
     return LocalOps(apply=lambda U, V, nvec: op.apply(U, V, nvec), halo_add=binding.halo_add,
-                    pack_f32=binding.halo_pack_f32, unpack_f32=binding.halo_unpack_f32), op
+                    pack_f32=binding.halo_pack_f32, unpack_f32=binding.halo_unpack_f32, axpby=binding.axpby), op
 
 
 def _buffers32(like, pe: int, count: int):
@@ -239,6 +243,53 @@ def dd_apply_rank_batches(plan: SlabPlan, ops: LocalOps, U_list, V_list, nvec: i
     return V_list
 
 
+def cheb_steps(m: int, a: float, b: float, a0: float):
+    """The scalars of Alg. 6 l.2-16 (reading 10), in the paper's order and names: yields, for
+    the first step, ("first", alpha1, alpha1 * alpha2) -- Y <- alpha1 A X + alpha1 alpha2 X -- and for every step
+    d = 2..m ("step", alpha1, alpha2, -c alpha1) -- X <- alpha1 A Y + alpha2 X - c alpha1 Y, then swap."""
+    if m < 1 or not (b > a) or not (a0 < a):
+        raise ValueError("need m >= 1, b > a, a0 < a")
+    e = (b - a) / 2.0
+    c = (b + a) / 2.0
+    sigma = e / (a0 - c)
+    sigma1 = sigma
+    gamma = 2.0 / sigma1
+    alpha1 = sigma1 / e
+    alpha2 = -c
+    yield ("first", alpha1, alpha1 * alpha2)
+    for _ in range(2, m + 1):
+        sigma2 = 1.0 / (gamma - sigma)
+        alpha1 = 2.0 * sigma2 / e
+        alpha2 = -sigma * sigma2
+        yield ("step", alpha1, alpha2, -(c * alpha1))
+        sigma = sigma2
+
+
+def dd_cheb_filter_rank(plan: SlabPlan, ops: LocalOps, X_loc, Y_loc, V_loc, nvec: int, m: int, a: float, b: float, a0: float,
+                        dist, fp32_payload: bool = False):
+    """One task of the Chebyshev filter on a decomposed mesh (the paper's multi-GPU eigenproblem runs):
+    Alg. 6 l.2-17 with every product V = A U evaluated by dd_apply_rank (ghost exchange, fused local kernels, halo add)
+    and the three-term update applied to the OWNED rows by fe_mf_axpby -- a slab context cannot fuse it into the kernel,
+    because the ghost rows of V first travel to their owner.  X_loc / Y_loc / V_loc: local multivectors (owned planes +
+    ghost plane; the ghost planes are scratch).  Returns (filtered block, iterate m - 1): the same two buffers, possibly
+    exchanged (the paper's swap(X, Y), is an exchange of references here)."""
+    own = plan.n_owned_planes * plan.plane_nodes * nvec
+    X, Y = X_loc, Y_loc
+    for step in cheb_steps(m, a, b, a0):
+        if step[0] == "first":
+            _, a1, a1a2 = step
+            dd_apply_rank(plan, ops, X, V_loc, nvec, dist, fp32_payload=fp32_payload)
+            ops.axpby(Y[:own], V_loc[:own], 0.0, a1)
+            ops.axpby(Y[:own], X[:own], 1.0, a1a2)
+        else:
+            _, a1, a2, mca1 = step
+            dd_apply_rank(plan, ops, Y, V_loc, nvec, dist, fp32_payload=fp32_payload)
+            ops.axpby(X[:own], V_loc[:own], a2, a1)
+            ops.axpby(X[:own], Y[:own], 1.0, mca1)
+            X, Y = Y, X
+    return Y, X
+
+
 class SlabGroup:
     """All tasks of a decomposed mesh in ONE process on one device: the messages become device copies.  This is the
     form the path takes on a single GPU (tests, bench); with one process per GPU use dd_apply_rank."""
@@ -306,3 +357,24 @@ class SlabGroup:
                 else:
                     self.ops[pl.up].halo_add(V_locs[pl.up][:pe], V[own:own + pe])
         return V_locs
+
+    def cheb_filter(self, X_locs, Y_locs, V_locs, nvec: int, m: int, a: float, b: float, a0: float, fp32_payload: bool = False):
+        """dd_cheb_filter_rank for all tasks of the group.  Returns (filtered blocks, iterates m - 1): the two lists of
+        buffers, possibly exchanged."""
+        owns = [pl.n_owned_planes * pl.plane_nodes * nvec for pl in self.plans]
+        X, Y = X_locs, Y_locs
+        for step in cheb_steps(m, a, b, a0):
+            if step[0] == "first":
+                _, a1, a1a2 = step
+                self.apply(X, V_locs, nvec, fp32_payload=fp32_payload)
+                for o, own, x, y, v in zip(self.ops, owns, X, Y, V_locs):
+                    o.axpby(y[:own], v[:own], 0.0, a1)
+                    o.axpby(y[:own], x[:own], 1.0, a1a2)
+            else:
+                _, a1, a2, mca1 = step
+                self.apply(Y, V_locs, nvec, fp32_payload=fp32_payload)
+                for o, own, x, y, v in zip(self.ops, owns, X, Y, V_locs):
+                    o.axpby(x[:own], v[:own], a2, a1)
+                    o.axpby(x[:own], y[:own], 1.0, mca1)
+                X, Y = Y, X
+        return Y, X

@@ -36,8 +36,11 @@ def _oracle_ops(w, plan):
     def unpack_f32(dst, src, add):
         return dst.add_(src.double()) if add else dst.copy_(src.double())
 
+    def axpby(Z, W, beta, gamma):
+        return Z.copy_(gamma * W) if beta == 0.0 else Z.mul_(beta).add_(W, alpha=gamma)
+
     return dd.LocalOps(apply=apply, halo_add=lambda dst, src: dst.add_(src),
-                       pack_f32=lambda dst, src: dst.copy_(src.to(torch.float32)), unpack_f32=unpack_f32)
+                       pack_f32=lambda dst, src: dst.copy_(src.to(torch.float32)), unpack_f32=unpack_f32, axpby=axpby)
 
 
 def _worker_batches(rank, world, port, bc, q, fp32=False):
@@ -172,3 +175,96 @@ def test_plan_bookkeeping():
                     assert pl.up == (t + 1 if t < ns - 1 else None) and pl.down == (t - 1 if t > 0 else None)
                     assert pl.has_ghost == (t < ns - 1)
     assert dd.slab_layers(7, 3) == [(0, 3), (3, 5), (5, 7)]
+
+
+# ---- the Chebyshev filter on a decomposed mesh ----------------------------------------------------------------------
+
+def _filter_interval(w):
+    bcs = "periodic" if w.bc == inputs.BC_PERIODIC else "dirichlet"
+    op = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma)
+    b = orc.lanczos_upper_bound(op.apply, inputs.uniform_pm1(w.seed + 1, 0, w.ndof), 10)
+    return op, 0.4 * b, b, 0.0
+
+
+def _worker_cheb(rank, world, port, bc, m, fp32, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = _workload(bc)
+        nvec = w.nvec
+        _, a, b, a0 = _filter_interval(w)
+        plan = dd.make_plan(w.ncells, w.p, bc == inputs.BC_PERIODIC, world, rank)
+        pe = plan.plane_nodes * nvec
+        first = plan.z0 * plan.p
+        Xg = inputs.multivector(w.seed, w.ndof, nvec)
+        X = torch.full((plan.nplanes * pe,), float("nan"), dtype=torch.float64)
+        X[:plan.n_owned_planes * pe] = torch.from_numpy(Xg.reshape(-1)[first * pe:(first + plan.n_owned_planes) * pe].copy())
+        Y = torch.full_like(X, float("nan")); V = torch.full_like(X, float("nan"))
+        res, prev = dd.dd_cheb_filter_rank(plan, _oracle_ops(w, plan), X, Y, V, nvec, m, a, b, a0, dist, fp32_payload=fp32)
+        assert {res.data_ptr(), prev.data_ptr()} == {X.data_ptr(), Y.data_ptr()}
+        q.put((rank, plan.z0, plan.n_owned_planes, res[:plan.n_owned_planes * pe].numpy().copy()))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("bc,m,fp32", [(inputs.BC_PERIODIC, 4, False), (inputs.BC_DIRICHLET, 5, False), (inputs.BC_PERIODIC, 3, True)])
+def test_decomposed_chebyshev_filter_over_gloo(bc, m, fp32):
+    """world 2: Alg. 6 with every product through the point-to-point exchange; odd and even m (the result ends in either
+    buffer); the FP32 payload against the oracle that rounds the same planes in every step."""
+    world = 2
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker_cheb, args=(r, world, port, bc, m, fp32, q)) for r in range(world)]
+    for p in procs: p.start()
+    res = sorted((q.get(timeout=300) for _ in range(world)), key=lambda r: r[0])
+    for p in procs: p.join(timeout=60)
+    assert all(p.exitcode == 0 for p in procs)
+    w = _workload(bc)
+    op, a, b, a0 = _filter_interval(w)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    Y = ddo.dd_chebyshev_filter(op, X, world, m, a, b, a0, fp32_payload=fp32)
+    if not fp32:
+        assert np.abs(Y - orc.chebyshev_filter(op.apply, X, m, a, b, a0)).max() <= 1e-12 * np.abs(Y).max()
+    plane = w.nd[0] * w.nd[1] * w.nvec
+    for rank, z0, nown, Yown in res:
+        ref = Y.reshape(-1)[z0 * w.p * plane:(z0 * w.p + nown) * plane]
+        assert np.abs(Yown - ref).max() <= 1e-12 * np.abs(Y).max(), rank
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("nslabs,m", [(1, 3), (3, 4), (5, 6)])
+def test_slab_group_chebyshev_filter_single_process(bc, nslabs, m):
+    w = _workload(bc)
+    nvec = w.nvec
+    op, a, b, a0 = _filter_interval(w)
+    grp = dd.SlabGroup(w, nslabs, make_ops=_oracle_ops)
+    X = inputs.multivector(w.seed, w.ndof, nvec)
+    Xt = torch.from_numpy(X.reshape(-1).copy())
+    Xl = grp.scatter(Xt, nvec)
+    Yl = [torch.full_like(u, float("nan")) for u in Xl]
+    Vl = [torch.full_like(u, float("nan")) for u in Xl]
+    res, prev = grp.cheb_filter(Xl, Yl, Vl, nvec, m, a, b, a0)
+    out = grp.gather(res, nvec, torch.full_like(Xt, float("nan")))
+    Y = orc.chebyshev_filter(op.apply, X, m, a, b, a0)
+    assert np.abs(out.numpy().reshape(Y.shape) - Y).max() <= 1e-12 * np.abs(Y).max()
+    # the second return value is iterate m - 1 (fe_cheb_filter's contract for X)
+    outp = grp.gather(prev, nvec, torch.full_like(Xt, float("nan")))
+    Yp = orc.chebyshev_filter(op.apply, X, m - 1, a, b, a0) if m > 1 else X
+    assert np.abs(outp.numpy().reshape(Y.shape) - Yp).max() <= 1e-12 * np.abs(Yp).max()
+
+
+def test_cheb_steps_are_algorithm_6():
+    """The scalar recurrence against the oracle's filter on a 1 x 1 'matrix' (apply = multiplication by lambda)."""
+    a, b, a0, lam = 1.0, 3.0, 0.2, 0.7
+    for m in (1, 2, 5, 8):
+        x, y = 1.0, None
+        for st in dd.cheb_steps(m, a, b, a0):
+            if st[0] == "first":
+                y = st[1] * lam * x + st[2] * x
+            else:
+                x, y = y, st[1] * lam * y + st[2] * x + st[3] * y
+        ref = orc.chebyshev_filter(lambda v: lam * v, np.array([[1.0]]), m, a, b, a0)[0, 0]
+        assert abs(y - ref) <= 1e-14 * abs(ref)
+    with pytest.raises(ValueError):
+        list(dd.cheb_steps(3, 2.0, 1.0, 0.0))
