@@ -51,6 +51,8 @@ int main(int argc, char** argv) {
     if (s.geom_mode != 0) return 4;        // the Cartesian kernel reads the uniform metric only
     if (s.kernel == "cells" && (s.nvec < 1 || s.nvec > 3)) return 4;
     emul_set_bv(s, 8);
+    for (int k = 0; k < 7; ++k) s.P.ug[k] *= s.alpha;   // launch_accumulate, kinds 2 / 3: alpha inside the metric constants,
+    s.P.alpha = 1.0;                                    // P.alpha = 1
   }
   const fe::ApplyParams& P = s.P;
   switch (p) {

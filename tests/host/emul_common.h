@@ -3,6 +3,8 @@
 // and the kernel parameters the way csrc/fe_dispatch.cu make_params does (alpha = 1).
 //   usage: PROGRAM KERNEL p ncx ncy ncz bc zopen geom_mode nvec sigma lox loy loz hix hiy hiz X.bin Y.bin [verts.bin|-] [key=value ...]
 //          bc 0 periodic / 1 Dirichlet ; geom_mode 0 uniform box, 1 per cell, 2 per q-point (1, 2 need verts.bin)
+//          alpha=c        Z += c A W instead of Z += A W (fe_mf_accumulate; the Cartesian kernels take it inside the metric constants)
+//          z0=FILE        initial contents of Z (default: zeros)
 //          idw=c          Z = A W + c W (the identity term of the Cartesian TMA kernels, periodic meshes)
 //          kappa=FILE     kappa at the quadrature points [cell][n^3] of a uniform box (fe_mf_set_kappa); sigma is then unused
 //          dscale=FILE    d = diag(M)^-1/2 [ndof] (fe_mf_set_mass_scaling): Z = d.(A (d.W)); on a uniform box with kappa the
@@ -25,7 +27,7 @@ struct EmulSetup {
   int p, n, nn, ncx, ncy, ncz, bc, zopen, geom_mode, nvec;
   int ndx, ndy, ndz;
   long long ndof, ncells;
-  double sigma, idw = 0.0, detj0 = 1.0;
+  double sigma, idw = 0.0, detj0 = 1.0, alpha = 1.0;
   int layer0 = 0, layer1 = -1, nq = 0;
   std::vector<double> X, Y, verts, G, kappa, dscale;
   fe::Tables1D tab;
@@ -51,10 +53,12 @@ inline void emul_setup(EmulSetup& s, int argc, char** argv) {
   double lo[3], hi[3], h[3];
   for (int d = 0; d < 3; ++d) { lo[d] = atof(argv[11 + d]); hi[d] = atof(argv[14 + d]); }
   s.out_path = argv[18];
-  std::string kappa_path, dscale_path;
+  std::string kappa_path, dscale_path, z0_path;
   for (int a = 20; a < argc; ++a) {
     const std::string kv = argv[a];
     if (kv.rfind("idw=", 0) == 0) s.idw = atof(kv.c_str() + 4);
+    else if (kv.rfind("alpha=", 0) == 0) s.alpha = atof(kv.c_str() + 6);
+    else if (kv.rfind("z0=", 0) == 0) z0_path = kv.substr(3);
     else if (kv.rfind("kappa=", 0) == 0) kappa_path = kv.substr(6);
     else if (kv.rfind("dscale=", 0) == 0) dscale_path = kv.substr(7);
     else if (kv.rfind("nq=", 0) == 0) s.nq = atoi(kv.c_str() + 3);
@@ -69,7 +73,8 @@ inline void emul_setup(EmulSetup& s, int argc, char** argv) {
   s.ndx = ncx * p + add; s.ndy = ncy * p + add; s.ndz = ncz * p + (s.zopen ? 1 : add);
   s.ndof = (long long)s.ndx * s.ndy * s.ndz; s.ncells = (long long)ncx * ncy * ncz;
   s.X = emul_read_bin(argv[17], (size_t)s.ndof * s.nvec);
-  s.Y.assign((size_t)s.ndof * s.nvec, 0.0);
+  if (z0_path.empty()) s.Y.assign((size_t)s.ndof * s.nvec, 0.0);
+  else s.Y = emul_read_bin(z0_path.c_str(), (size_t)s.ndof * s.nvec);
   if (s.geom_mode != 0) s.verts = emul_read_bin(argv[19], (size_t)3 * (ncx + 1) * (ncy + 1) * (ncz + 1));
   const size_t npts = s.nq ? (size_t)s.nq * s.nq * s.nq : (size_t)nn;   // points per cell of the rule in force
   if (!kappa_path.empty()) s.kappa = emul_read_bin(kappa_path.c_str(), npts * s.ncells);
@@ -132,7 +137,7 @@ inline void emul_setup(EmulSetup& s, int argc, char** argv) {
   }
   P.geom = s.G.data();
   P.W = s.X.data(); P.Z = s.Y.data();
-  P.alpha = 1.0;
+  P.alpha = s.alpha;
   P.ncx = ncx; P.ncy = ncy; P.ncz = ncz; P.ndx = s.ndx; P.ndy = s.ndy; P.ndz = s.ndz;
   P.nvec = s.nvec;
   P.dirichlet = s.bc ? 1 : 0; P.zopen = s.zopen; P.geom_mode = s.geom_mode; P.nsm = 148;

@@ -32,6 +32,8 @@ template <typename Kernel>
 static void launch(EmulSetup& s, int bv, int nt, size_t smem_bytes, bool cartesian, int padx, Kernel kernel) {
   if (smem_bytes > sizeof(fe::smem_raw) || smem_bytes > 232448) { fprintf(stderr, "shared memory %zu too large\n", smem_bytes); exit(8); }
   emul_set_bv(s, bv);
+  if (cartesian)                          // launch_accumulate, kinds 8 / 9: the result is linear in the metric constants
+    for (int k = 0; k < 7; ++k) s.P.ug[k] *= s.alpha;
   if (cartesian && !s.dscale.empty()) {   // launch_accumulate, EIG kernels: diag(M)^-1/2 = (det J)^-1/2 kron diag(w~)^-1/2, the tables carry the second factor
     for (int k = 0; k < 7; ++k) s.P.ug[k] /= s.detj0;
     s.P.dscale = nullptr;

@@ -399,3 +399,50 @@ def test_seeded_random_configurations_on_host_threads(emul_tma, emul_apply):
             assert np.all(Y == 0.0), (case, kernel, p, nc, bc, nvec)
         else:
             assert np.abs(Y - Yo).max() <= 1e-12 * scale, (case, kernel, p, nc, bc, nvec, idw)
+
+
+# ---- S9: the Chebyshev step as fe_cheb_filter composes it from accumulate launches ----------------------------------
+
+@pytest.mark.parametrize("kernel,p,nc,bc,nvec,m", [("plane", 6, (2, 2, 2), "periodic", 16, 5), ("line8", 3, (2, 3, 2), "periodic", 8, 6),
+                                                  ("line16", 5, (2, 2, 2), "dirichlet", 16, 4), ("plane", 6, (2, 2, 2), "dirichlet", 16, 3)])
+def test_chebyshev_filter_from_accumulate_launches_on_host_threads(emul_tma, kernel, p, nc, bc, nvec, m):
+    """The contract between fe_cheb_filter (csrc/fe_dispatch.cu) and the Cartesian TMA kernels, with the kernels run from
+    their exact source: Alg. 6's recurrence in the scaled variables X_k = s_k U_k is a chain of accumulate launches
+    U_{k-1} += al (A - c I) U_k, each ONE kernel launch with alpha = al and the identity term idw = -c al; on a Dirichlet
+    mesh the kernels neither read nor write boundary rows, whose entries follow the scalar recurrence q_k and are written
+    by the final scaling kernel.  The host recurrence below restates fe_cheb_filter's; the result is the oracle's filter."""
+    lo, hi, sigma = (0.0, 0.0, 0.0), (1.0, 1.5, 0.8), 0.6
+    mesh = orc.Mesh(nc, p, bc, lo, hi)
+    op = orc.Operator(mesh, sigma)
+    X0 = inputs.multivector(1700 + p, mesh.ndof, nvec)
+    b = orc.lanczos_upper_bound(op.apply, inputs.uniform_pm1(1701, 0, mesh.ndof), 10)
+    a, a0 = 0.35 * b, 0.0
+    bcode = 0 if bc == "periodic" else 1
+
+    def accumulate(al, W, Z):            # Z += al (A - c I) W in one launch
+        return emul_tma(kernel, p, nc, bcode, 0, 0, nvec, sigma, lo, hi, W, alpha=repr(al), idw=repr(-c * al), z0=Z)
+
+    e, c = (b - a) / 2.0, (b + a) / 2.0
+    sig = e / (a0 - c)
+    gamma = 2.0 / sig
+    alpha1 = sig / e
+    Uprev, Ucur = X0.copy(), accumulate(alpha1, X0, np.zeros_like(X0))
+    s_prev = s_cur = 1.0
+    q_prev, q_cur = 1.0, -c * alpha1
+    for _ in range(2, m + 1):
+        sig2 = 1.0 / (gamma - sig)
+        alpha1, alpha2 = 2.0 * sig2 / e, -sig * sig2
+        s_next = alpha2 * s_prev
+        al = alpha1 * s_cur / s_next
+        q_prev, q_cur = q_cur, -c * alpha1 * q_cur + alpha2 * q_prev
+        Uprev, Ucur = Ucur, accumulate(al, Ucur, Uprev)
+        s_prev, s_cur = s_cur, s_next
+        sig = sig2
+    Y = s_cur * Ucur
+    if bc == "dirichlet":                # fe_scale2_kernel: boundary rows still hold x0 (or 0 in the buffer that started at 0)
+        ix, iy, iz = np.meshgrid(*[np.arange(n) for n in mesh.nd], indexing="ij")
+        bnd = (ix == 0) | (ix == mesh.nd[0] - 1) | (iy == 0) | (iy == mesh.nd[1] - 1) | (iz == 0) | (iz == mesh.nd[2] - 1)
+        rows = (ix + mesh.nd[0] * (iy + mesh.nd[1] * iz))[bnd]
+        Y[rows] = q_cur * X0[rows]
+    Yo = orc.chebyshev_filter(op.apply, X0, m, a, b, a0)
+    assert _relerr(Y, Yo) <= 1e-12
