@@ -167,7 +167,7 @@ fe_apply_oi(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUt
             const OiParams O, int use_tma) {
   constexpr int N = PDEG + 1, NQ3 = NQ * NQ * NQ;
   extern __shared__ __align__(128) unsigned char smem_oi[];
-  __shared__ uint64_t bar;
+  FE_STATIC_SHARED uint64_t bar;
   double* B0 = reinterpret_cast<double*>(smem_oi);
   double* B1 = B0 + (size_t)NQ3 * bv;
   double* B2 = B1 + (size_t)NQ3 * bv;

@@ -10,6 +10,14 @@
 
 #include "fe_kernels_cart2.cuh"
 
+// A statically allocated shared-memory variable of a kernel.  (The host-thread builds of the tests define __shared__ away
+// so that "extern __shared__ T name[]" becomes a plain extern array; a static variable then needs "static" instead.)
+#ifdef FE_HOST_EMULATION
+#define FE_STATIC_SHARED static
+#else
+#define FE_STATIC_SHARED __shared__
+#endif
+
 namespace fe {
 
 // The PTX wrappers.  FE_TMA_WRAPPERS_PROVIDED: tests/host/shim/cuda.h supplies host stand-ins with the same names and

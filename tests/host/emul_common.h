@@ -168,3 +168,15 @@ inline int emul_write(const EmulSetup& s) {
   fclose(f);
   return 0;
 }
+
+#ifdef FE_TMA_WRAPPERS_PROVIDED   // programs that include tests/host/shim/cuda.h: the tensor map as the product computes its numbers
+inline CUtensorMap make_map(const EmulSetup& s, double* base, int bv, int trim, int padx) {
+  fe::TensorMapDesc d;
+  if (!fe::tensor_map_desc(d, s.ndx, s.ndy, s.ndz, s.n, s.zopen, s.nvec, bv, trim, padx)) { fprintf(stderr, "tensor_map_desc refused\n"); exit(7); }
+  CUtensorMap tm;
+  tm.base = reinterpret_cast<double*>(reinterpret_cast<char*>(base) + d.base_offset);
+  for (int k = 0; k < 4; ++k) { tm.dims[k] = d.dims[k]; tm.box[k] = d.box[k]; }
+  for (int k = 0; k < 3; ++k) tm.strides[k] = d.strides[k];
+  return tm;
+}
+#endif

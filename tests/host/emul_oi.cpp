@@ -1,9 +1,8 @@
 // Test helper: the kernels of the n_q != n_p rule -- fe_apply_oi (compile-time sizes, n_q = n_p + 2:
 // csrc/fe_kernels_oi.cuh) in its loads / atomics mode and fe_apply_general_oi (any n_q: csrc/fe_kernels.cuh) -- from their
 // exact source on CPU threads.  Tables from the product's csrc/fe_oi_tables.h, per-point geometry the way
-// fe_mf_set_quadrature builds it, launch parameters restated from csrc/fe_tu_oi.cu.  The bulk-tensor mode of fe_apply_oi is
-// not run here (its mbarrier is a static __shared__ variable, which the thread stand-in cannot share).
-//   usage: tests/host/emul_common.h ; KERNEL = oi | general_oi ; nq=N required
+// fe_mf_set_quadrature builds it, launch parameters restated from csrc/fe_tu_oi.cu and launch_accumulate (kind 11).
+//   usage: tests/host/emul_common.h ; KERNEL = oi (loads / atomics) | oi_tma (cell tile by bulk tensor copies) | general_oi ; nq=N required
 #include "../../paper_2208_07129_b200/csrc/fe_kernels_oi.cuh"
 #include "../../paper_2208_07129_b200/csrc/fe_oi_tables.h"
 #include "emul_common.h"
@@ -20,10 +19,14 @@ static void run(EmulSetup& s, const fe::OiParams& O, int bv) {
   const unsigned grid = (unsigned)(s.ncells * P.nvb);
   CUtensorMap dummy;
   std::memset(&dummy, 0, sizeof(dummy));
-  if (s.kernel == "oi") {
+  if (s.kernel == "oi" || s.kernel == "oi_tma") {
     if (O.nq != PDEG + 3 || (bv != 2 && bv != 4)) { fprintf(stderr, "the compile-time kernel needs nq = p + 3 and 2 or 4 vectors per block\n"); exit(4); }
-    if (bv == 4) emul_launch(grid, 1, 256, [&] { fe::fe_apply_oi<PDEG, PDEG + 3, 4>(dummy, dummy, P, O, 0); });
-    else emul_launch(grid, 1, 256, [&] { fe::fe_apply_oi<PDEG, PDEG + 3, 2>(dummy, dummy, P, O, 0); });
+    const int use_tma = s.kernel == "oi_tma" ? 1 : 0;
+    if (use_tma && (s.nvec & 1)) { fprintf(stderr, "the bulk-tensor mode needs an even nvec\n"); exit(4); }
+    const CUtensorMap tw = use_tma ? make_map(s, s.X.data(), bv, 0, 0) : dummy, tz = use_tma ? make_map(s, s.Y.data(), bv, 0, 0) : dummy;
+    if (bv == 4) emul_launch(grid, 1, 256, [&] { fe::fe_apply_oi<PDEG, PDEG + 3, 4>(tw, tz, P, O, use_tma); });
+    else emul_launch(grid, 1, 256, [&] { fe::fe_apply_oi<PDEG, PDEG + 3, 2>(tw, tz, P, O, use_tma); });
+    fe::emul_check_nothing_pending();
   } else {
     emul_launch(grid, 1, 256, [&] { fe::fe_apply_general_oi<PDEG>(P, O); });
   }

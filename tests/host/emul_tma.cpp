@@ -16,16 +16,6 @@ namespace fe { alignas(1024) unsigned char smem_raw[256 * 1024]; }   // the dyna
 
 static constexpr int line_padx(int p, int bv) { return ((bv == 8 || bv == 4) && (p + 1) % 2 == 0 && p >= 3) ? 1 : 0; }   // fe_ctx.h
 
-static CUtensorMap make_map(const EmulSetup& s, double* base, int bv, int trim, int padx) {
-  fe::TensorMapDesc d;
-  if (!fe::tensor_map_desc(d, s.ndx, s.ndy, s.ndz, s.n, s.zopen, s.nvec, bv, trim, padx)) { fprintf(stderr, "tensor_map_desc refused\n"); exit(7); }
-  CUtensorMap tm;
-  tm.base = reinterpret_cast<double*>(reinterpret_cast<char*>(base) + d.base_offset);
-  for (int k = 0; k < 4; ++k) { tm.dims[k] = d.dims[k]; tm.box[k] = d.box[k]; }
-  for (int k = 0; k < 3; ++k) tm.strides[k] = d.strides[k];
-  return tm;
-}
-
 static int g_item_counter = 0;
 
 template <typename Kernel>

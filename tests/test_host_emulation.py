@@ -326,9 +326,9 @@ def test_item_ranges_of_the_persistent_kernels_on_host_threads(emul_tma, kernel,
 
 # ---- n_q != n_p Gauss points per direction (NEXT-2) ------------------------------------------------------------------
 
-@pytest.fixture(scope="module")
-def emul_oi(tmp_path_factory):
-    return _emulator(tmp_path_factory, "emul_oi")
+@pytest.fixture(scope="module", params=["copies_at_issue", "copies_as_late_as_allowed"])
+def emul_oi(tmp_path_factory, request):
+    return _emulator(tmp_path_factory, "emul_oi", ["-DFE_EMUL_LAZY_TMA"] if request.param == "copies_as_late_as_allowed" else [])
 
 
 OI_CASES = [
@@ -337,6 +337,9 @@ OI_CASES = [
     ("oi", 3, 6, (2, 2, 2), "dirichlet", "perturbed", 6),
     ("oi", 4, 7, (2, 2, 2), "periodic", "perturbed", 5),        # odd nvec: a half-empty last block
     ("oi", 6, 9, (2, 2, 2), "periodic", "perturbed", 2),        # config 2's degree with the paper's n_q = n_p + 2
+    ("oi_tma", 2, 5, (2, 3, 2), "periodic", "box", 4),          # the cell tile by bulk tensor copies; wrapped nodes by loads / atomics
+    ("oi_tma", 3, 6, (2, 2, 2), "dirichlet", "perturbed", 6),   # boundary nodes zeroed in the tile
+    ("oi_tma", 6, 9, (2, 2, 2), "periodic", "perturbed", 2),
     ("general_oi", 3, 5, (2, 2, 2), "periodic", "perturbed", 3),
     ("general_oi", 2, 7, (2, 2, 3), "dirichlet", "perturbed", 1),
     ("general_oi", 4, 7, (2, 2, 2), "periodic", "box", 1),      # n_q = n_p + 2 with one vector: the run-time kernel
@@ -346,7 +349,7 @@ OI_CASES = [
 @pytest.mark.parametrize("kernel,p,nq,nc,bc,geometry,nvec", OI_CASES)
 def test_overintegration_kernels_on_host_threads_match_the_oracle(emul_oi, kernel, p, nq, nc, bc, geometry, nvec):
     """Rectangular tables from csrc/fe_oi_tables.h (N: n_q x n_p, the collocation derivative on the n_q points, their even /
-    odd halves), per-point geometry at the n_q^3 points; fe_apply_oi in its loads / atomics mode."""
+    odd halves), per-point geometry at the n_q^3 points; fe_apply_oi in both of its modes."""
     lo, hi, sigma = (0.0, -1.0, 0.5), (1.0, 0.5, 2.0), 0.7
     verts, mode = None, 0
     if geometry == "perturbed":

@@ -101,6 +101,7 @@ def test_tma_kernels_have_no_shared_memory_race(tsan, kernel, p, nc, bc, nvec, g
 @pytest.mark.parametrize("program,kernel,p,nc,bc,nvec,geometry,options",
                          [("emul_apply", "general", 3, (2, 2, 2), "periodic", 3, "perturbed", {}), ("emul_apply", "cart", 4, (2, 2, 2), "dirichlet", 11, "box", {}),
                           ("emul_apply", "cells", 3, (3, 2, 2), "periodic", 2, "box", {}), ("emul_oi", "oi", 3, (2, 2, 2), "periodic", 4, "perturbed", {"nq": 6}),
+                          ("emul_oi", "oi_tma", 3, (2, 2, 2), "periodic", 4, "perturbed", {"nq": 6}),
                           ("emul_oi", "general_oi", 2, (2, 2, 2), "dirichlet", 3, "perturbed", {"nq": 5})])
 def test_fallback_and_overintegration_kernels_have_no_shared_memory_race(tsan, program, kernel, p, nc, bc, nvec, geometry, options):
     tmp, run = tsan
