@@ -29,6 +29,10 @@ stays FP64.  A single task exchanges nothing, so nothing is rounded.  Pins: the 
 only in the cell layer under a cut plane, on the cut plane itself it is the rounding error of the exact ghost row when
 U is FP32-representable, and it is of the size of the FP32 unit roundoff.
 
+dd_constrained_apply: Eq. 17 in full, with the constraint matrices C^(t), C^(t)T of oracle/constraints_oracle.py around the
+local cell loop.  Pin: equal to C^T A C of the undecomposed mesh (constraints_oracle on the global rows around
+fe_oracle.Operator.apply) when every set lies inside one task's local rows; a set that straddles a cut is refused.
+
 dd_chebyshev_filter: the filter recurrence of fe_oracle.chebyshev_filter with the decomposed apply as its operator.  Pins:
 equal to the single-domain filter for every slab count (1e-12: m steps of summation-order differences, amplified by the
 filter's growth outside [a, b]); with the FP32 payload the deviation stays at the FP32 level times that growth.
@@ -132,3 +136,48 @@ def dd_chebyshev_filter(op, X: np.ndarray, nslabs: int, m: int, a: float, b: flo
     rounded to binary32 on their way across a cut."""
     from .fe_oracle import chebyshev_filter
     return chebyshev_filter(lambda V: dd_apply(op, V, nslabs, fp32_payload=fp32_payload), X, m, a, b, a0)
+
+
+# ---- Eq. 17 in full: the constraint matrices inside the decomposed apply ----------------------------------------------
+
+def restrict_sets(sets, rows: np.ndarray):
+    """C^(t): the global constraint sets (oracle/constraints_oracle.ConstraintSet, global row indices) restricted to the
+    local rows of a task.  A set takes part in task t if one of its slaves is a local row; then ALL its slaves and
+    masters must be local rows (the locally dense sets of PAPER.md:290 live on one face / edge; a set that straddles a cut
+    would need masters the task does not hold) -- otherwise ValueError.  A global row on a cut plane is local to two tasks:
+    both get the set."""
+    from .constraints_oracle import ConstraintSet
+    pos = {}
+    for k, r in enumerate(rows):                      # a single periodic task holds plane 0 twice (first plane and ghost plane)
+        pos.setdefault(int(r), []).append(k)
+    out = []
+    for I in sets:
+        here = [int(s) in pos for s in I.slaves]
+        if not any(here):
+            continue
+        nodes = [int(v) for v in np.concatenate([I.masters, I.slaves])]
+        if not all(v in pos for v in nodes):
+            raise ValueError("a constraint set straddles a subdomain boundary")
+        copies = {len(pos[v]) for v in nodes}
+        if len(copies) != 1:
+            raise ValueError("a constraint set mixes rows the task holds once and rows it holds twice")
+        for c in range(copies.pop()):                 # one local set per copy
+            out.append(ConstraintSet([pos[int(m_)][c] for m_ in I.masters], [pos[int(s)][c] for s in I.slaves], I.W, I.b))
+    return out
+
+
+def dd_constrained_apply(op, X: np.ndarray, nslabs: int, sets) -> np.ndarray:
+    """Eq. 17:  V = sum_t P^(t)T C^(t)T ( sum_{e in E_t} Q^T A^(e) Q ) C^(t) P^(t) U, the homogeneous part
+    of the constraints (an operator apply).  Step by step per task: extract owned + ghost rows, distribute, the local cell
+    loop, distribute-transpose, add into the global rows."""
+    from .constraints_oracle import distribute, distribute_transpose
+    m = op.mesh
+    X = np.asarray(X, dtype=np.float64)
+    V = np.zeros_like(X)
+    for (z0, z1) in slab_layers(m.ncells[2], nslabs):
+        rows, _ = slab_rows(m, z0, z1)
+        loc = restrict_sets(sets, rows)
+        U_loc = distribute(loc, X[rows], homogeneous=True)
+        V_loc = distribute_transpose(loc, slab_apply(op, z0, z1, U_loc))
+        np.add.at(V, rows, V_loc)
+    return V

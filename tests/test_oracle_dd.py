@@ -144,3 +144,46 @@ def test_decomposed_chebyshev_filter_is_the_single_domain_filter(bc):
     dev = np.abs(Y32 - Y).max() / np.abs(Y).max()
     assert 1e-10 < dev < 1e-4                                           # FP32 roundoff per step, not FP64, not O(1)
     assert np.array_equal(ddo.dd_chebyshev_filter(op, X, 1, m, a, b, a0, fp32_payload=True), ddo.dd_chebyshev_filter(op, X, 1, m, a, b, a0))
+
+
+def plane_local_sets(mesh, rng, nsets_per_plane=2, planes=None):
+    """Closed constraint sets whose nodes all lie in ONE node plane each (so that no set straddles a z-cut): per chosen
+    plane a master-less set (a "hole" pinned to zero) and sets with 2-4 masters and 1-3 slaves."""
+    from oracle import constraints_oracle as co
+    ndx, ndy, ndz = mesh.nd
+    plane = ndx * ndy
+    sets = []
+    for iz in (range(ndz) if planes is None else planes):
+        nodes = iz * plane + rng.permutation(plane)
+        k = 0
+        sets.append(co.ConstraintSet([], nodes[k:k + 2], np.zeros((2, 0)), None)); k += 2
+        for _ in range(nsets_per_plane):
+            nm, ns = int(rng.integers(2, 5)), int(rng.integers(1, 4))
+            sets.append(co.ConstraintSet(nodes[k:k + nm], nodes[k + nm:k + nm + ns], rng.uniform(-1, 1, (ns, nm)), None))
+            k += nm + ns
+    return sets
+
+
+@pytest.mark.parametrize("bc", ["periodic", "dirichlet"])
+def test_equation_17_in_full_constraints_inside_the_decomposed_apply(bc):
+    """sum_t P^T C_t^T A_t C_t P U = C^T A C U for sets that live inside node planes -- the cut planes included, whose
+    sets belong to two tasks -- and a set that straddles a cut is refused."""
+    from oracle import constraints_oracle as co
+    p, nc = 2, (2, 3, 4)
+    mesh = orc.Mesh(nc, p, bc, (0.0, 0.0, 0.0), (1.0, 1.2, 2.0))
+    op = orc.Operator(mesh, 0.7)
+    rng = np.random.default_rng(17)
+    sets = plane_local_sets(mesh, rng)
+    X = rng.uniform(-1, 1, (mesh.ndof, 3))
+    Y = co.distribute_transpose(sets, op.apply(co.distribute(sets, X, homogeneous=True)))
+    assert np.abs(Y - op.apply(X)).max() > 1e-3 * np.abs(Y).max()          # the constraints matter
+    for ns in (1, 2, 4):
+        Yd = ddo.dd_constrained_apply(op, X, ns, sets)
+        assert np.abs(Yd - Y).max() <= 1e-13 * np.abs(Y).max(), ns
+    # a set that straddles a cut: master in plane 5, slave in plane 1, both nodes otherwise unconstrained
+    plane = mesh.nd[0] * mesh.nd[1]
+    used = set(int(v) for I in sets for v in np.concatenate([I.masters, I.slaves]))
+    free5 = next(r for r in range(5 * plane, 6 * plane) if r not in used)
+    free1 = next(r for r in range(plane, 2 * plane) if r not in used)
+    with pytest.raises(ValueError):
+        ddo.dd_constrained_apply(op, X, 4, sets + [co.ConstraintSet([free5], [free1], [[0.5]], None)])
