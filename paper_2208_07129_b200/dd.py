@@ -53,6 +53,7 @@ class SlabPlan:
     p: int
     periodic: bool
     plane_nodes: int                 # nd_x * nd_y
+    ncz_total: int = 0               # cell layers of the whole mesh (make_plan sets it; needed by restrict_sets only)
 
     @property
     def nplanes(self) -> int:        # planes of the local multivector (owned + the top plane)
@@ -89,7 +90,45 @@ class SlabPlan:
 def make_plan(ncells: Sequence[int], p: int, periodic: bool, nslabs: int, rank: int) -> SlabPlan:
     z0, z1 = slab_layers(ncells[2], nslabs)[rank]
     add = 0 if periodic else 1
-    return SlabPlan(rank, nslabs, z0, z1, p, periodic, (ncells[0] * p + add) * (ncells[1] * p + add))
+    return SlabPlan(rank, nslabs, z0, z1, p, periodic, (ncells[0] * p + add) * (ncells[1] * p + add), ncells[2])
+
+
+def restrict_sets(sets, plan: SlabPlan):
+    """C^(t) of Eq. 17: constraint sets given in GLOBAL node indices -- tuples (masters, slaves, W, b) as
+    constraints.Constraints takes them -- restricted to the local rows of task `plan` (host-side index marshalling).  A set
+    takes part if one of its slaves is a local row; then all its nodes must be local rows, else ValueError (a set that
+    straddles a cut would need masters the task does not hold).  A row on a cut plane is local to two tasks, and a single
+    periodic task holds plane 0 twice (first plane and ghost plane): one local set per copy."""
+    if plan.ncz_total <= 0:
+        raise ValueError("restrict_sets needs a plan from make_plan (ncz_total)")
+    ndz = plan.ncz_total * plan.p + (0 if plan.periodic else 1)
+    local_planes = {}
+    for l in range(plan.nplanes):
+        g = plan.z0 * plan.p + l
+        local_planes.setdefault(g % ndz if plan.periodic else g, []).append(l)
+    pn = plan.plane_nodes
+    out = []
+    for (masters, slaves, W, b) in sets:
+        masters = [int(v) for v in masters]
+        slaves = [int(v) for v in slaves]
+        if not any(v // pn in local_planes for v in slaves):
+            continue
+        nodes = masters + slaves
+        if not all(v // pn in local_planes for v in nodes):
+            raise ValueError("a constraint set straddles a subdomain boundary")
+        copies = {len(local_planes[v // pn]) for v in nodes}
+        if len(copies) != 1:
+            raise ValueError("a constraint set mixes rows the task holds once and rows it holds twice")
+        for c in range(copies.pop()):
+            loc = lambda v: local_planes[v // pn][c] * pn + v % pn      # noqa: E731
+            out.append(([loc(v) for v in masters], [loc(v) for v in slaves], W, b))
+    return out
+
+
+def device_constraints(sets, plan: SlabPlan, device: int = 0):
+    """The task's constraint object on the device (include/fe_constraints.h) from sets in global node indices."""
+    from . import constraints
+    return constraints.Constraints(plan.nplanes * plan.plane_nodes, restrict_sets(sets, plan), device)
 
 
 def slab_geometry(w, plan: SlabPlan):
@@ -131,17 +170,24 @@ def _buffers32(like, pe: int, count: int):
 
 
 def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, scratch=None, fp32_payload: bool = False,
-                  scratch32=None):
+                  scratch32=None, constraints=None):
     """One task of the decomposed apply with torch.distributed point-to-point messages (dist = torch.distributed).
     U_loc / V_loc: flat tensors of nplanes * plane_nodes * nvec doubles; the ghost plane of U_loc is overwritten.
     `scratch`: one plane, receives the neighbour's ghost plane of V.  fp32_payload: the planes travel as FP32
-    (`scratch32`: two float32 planes, the send and the receive buffer)."""
+    (`scratch32`: two float32 planes, the send and the receive buffer).  constraints: the task's C^(t) (an object with
+    distribute(U, nvec, homogeneous=True) and distribute_transpose(V, nvec): constraints.Constraints from
+    device_constraints) -- Eq. 17 in full, V = sum_t P^T C^T A C P U; the slave rows of U_loc are then overwritten by their
+    constrained values."""
     pe = plan.plane_nodes * nvec
     own = plan.n_owned_planes * pe
     if plan.nslabs == 1:                       # a single periodic task is its own neighbour
         if plan.has_ghost:
             U_loc[own:own + pe].copy_(U_loc[:pe])
+        if constraints is not None:
+            constraints.distribute(U_loc, nvec, homogeneous=True)
         ops.apply(U_loc, V_loc, nvec)
+        if constraints is not None:
+            constraints.distribute_transpose(V_loc, nvec)
         if plan.has_ghost:
             ops.halo_add(V_loc[:pe], V_loc[own:own + pe])
         return V_loc
@@ -157,7 +203,11 @@ def dd_apply_rank(plan: SlabPlan, ops: LocalOps, U_loc, V_loc, nvec: int, dist, 
         r.wait()
     if fp32_payload and plan.up is not None:
         ops.unpack_f32(U_loc[own:own + pe], r32, False)
+    if constraints is not None:                # C^(t)
+        constraints.distribute(U_loc, nvec, homogeneous=True)
     ops.apply(U_loc, V_loc, nvec)
+    if constraints is not None:                # C^(t)T
+        constraints.distribute_transpose(V_loc, nvec)
     # P^(t)T: ghost plane of V goes up, the neighbour's comes from below and is added into the first plane
     if scratch is None and not fp32_payload:
         scratch = V_loc.new_empty(pe)
@@ -327,9 +377,10 @@ class SlabGroup:
             out[first * pe:(first + pl.n_owned_planes) * pe].copy_(V[:pl.n_owned_planes * pe])
         return out
 
-    def apply(self, U_locs, V_locs, nvec: int, fp32_payload: bool = False):
+    def apply(self, U_locs, V_locs, nvec: int, fp32_payload: bool = False, constraints=None):
         """V^(t) for every task, ghost planes exchanged and added: on return the owned planes of V_locs hold A U.
-        fp32_payload: every plane that crosses a task boundary goes through an FP32 message buffer (pack / unpack)."""
+        fp32_payload: every plane that crosses a task boundary goes through an FP32 message buffer (pack / unpack).
+        constraints: one C^(t) per task (see dd_apply_rank): the owned planes then hold C^T A C U."""
         plans = self.plans
         fp32 = fp32_payload and self.nslabs > 1
         if fp32:
@@ -343,8 +394,12 @@ class SlabGroup:
                     self.ops[pl.rank].unpack_f32(U[own:own + pe], m32, False)
                 else:
                     U[own:own + pe].copy_(U_locs[pl.up][:pe])
-        for o, U, V in zip(self.ops, U_locs, V_locs):         # A^(t)
+        for t, (o, U, V) in enumerate(zip(self.ops, U_locs, V_locs)):     # C^(t)T A^(t) C^(t)
+            if constraints is not None:
+                constraints[t].distribute(U, nvec, homogeneous=True)
             o.apply(U, V, nvec)
+            if constraints is not None:
+                constraints[t].distribute_transpose(V, nvec)
         # P^(t)T: every first plane is final after the local applies only in its OWN task's sum, so the adds are
         # independent of one another (a task's ghost plane is never another add's destination)
         for pl, V in zip(plans, V_locs):

@@ -268,3 +268,116 @@ def test_cheb_steps_are_algorithm_6():
         assert abs(y - ref) <= 1e-14 * abs(ref)
     with pytest.raises(ValueError):
         list(dd.cheb_steps(3, 2.0, 1.0, 0.0))
+
+
+# ---- Eq. 17 in full: constraints inside the decomposed apply --------------------------------------------------------
+
+class _OracleConstraints:
+    """Stand-in for constraints.Constraints (host logic tests only): the oracle's C, C^T on the local sets."""
+
+    def __init__(self, local_sets):
+        from oracle import constraints_oracle as co
+        self.co, self.sets = co, [co.ConstraintSet(m, s, W, b) for (m, s, W, b) in local_sets]
+
+    def distribute(self, U, nvec, homogeneous=False):
+        U.copy_(torch.from_numpy(self.co.distribute(self.sets, U.numpy().reshape(-1, nvec), homogeneous=homogeneous).reshape(-1)))
+
+    def distribute_transpose(self, V, nvec):
+        V.copy_(torch.from_numpy(self.co.distribute_transpose(self.sets, V.numpy().reshape(-1, nvec)).reshape(-1)))
+
+
+def _plane_sets(w, seed=17):
+    """Closed sets in global node indices, every set inside one node plane (tuples as constraints.Constraints takes them)."""
+    rng = np.random.default_rng(seed)
+    plane = w.nd[0] * w.nd[1]
+    sets = []
+    for iz in range(w.nd[2]):
+        nodes = iz * plane + rng.permutation(plane)
+        sets.append(([], nodes[:2], np.zeros((2, 0)), None))
+        sets.append((nodes[2:5], nodes[5:7], rng.uniform(-1, 1, (2, 3)), None))
+    return sets
+
+
+def _constrained_reference(w, sets, X):
+    from oracle import constraints_oracle as co
+    bcs = "periodic" if w.bc == inputs.BC_PERIODIC else "dirichlet"
+    op = orc.Operator(orc.Mesh(w.ncells, w.p, bcs, w.box_lo, w.box_hi), w.sigma)
+    S = [co.ConstraintSet(m, s, W, b) for (m, s, W, b) in sets]
+    return co.distribute_transpose(S, op.apply(co.distribute(S, X, homogeneous=True)))
+
+
+def _worker_constrained(rank, world, port, bc, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = _workload(bc)
+        nvec = w.nvec
+        plan = dd.make_plan(w.ncells, w.p, bc == inputs.BC_PERIODIC, world, rank)
+        cons = _OracleConstraints(dd.restrict_sets(_plane_sets(w), plan))
+        X = inputs.multivector(w.seed, w.ndof, nvec)
+        pe = plan.plane_nodes * nvec
+        first = plan.z0 * plan.p
+        U = torch.full((plan.nplanes * pe,), float("nan"), dtype=torch.float64)
+        U[:plan.n_owned_planes * pe] = torch.from_numpy(X.reshape(-1)[first * pe:(first + plan.n_owned_planes) * pe].copy())
+        V = torch.full_like(U, float("nan"))
+        dd.dd_apply_rank(plan, _oracle_ops(w, plan), U, V, nvec, dist, constraints=cons)
+        q.put((rank, plan.z0, plan.n_owned_planes, V[:plan.n_owned_planes * pe].numpy().copy()))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+def test_constrained_decomposed_apply_over_gloo(bc):
+    world = 2
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker_constrained, args=(r, world, port, bc, q)) for r in range(world)]
+    for p in procs: p.start()
+    res = sorted((q.get(timeout=240) for _ in range(world)), key=lambda r: r[0])
+    for p in procs: p.join(timeout=60)
+    assert all(p.exitcode == 0 for p in procs)
+    w = _workload(bc)
+    X = inputs.multivector(w.seed, w.ndof, w.nvec)
+    Y = _constrained_reference(w, _plane_sets(w), X)
+    plane = w.nd[0] * w.nd[1] * w.nvec
+    for rank, z0, nown, Vown in res:
+        ref = Y.reshape(-1)[z0 * w.p * plane:(z0 * w.p + nown) * plane]
+        assert np.abs(Vown - ref).max() <= 1e-13 * np.abs(Y).max(), rank
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_DIRICHLET])
+@pytest.mark.parametrize("nslabs", [1, 3, 5])
+def test_slab_group_constrained_apply_single_process(bc, nslabs):
+    """nslabs = 1 on the periodic mesh: the task holds plane 0 twice and gets the sets of that plane twice."""
+    w = _workload(bc)
+    nvec = w.nvec
+    sets = _plane_sets(w)
+    grp = dd.SlabGroup(w, nslabs, make_ops=_oracle_ops)
+    cons = [_OracleConstraints(dd.restrict_sets(sets, pl)) for pl in grp.plans]
+    X = inputs.multivector(w.seed, w.ndof, nvec)
+    Xt = torch.from_numpy(X.reshape(-1).copy())
+    U = grp.scatter(Xt, nvec)
+    V = [torch.full_like(u, float("nan")) for u in U]
+    grp.apply(U, V, nvec, constraints=cons)
+    out = grp.gather(V, nvec, torch.full_like(Xt, float("nan")))
+    Y = _constrained_reference(w, sets, X)
+    assert np.abs(out.numpy().reshape(Y.shape) - Y).max() <= 1e-13 * np.abs(Y).max()
+
+
+def test_restrict_sets_bookkeeping():
+    w = _workload(inputs.BC_DIRICHLET)                      # (2, 2, 5) cells, p = 3: 16 node planes
+    plane = w.nd[0] * w.nd[1]
+    plans = [dd.make_plan(w.ncells, w.p, False, 2, t) for t in range(2)]       # layers [0,3) and [3,5): the cut is plane 9
+    on_cut = ([9 * plane + 1], [9 * plane + 2], [[1.0]], None)
+    below = ([2 * plane], [2 * plane + 3], [[1.0]], None)
+    for pl, expect in zip(plans, ([(9, 9), (2, 2)], [(0, 0)])):
+        loc = dd.restrict_sets([on_cut, below], pl)
+        assert [(m[0] // plane, s[0] // plane) for (m, s, _, _) in loc] == expect       # local plane numbers
+    with pytest.raises(ValueError):                          # master above the cut, slave below it
+        dd.restrict_sets([([12 * plane], [3 * plane], [[1.0]], None)], plans[0])
+    with pytest.raises(ValueError):
+        dd.restrict_sets([on_cut], dd.SlabPlan(0, 2, 0, 3, 3, False, plane))   # a hand-made plan without ncz_total
+    per = dd.make_plan((2, 2, 5), 3, True, 1, 0)             # a single periodic task: plane 0 twice
+    loc = dd.restrict_sets([([1], [2], [[1.0]], None)], per)
+    assert [(m[0], s[0]) for (m, s, _, _) in loc] == [(1, 2), (15 * per.plane_nodes + 1, 15 * per.plane_nodes + 2)]
